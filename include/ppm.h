@@ -1,0 +1,116 @@
+/*
+ * ppm.h — C ABI of the B200-native PPM+PPB timestep library (libppm_b200.so).
+ *
+ * One hot path of arxiv/paper_1810_13416 (Woodward et al.): the directionally split 3-D PPM
+ * gas-dynamics timestep fused with PPB ten-moment advection of the fractional volume FV
+ * (BASELINE.json north_star, which also names this call
+ * list).  The numerical definition of every step is SURVEY.md section 8(c) (H0-H9, P1-P4, C1-C7),
+ * restated in DESIGN.md.  All arithmetic on the device is fp32, one GPU, no CPU
+ * fallback: every entry point fails with PPM_ECUDA if no sm_100 device / kernel image is usable.
+ *
+ * Conventions
+ *  - plain C types only; every call returns a status code, never throws or aborts.
+ *  - NULL / size / non-paired-periodic / dt <= 0 / unknown order -> PPM_EINVAL, no side effects.
+ *  - CUDA failures -> PPM_ECUDA; text kept for ppm_last_error().
+ *  - ppm_step only enqueues kernels on the context's stream; a sticky device flag (NaN, or a
+ *    density/pressure floor was hit) is reported as PPM_ESTATE by the next synchronising call
+ *    (ppm_cfl_dt, ppm_reduce_conserved, ppm_get_state, ppm_sync).
+ *  - pointers marked [host] / [device] say where the memory lives; pointers passed in arrays
+ *    (fields[]) are borrowed for the duration of the call only.
+ *
+ * State: 15 fp32 fields per cell, each a dense [nz][ny][nx] array, x fastest (SoA planes):
+ *   0 rho  1 ux  2 uy  3 uz  4 p   5..14 = m000 m100 m010 m001 m200 m020 m002 m110 m101 m011
+ * where m_abc are the coefficients of FV in the cell-local Legendre basis P0=1, P1=s, P2=s^2-1/12
+ * on [-1/2,1/2]^3 (m000 = cell mean; "cell average and its 9 lowest-order moments").
+ * Internally rho and p are stored as perturbations to the hydrostatic base state.
+ */
+#ifndef PPM_B200_H
+#define PPM_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ppm_ctx ppm_ctx; /* opaque; owns only small device scratch (tables, reduction cells) */
+
+enum { PPM_OK = 0, PPM_EINVAL = 1, PPM_ENOMEM = 2, PPM_ECUDA = 3, PPM_ESTATE = 4 };
+enum { PPM_BC_PERIODIC = 0, PPM_BC_REFLECT = 1 }; /* per face: xlo,xhi,ylo,yhi,zlo,zhi; periodic must pair up */
+enum { PPM_GRAV_NONE = 0, PPM_GRAV_CONST_Z = 1, PPM_GRAV_RADIAL = 2 };
+#define PPM_NFIELDS 15
+#define PPM_NGHOST 4 /* stencil reach per sweep */
+
+/* "Gravity profile": the acceleration AND the hydrostatic base state it balances.
+ * Node k sits at s = s0 + k*ds.  Point values are linear interpolations between nodes.
+ *  CONST_Z: s = z, acceleration g(z) along +z.  The table MUST have n = 2*(nz+8)+1 nodes with
+ *           s0 = -4*dx, ds = dx/2, so that every cell centre and face is a node (else PPM_EINVAL).
+ *  RADIAL : s = r = |X - center|, acceleration g(r) * (X - center)/r.
+ * g, rho0, p0: [host] arrays of n floats, copied by ppm_create (fp32 on purpose: the oracle and
+ * the GPU must see bit-identical nodes). */
+typedef struct {
+    int kind; /* PPM_GRAV_* */
+    int n;
+    double s0, ds;
+    double center[3];
+    const float *g, *rho0, *p0;
+} ppm_gravity;
+
+typedef struct {
+    size_t struct_size; /* = sizeof(ppm_params); checked */
+    int nx, ny, nz;     /* cells; each >= 1 */
+    double dx;          /* cubic cells; cell (i,j,k) is centred at ((i+.5)dx, (j+.5)dx, (k+.5)dx) */
+    double gamma;       /* ideal-gas adiabatic index, > 1 */
+    double rho_floor, p_floor; /* > 0 */
+    ppm_gravity grav;
+    int bc[6];
+    void *stream; /* cudaStream_t the library enqueues on (0 = default stream) */
+} ppm_params;
+
+/* Creates a context.  dev_buf_a, dev_buf_b: [device] two caller-owned buffers of
+ * 15*nx*ny*nz floats each, 16-byte aligned (e.g. torch tensors).  The library BORROWS them for the
+ * life of the context: the state lives in one, the other is sweep scratch, and they ping-pong.  It
+ * never frees them.  Contents are undefined until ppm_set_state has covered every z-slab. */
+int ppm_create(ppm_ctx **out, const ppm_params *prm, float *dev_buf_a, float *dev_buf_b);
+
+/* Loads the full state (rho, ux, uy, uz, p, m000..m011) for z-planes [z0, z0+nz_slab).
+ * fields[f]: [host] array of 15 pointers, each to a dense [nz_slab][ny][nx] float array that lives on
+ * the host (src_is_device = 0) or on the device (src_is_device = 1).  Converts rho, p to
+ * perturbation form (rho' = rho - rho0 at the cell centre, formed in fp64, rounded once to fp32;
+ * SURVEY 8(c) C1).  Asynchronous w.r.t. the host only if the sources are device or pinned memory. */
+int ppm_set_state(ppm_ctx *ctx, const float *const fields[PPM_NFIELDS], int z0, int nz_slab, int src_is_device);
+
+/* Inverse of ppm_set_state; synchronises the stream before returning. */
+int ppm_get_state(ppm_ctx *ctx, float *const fields[PPM_NFIELDS], int z0, int nz_slab, int dst_is_device);
+
+/* One timestep = three 1-D sweeps (ghost fill, PPM hydro, PPB remap fused) with the same dt.
+ * sweep_order 0..5 = xyz, xzy, yxz, yzx, zxy, zyx.  Only enqueues work (3 kernel launches). */
+int ppm_step(ppm_ctx *ctx, double dt, int sweep_order);
+
+/* One sweep along axis d (0,1,2) — the unit ppm_step is made of; exposed for per-sweep parity tests. */
+int ppm_sweep(ppm_ctx *ctx, double dt, int axis);
+
+/* dt = cfl*dx / max over cells of max_d(|u_d|) + c.  Synchronises the stream.  dt_out: [host]. */
+int ppm_cfl_dt(ppm_ctx *ctx, double cfl, double *dt_out);
+
+/* out[6] [host] = mass, momentum x, y, z, total energy, tracked mass (sum rho*m000), each * dx^3;
+ * fp64 accumulation in a fixed order (deterministic).  Synchronises the stream. */
+int ppm_reduce_conserved(ppm_ctx *ctx, double out[6]);
+
+/* Waits for the stream and reports the sticky state flag (PPM_OK / PPM_ESTATE / PPM_ECUDA). */
+int ppm_sync(ppm_ctx *ctx);
+
+/* Tuning knob for benchmarks: cells marched per thread along the sweep axis before the pencil is
+ * split into another chunk (0 = library default).  Results do not depend on it. */
+int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
+
+/* Number of kernel launches the context has enqueued so far (bench.py reports it). */
+long long ppm_launch_count(const ppm_ctx *ctx);
+
+void ppm_destroy(ppm_ctx *ctx);
+const char *ppm_last_error(const ppm_ctx *ctx); /* never NULL; "" if no error; ctx may be NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PPM_B200_H */

@@ -174,49 +174,40 @@ double oracle_h5_Fminus(double ql, double qr, double qi, double sigma) {
 void oracle_h6_trace(const double ql[5], const double qr[5], const double qi[5], double rho, double c,
                      double dtdx, const double src[3], double WL[5], double WR[5]) {
     const double u = qi[1];
-    const double lam_m = u - c, lam_0 = u, lam_p = u + c;
-    const double s_m = lam_m * dtdx, s_0 = lam_0 * dtdx, s_p = lam_p * dtdx;
+    const double s_m = (u - c) * dtdx, s_0 = u * dtdx, s_p = (u + c) * dtdx;   /* sigma^k = lambda^k dt/dx */
     const double c2 = c * c;
 #define FP(k, s) oracle_h5_Fplus(ql[k], qr[k], qi[k], (s))
 #define FM(k, s) oracle_h5_Fminus(ql[k], qr[k], qi[k], (s))
-    {   /* left of face i+1/2 */
+    {   /* left of face i+1/2: reference = average over the fastest wave toward the face (u + c) */
         double sp = fmax(s_p, 0.0);
         double rt = FP(0, sp), ut = FP(1, sp), pt = FP(4, sp);
-        double am = 0.0, a0 = 0.0;
-        if (lam_m > 0.0) {
-            double dr = rt - FP(0, s_m), du = ut - FP(1, s_m), dp = pt - FP(4, s_m);
-            (void)dr;
-            am = (dp - rho * c * du) / (2.0 * c2);
-        }
-        if (lam_0 > 0.0) {
-            double dr = rt - FP(0, s_0), dp = pt - FP(4, s_0);
-            a0 = dr - dp / c2;
-        }
+        /* family k in {-, 0}: its own domain of dependence max(sigma^k, 0); a wave that moves AWAY from
+         * the face has the zero-width domain F+(.;0) = q_R (reading R8': no hard switch on
+         * the sign of lambda^k, so the traced state is a continuous function of the data) */
+        double smk = fmax(s_m, 0.0), s0k = fmax(s_0, 0.0);
+        double du = ut - FP(1, smk), dp = pt - FP(4, smk);
+        double am = (dp - rho * c * du) / (2.0 * c2);
+        double dr0 = rt - FP(0, s0k), dp0 = pt - FP(4, s0k);
+        double a0 = dr0 - dp0 / c2;
         WL[0] = rt - am - a0;
         WL[1] = ut + (c / rho) * am;
         WL[4] = pt - c2 * am;
-        double s0p = fmax(s_0, 0.0);
-        WL[2] = FP(2, s0p);
-        WL[3] = FP(3, s0p);
+        WL[2] = FP(2, s0k);
+        WL[3] = FP(3, s0k);
     }
-    {   /* right of face i-1/2 */
+    {   /* right of face i-1/2: reference = average over the domain of u - c */
         double sm = fmax(-s_m, 0.0);
         double rt = FM(0, sm), ut = FM(1, sm), pt = FM(4, sm);
-        double ap = 0.0, a0 = 0.0;
-        if (lam_p < 0.0) {
-            double du = ut - FM(1, -s_p), dp = pt - FM(4, -s_p);
-            ap = (dp + rho * c * du) / (2.0 * c2);
-        }
-        if (lam_0 < 0.0) {
-            double dr = rt - FM(0, -s_0), dp = pt - FM(4, -s_0);
-            a0 = dr - dp / c2;
-        }
+        double spk = fmax(-s_p, 0.0), s0k = fmax(-s_0, 0.0);
+        double du = ut - FM(1, spk), dp = pt - FM(4, spk);
+        double ap = (dp + rho * c * du) / (2.0 * c2);
+        double dr0 = rt - FM(0, s0k), dp0 = pt - FM(4, s0k);
+        double a0 = dr0 - dp0 / c2;
         WR[0] = rt - ap - a0;
         WR[1] = ut - (c / rho) * ap;
         WR[4] = pt - c2 * ap;
-        double s0m = fmax(-s_0, 0.0);
-        WR[2] = FM(2, s0m);
-        WR[3] = FM(3, s0m);
+        WR[2] = FM(2, s0k);
+        WR[3] = FM(3, s0k);
     }
 #undef FP
 #undef FM

@@ -1,0 +1,199 @@
+// ppm_api.cu — the C ABI declared in include/ppm.h (host driver; argument validation, launches).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "ppm_internal.h"
+
+static char g_err[512] = "";
+
+static void set_err(ppm_ctx* c, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c ? c->err : g_err, 512, fmt, ap);
+    va_end(ap);
+}
+
+#define CU(call)                                                                            \
+    do {                                                                                    \
+        cudaError_t e_ = (call);                                                            \
+        if (e_ != cudaSuccess) {                                                            \
+            set_err(c, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return PPM_ECUDA;                                                               \
+        }                                                                                   \
+    } while (0)
+
+static const int ORDERS[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+
+extern "C" const char* ppm_last_error(const ppm_ctx* c) { return c ? c->err : g_err; }
+
+extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a, float* dev_buf_b) {
+    ppm_ctx* c = nullptr;
+    if (!out) { set_err(c, "ppm_create: out is NULL"); return PPM_EINVAL; }
+    *out = nullptr;
+    if (!prm || !dev_buf_a || !dev_buf_b || dev_buf_a == dev_buf_b) { set_err(c, "ppm_create: NULL or aliased argument"); return PPM_EINVAL; }
+    if (prm->struct_size != sizeof(ppm_params)) { set_err(c, "ppm_create: struct_size %zu != %zu", prm->struct_size, sizeof(ppm_params)); return PPM_EINVAL; }
+    if (prm->nx < 1 || prm->ny < 1 || prm->nz < 1) { set_err(c, "ppm_create: grid dims must be >= 1"); return PPM_EINVAL; }
+    if (!(prm->dx > 0.0) || !(prm->gamma > 1.0) || !(prm->rho_floor > 0.0) || !(prm->p_floor > 0.0)) {
+        set_err(c, "ppm_create: need dx > 0, gamma > 1, floors > 0"); return PPM_EINVAL;
+    }
+    if (((uintptr_t)dev_buf_a | (uintptr_t)dev_buf_b) & 15) { set_err(c, "ppm_create: device buffers must be 16-byte aligned"); return PPM_EINVAL; }
+    const int ext[3] = {prm->nx, prm->ny, prm->nz};
+    for (int d = 0; d < 3; ++d) {
+        const int lo = prm->bc[2 * d], hi = prm->bc[2 * d + 1];
+        if ((lo != PPM_BC_PERIODIC && lo != PPM_BC_REFLECT) || (hi != PPM_BC_PERIODIC && hi != PPM_BC_REFLECT)) {
+            set_err(c, "ppm_create: unknown boundary type on axis %d", d); return PPM_EINVAL;
+        }
+        if ((lo == PPM_BC_PERIODIC) != (hi == PPM_BC_PERIODIC)) { set_err(c, "ppm_create: periodic faces must pair up (axis %d)", d); return PPM_EINVAL; }
+        if (lo == PPM_BC_REFLECT && ext[d] < PPM_NGHOST) { set_err(c, "ppm_create: reflecting axis %d needs >= %d cells", d, PPM_NGHOST); return PPM_EINVAL; }
+    }
+    const ppm_gravity& g = prm->grav;
+    if (g.kind != PPM_GRAV_NONE && g.kind != PPM_GRAV_CONST_Z && g.kind != PPM_GRAV_RADIAL) { set_err(c, "ppm_create: unknown gravity kind"); return PPM_EINVAL; }
+    if (g.kind != PPM_GRAV_NONE) {
+        if (g.n < 2 || !g.g || !g.rho0 || !g.p0 || !(g.ds > 0.0)) { set_err(c, "ppm_create: gravity table missing"); return PPM_EINVAL; }
+        if (g.kind == PPM_GRAV_CONST_Z) {
+            const double tol = 1e-9 * prm->dx;
+            if (g.n != 2 * (prm->nz + 2 * PPM_NGHOST) + 1 || fabs(g.s0 + PPM_NGHOST * prm->dx) > tol || fabs(g.ds - 0.5 * prm->dx) > tol) {
+                set_err(c, "ppm_create: CONST_Z table must have n = 2*(nz+8)+1 nodes, s0 = -4 dx, ds = dx/2"); return PPM_EINVAL;
+            }
+        }
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { set_err(c, "ppm_create: no CUDA device (this library has no CPU fallback)"); return PPM_ECUDA; }
+
+    c = (ppm_ctx*)calloc(1, sizeof(ppm_ctx));
+    if (!c) { set_err(nullptr, "ppm_create: out of host memory"); return PPM_ENOMEM; }
+    c->prm = *prm;
+    c->prm.grav.g = c->prm.grav.rho0 = c->prm.grav.p0 = nullptr;   // host arrays are not kept
+    c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0;
+    c->stream = (cudaStream_t)prm->stream;
+    c->nblocks_red = 148 * 4;
+    c->chunk = 0;
+    c->err[0] = 0;
+    cudaError_t e;
+#define CUC(call) do { e = (call); if (e != cudaSuccess) { set_err(nullptr, "%s failed: %s", #call, cudaGetErrorString(e)); ppm_destroy(c); return e == cudaErrorMemoryAllocation ? PPM_ENOMEM : PPM_ECUDA; } } while (0)
+    CUC(cudaMalloc(&c->flag, sizeof(int)));
+    CUC(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
+    CUC(cudaMalloc(&c->cflmax, sizeof(unsigned int)));
+    CUC(cudaMalloc(&c->partial, sizeof(double) * 6 * c->nblocks_red));
+    CUC(cudaMalloc(&c->result, sizeof(double) * 6));
+    if (g.kind != PPM_GRAV_NONE) {
+        std::vector<float4> t32(g.n);
+        std::vector<double> t64(3 * (size_t)g.n);
+        for (int k = 0; k < g.n; ++k) {
+            t32[k] = make_float4(g.g[k], g.rho0[k], g.p0[k], 0.f);
+            t64[3 * k] = g.g[k]; t64[3 * k + 1] = g.rho0[k]; t64[3 * k + 2] = g.p0[k];
+        }
+        CUC(cudaMalloc(&c->tab, sizeof(float4) * g.n));
+        CUC(cudaMalloc(&c->tab64, sizeof(double) * 3 * g.n));
+        CUC(cudaMemcpy(c->tab, t32.data(), sizeof(float4) * g.n, cudaMemcpyHostToDevice));
+        CUC(cudaMemcpy(c->tab64, t64.data(), sizeof(double) * 3 * g.n, cudaMemcpyHostToDevice));
+    }
+#undef CUC
+    *out = c;
+    return PPM_OK;
+}
+
+extern "C" void ppm_destroy(ppm_ctx* c) {
+    if (!c) return;
+    cudaFree(c->flag); cudaFree(c->cflmax); cudaFree(c->partial); cudaFree(c->result);
+    cudaFree(c->tab); cudaFree(c->tab64);
+    free(c);
+}
+
+static int check_slab(ppm_ctx* c, const void* fields, int z0, int nzs, const char* who) {
+    if (!c) { set_err(nullptr, "%s: ctx is NULL", who); return PPM_EINVAL; }
+    if (!fields) { set_err(c, "%s: fields is NULL", who); return PPM_EINVAL; }
+    if (z0 < 0 || nzs < 1 || z0 + nzs > c->prm.nz) { set_err(c, "%s: slab [%d,%d) outside [0,%d)", who, z0, z0 + nzs, c->prm.nz); return PPM_EINVAL; }
+    return PPM_OK;
+}
+
+static int read_flag(ppm_ctx* c) {
+    int f = 0;
+    CU(cudaMemcpyAsync(&f, c->flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (f) { set_err(c, "state flag %d: %s", f, (f & 2) ? "NaN or non-positive density/pressure" : "density/pressure floor hit"); return PPM_ESTATE; }
+    return PPM_OK;
+}
+
+extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS], int z0, int nzs, int src_is_device) {
+    int rc = check_slab(c, fields, z0, nzs, "ppm_set_state");
+    if (rc) return rc;
+    for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_set_state: fields[%d] is NULL", f); return PPM_EINVAL; }
+    const long long plane = (long long)c->prm.nx * c->prm.ny, ncell = plane * c->prm.nz;
+    float* st = c->buf[c->cur];
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int f = 0; f < PPM_NFIELDS; ++f)
+        CU(cudaMemcpyAsync(st + f * ncell + z0 * plane, fields[f], sizeof(float) * plane * nzs, kind, c->stream));
+    CU(ppm_launch_to_perturbation(c, st, z0, nzs));
+    CU(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
+    return PPM_OK;
+}
+
+extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z0, int nzs, int dst_is_device) {
+    int rc = check_slab(c, fields, z0, nzs, "ppm_get_state");
+    if (rc) return rc;
+    for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_get_state: fields[%d] is NULL", f); return PPM_EINVAL; }
+    const long long plane = (long long)c->prm.nx * c->prm.ny, tot = plane * nzs;
+    float* scratch = c->buf[c->cur ^ 1];    // free between steps
+    CU(ppm_launch_to_full(c, c->buf[c->cur], scratch, z0, nzs));
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    for (int f = 0; f < PPM_NFIELDS; ++f)
+        CU(cudaMemcpyAsync(fields[f], scratch + f * tot, sizeof(float) * tot, kind, c->stream));
+    return read_flag(c);
+}
+
+extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
+    if (!c) { set_err(nullptr, "ppm_sweep: ctx is NULL"); return PPM_EINVAL; }
+    if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "ppm_sweep: need finite dt > 0 and axis in 0..2"); return PPM_EINVAL; }
+    CU(ppm_launch_sweep(c, axis, dt));
+    return PPM_OK;
+}
+
+extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
+    if (!c) { set_err(nullptr, "ppm_step: ctx is NULL"); return PPM_EINVAL; }
+    if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_step: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
+    for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt));
+    return PPM_OK;
+}
+
+extern "C" int ppm_cfl_dt(ppm_ctx* c, double cfl, double* dt_out) {
+    if (!c) { set_err(nullptr, "ppm_cfl_dt: ctx is NULL"); return PPM_EINVAL; }
+    if (!dt_out || !(cfl > 0.0)) { set_err(c, "ppm_cfl_dt: need cfl > 0 and dt_out"); return PPM_EINVAL; }
+    CU(ppm_launch_cfl(c));
+    unsigned int enc = 0;
+    CU(cudaMemcpyAsync(&enc, c->cflmax, sizeof(enc), cudaMemcpyDeviceToHost, c->stream));
+    int rc = read_flag(c);
+    if (rc) return rc;
+    float vmax;
+    memcpy(&vmax, &enc, sizeof(float));
+    if (!(vmax > 0.f)) { set_err(c, "ppm_cfl_dt: max signal speed is not positive"); return PPM_ESTATE; }
+    *dt_out = cfl * c->prm.dx / (double)vmax;
+    return PPM_OK;
+}
+
+extern "C" int ppm_reduce_conserved(ppm_ctx* c, double out[6]) {
+    if (!c) { set_err(nullptr, "ppm_reduce_conserved: ctx is NULL"); return PPM_EINVAL; }
+    if (!out) { set_err(c, "ppm_reduce_conserved: out is NULL"); return PPM_EINVAL; }
+    CU(ppm_launch_conserved(c));
+    CU(cudaMemcpyAsync(out, c->result, sizeof(double) * 6, cudaMemcpyDeviceToHost, c->stream));
+    return read_flag(c);
+}
+
+extern "C" int ppm_sync(ppm_ctx* c) {
+    if (!c) { set_err(nullptr, "ppm_sync: ctx is NULL"); return PPM_EINVAL; }
+    return read_flag(c);
+}
+
+extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
+    if (!c) { set_err(nullptr, "ppm_set_chunk: ctx is NULL"); return PPM_EINVAL; }
+    if (chunk_cells < 0) { set_err(c, "ppm_set_chunk: chunk_cells must be >= 0"); return PPM_EINVAL; }
+    c->chunk = chunk_cells;
+    return PPM_OK;
+}
+
+extern "C" long long ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }

@@ -197,14 +197,24 @@ def test_h6_entropy_wave_is_scalar_ppm_advection():
         assert WR[1] == pytest.approx(u, abs=1e-15) and WR[4] == pytest.approx(0.5, abs=1e-15)
         if u > 0:
             assert WL[0] == pytest.approx((P(0.5) - P(0.5 - s)) / s, abs=1e-12)
-            # the contact moves away from the left face: no correction, so the state is C&W's reference
-            # average over the domain of the fastest wave toward that face (u - c)
-            sm = (1.0 - u) * dtdx
-            assert WR[0] == pytest.approx((P(-0.5 + sm) - P(-0.5)) / sm, abs=1e-12)
+            # the contact moves away from the left face: its amplitude there is the edge value
+            # (zero-width domain of dependence; reading R8')
+            assert WR[0] == pytest.approx(rl, abs=1e-12)
         else:
             assert WR[0] == pytest.approx((P(-0.5 + s) - P(-0.5)) / s, abs=1e-12)
-            sp = (1.0 + u) * dtdx
-            assert WL[0] == pytest.approx((P(0.5) - P(0.5 - sp)) / sp, abs=1e-12)
+            assert WL[0] == pytest.approx(rr, abs=1e-12)
+
+
+def test_h6_is_continuous_across_the_sign_changes_of_the_characteristic_speeds():
+    # reading R8': no hard switch on sign(lambda^k) -> traced states are continuous in u
+    ql = np.array([0.9, 0.1, 0.3, -0.2, 0.8]); qr = np.array([1.2, -0.1, 0.1, 0.2, 1.1])
+    for u0 in (0.0, 1.0, -1.0):          # contact, and the two sonic points (c = 1)
+        outs = []
+        for eps in (-1e-9, 1e-9):
+            qi = 0.5 * (ql + qr) + np.array([0.02, 0, 0, 0, -0.03])
+            qi[1] = u0 + eps
+            outs.append(np.concatenate(ob.h6_trace(ql, qr, qi, 1.3, 1.0, 0.6)))
+        assert np.max(np.abs(outs[0] - outs[1])) < 1e-8
 
 
 def test_h6_acoustic_wave_uses_plus_characteristic_domain():
