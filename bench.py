@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py — cell-updates/s of the fused PPM+PPB timestep on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4|5|...] [--impl reference]
+
+A "step" is one ppm_step = the whole hot path (three fused hydro+PPB sweeps) over the
+whole synthetic grid.  value = cells * K / device time (CUDA events, max over ranks), inputs resident in
+HBM.  e2e = the same metric through the C ABI with pinned HOST buffers: ppm_set_state(host) + ppm_step +
+ppm_get_state(host) inside the timed region.  Multi-GPU: the path is "replicas only": each
+rank advances its own grid, no data-path collective; value sums the ranks' cells ("weak" scaling).
+
+--impl reference times the fp64 CPU oracle (as it stands) on a bounded window of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1810_13416_b200 import workloads as W  # noqa: E402
+
+METRIC = "cell-updates/s per 3-D PPM+PPB step (fp32); achieved HBM GB/s vs peak"
+UNIT = "cell-updates/s"
+BYTES_PER_CELL_SWEEP = 120.0      # 15 fp32 fields read + written by every sweep
+FLOPS_PER_CELL_SWEEP = 1409.0     # static count of the oracle's sweep body, FMA = 2
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md)
+# dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` capture
+# (profiles/), keyed by cells per side; None where no capture exists.
+NCU_TRAFFIC_BYTES = {}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return 6650.0, "fallback"
+
+
+def _dist():
+    ws = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    lr = int(os.environ.get("LOCAL_RANK", "0"))
+    return ws, rank, lr
+
+
+class _Clocks:
+    """samples nvidia-smi clocks / throttle reasons of one GPU while the timed region runs"""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, idx):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(idx), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+        return out
+
+
+def _load_state(g, w, nzs):
+    n = w.n
+    for z0 in range(0, n, nzs):
+        z1 = min(n, z0 + nzs)
+        g.set_state(w.fields((0, 0, z0), (n, n, z1), device=g.device), z0=z0)
+
+
+def _sample_window(w, side):
+    """central window of the workload used for the oracle timings"""
+    side = min(side, w.n)
+    lo = [(w.n - side) // 2] * 3
+    hi = [lo[0] + side] * 3
+    bc = [w.bc[k] if side == w.n else 2 for k in range(6)]
+    return lo, hi, bc
+
+
+def _time_oracle(w, side, steps, warmup):
+    from oracle import binding as ob          # bench.py's cpu_baseline / reference legs may use oracle/
+    lo, hi, bc = _sample_window(w, side)
+    f = w.fields(lo, hi).numpy()
+    o = ob.Oracle(hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], w.dx, w.gamma, bc, w.grav, org=lo,
+                  rho_floor=w.rho_floor, p_floor=w.p_floor)
+    o.set_state(f)
+    dt = 0.5 * o.cfl_dt(w.cfl)
+    for s in range(warmup):
+        o.step(dt, 0 if s % 2 == 0 else 5)
+    t0 = time.perf_counter()
+    for s in range(steps):
+        o.step(dt, 0 if s % 2 == 0 else 5)
+    t = time.perf_counter() - t0
+    cells = (hi[0] - lo[0]) ** 3
+    return cells * steps / t, t / steps, ob.num_threads(), "central %d^3 window of %s, %d steps" % (hi[0] - lo[0], w.name, steps)
+
+
+def run_reference(args):
+    ws, rank, _ = _dist()
+    if rank != 0:
+        return 0
+    w = W.make(args.workload)
+    val, sps, cores, sample = _time_oracle(w, args.ref_side, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s %d^3 (oracle on a bounded window)" % (w.name, w.n), "cfl": w.cfl},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_gpu(args):
+    ws, rank, lr = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the PPM+PPB path has no CPU fallback")
+    torch.cuda.set_device(lr)
+    dev = torch.device("cuda", lr)
+    if ws > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1810_13416_b200.binding import PPM, NF
+
+    w = W.make(args.workload)
+    n = w.n
+    ncell = n ** 3
+    g = PPM.from_workload(w, device=dev)
+    if args.chunk:
+        g.set_chunk(args.chunk)
+    _load_state(g, w, 8 if n >= 1024 else 32)
+    dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
+
+    def barrier():
+        if ws > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    for s in range(Wm):
+        g.step(dt, 0 if s % 2 == 0 else 5)
+    barrier()
+    clk = _Clocks(lr)
+    l0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(g.stream)
+    for s in range(K):
+        g.step(dt, 0 if s % 2 == 0 else 5)
+    e1.record(g.stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count() - l0
+    clocks = clk.stop()
+    g.sync()                         # raises if the state flag (NaN / floor) was set
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        try:
+            Ke = args.e2e_steps
+            host_in = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
+            host_out = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
+            g.get_state(out=host_in)
+            g.set_state(host_in); g.step(dt, 0); g.get_state(out=host_out)      # warm-up
+            barrier()
+            t0 = time.perf_counter()
+            for s in range(Ke):
+                g.set_state(host_in)
+                g.step(dt, 0 if s % 2 == 0 else 5)
+                g.get_state(out=host_out)       # synchronises
+                host_in, host_out = host_out, host_in
+            torch.cuda.synchronize()
+            te = time.perf_counter() - t0
+            e2e = {"ms": te * 1e3 / Ke, "steps": Ke, "bytes": NF * ncell * 4}
+            del host_in, host_out
+        except Exception as ex:                                                  # e.g. not enough pinned host memory
+            e2e = {"error": str(ex)[:200]}
+
+    # ---- reduce over ranks ----
+    if ws > 1:
+        t = torch.tensor([ms, e2e["ms"] if e2e and "ms" in e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+        if e2e and "ms" in e2e:
+            e2e["ms"] = float(t[1])
+    if rank != 0:
+        if ws > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peak, peak_kind = _peaks()
+    value = ws * ncell * K / (ms * 1e-3)
+    per_launch_s = ms * 1e-3 / max(launches, 1)
+    achieved = BYTES_PER_CELL_SWEEP * ncell / per_launch_s / 1e9
+    alu = FLOPS_PER_CELL_SWEEP * ncell / per_launch_s / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": Wm,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "%s %d^3, %s, dt fixed at 0.7*CFL dt, sweep order xyz/zyx alternating" % (w.name, n, "reflecting walls + radial gravity" if w.grav else "periodic"),
+                   "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (NF * ncell * 4 / 1e9),
+                   "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": NCU_TRAFFIC_BYTES.get(n), "peak_kind": "of " + peak_kind,
+                     "kernel": "ppm_sweep_kernel (3 launches per step; every launch moves 120 B/cell)",
+                     "alu": {"achieved": alu, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu / FP32_PEAK_TFLOPS,
+                             "flops_per_cell_sweep": FLOPS_PER_CELL_SWEEP}},
+        "clocks": clocks, "gpu_launches": int(launches),
+    }
+    if e2e and "ms" in e2e:
+        line["e2e"] = {"value": ws * ncell / (e2e["ms"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["bytes"],
+                       "d2h_bytes_per_step": e2e["bytes"], "steps": e2e["steps"], "ms_per_step": e2e["ms"]}
+    else:
+        line["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                       "note": (e2e or {}).get("error", "skipped")}
+    if ws == 1 and not args.no_cpu_baseline:
+        val, _, cores, sample = _time_oracle(w, args.ref_side, 2, 0)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    print(json.dumps(line))
+    if ws > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number (4 = 512^3, 5 = 1024^3)")
+    ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

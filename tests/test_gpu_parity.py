@@ -1,0 +1,244 @@
+"""GPU-vs-oracle parity through the C ABI (libppm_b200.so) — `pytest -m gpu` on a B200.
+
+Bars (BASELINE.json north_star; norms in tests/parity_norms.py):
+  max relative error per variable <= 1e-5 after one step, <= 1e-4 after the config's step count on smooth
+  flows; L1 error <= 1e-4 on the shock config; conserved totals within 1e-6 relative; dt within 1e-6.
+Every input comes from the seeded generators in paper_1810_13416_b200.workloads; no expected value comes
+from the CUDA path.  Full-size configs (128^3 .. 1024^3) are checked on oracle WINDOWS: the update reaches 4
+cells per axis per step, so a window plus a 4*steps apron regenerated from the input formulas reproduces the
+global result on the window exactly (tests/test_oracle_invariants.py::test_window_reproduces_full_grid).
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1810_13416_b200 import workloads as W
+
+from parity_norms import conserved_rel, l1_rel, max_rel, merge_scales
+
+pytestmark = pytest.mark.gpu
+
+ONE_STEP, MULTI_STEP, L1_SHOCK, CONS, DT_TOL = 1e-5, 1e-4, 1e-4, 1e-6, 1e-6
+
+
+def _gpu():
+    from paper_1810_13416_b200.binding import PPM       # loads libppm_b200.so; raises if missing
+    return PPM
+
+
+def _oracle(w, n=None, org=(0, 0, 0), bc=None):
+    from oracle import binding as ob
+    n = n or (w.n, w.n, w.n)
+    return ob.Oracle(n[0], n[1], n[2], w.dx, w.gamma, bc or w.bc, w.grav, org=org, rho_floor=w.rho_floor, p_floor=w.p_floor)
+
+
+def _load(g, w, device="cuda", nzs=32):
+    n = w.n
+    for z0 in range(0, n, nzs):
+        z1 = min(n, z0 + nzs)
+        g.set_state(w.fields((0, 0, z0), (n, n, z1), device=device), z0=z0)
+
+
+def _run_pair(w, steps, chunk=0, check_each=()):
+    """steps on both sides with the GPU's dt; returns dict of results after step 1 and at the end."""
+    PPM = _gpu()
+    f = w.fields()
+    o = _oracle(w)
+    o.set_state(f.numpy())
+    g = PPM.from_workload(w)
+    if chunk:
+        g.set_chunk(chunk)
+    g.set_state(f.cuda())
+    out = {}
+    c0g, c0o = g.reduce_conserved(), o.reduce_conserved()
+    full0 = o.get_state()
+    out["cons0"] = conserved_rel(c0g, c0o, full0, w.dx, w.gamma)
+    for s in range(steps):
+        dt = g.cfl_dt(w.cfl)
+        assert abs(dt - o.cfl_dt(w.cfl)) <= DT_TOL * dt
+        order = 0 if s % 2 == 0 else 5
+        g.step(dt, order)
+        o.step(dt, order)
+        if s == 0 or s + 1 == steps or (s + 1) in check_each:
+            gs = g.get_state().cpu().numpy().astype(np.float64)
+            os_ = o.get_state()
+            out[s + 1] = (max_rel(gs, os_), l1_rel(gs, os_))
+    out["cons1"] = conserved_rel(g.reduce_conserved(), o.reduce_conserved(), o.get_state(), w.dx, w.gamma)
+    out["drift_gpu"] = np.abs(g.reduce_conserved() - c0g)
+    out["c0"] = c0g
+    out["final"] = (gs, os_)
+    g.close()
+    return out
+
+
+# ---------------------------------------------------------------- config 1: the full config -----------
+def test_cfg1_full_32cubed_20_steps():
+    w = W.make(1)
+    r = _run_pair(w, w.steps)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[w.steps][0].values()) <= MULTI_STEP, r[w.steps][0]
+    assert r["cons0"].max() <= CONS and r["cons1"].max() <= CONS
+    # the scheme is conservative on the periodic box: mass, energy, tracked mass drift only by fp32 round-off
+    c0, d = r["c0"], r["drift_gpu"]
+    assert d[0] <= 2e-6 * c0[0] and d[4] <= 2e-6 * c0[4] and d[5] <= 2e-6 * c0[5]
+    fv = r["final"][0][5]
+    assert fv.min() >= 0.0 and fv.max() <= 1.0
+
+
+@pytest.mark.parametrize("chunk", [8, 13])
+def test_pencil_chunking_does_not_change_results(chunk):
+    PPM = _gpu()
+    w = W.make(1)
+    f = w.fields().cuda()
+    res = []
+    for ch in (0, chunk):
+        g = PPM.from_workload(w)
+        g.set_chunk(ch)
+        g.set_state(f)
+        for s in range(2):
+            g.step(0.02, s * 5)
+        res.append(g.get_state().cpu().numpy())
+        g.close()
+    assert np.array_equal(res[0], res[1])
+
+
+# ---------------------------------------------------------------- reduced-size, full step counts ------
+def test_cfg2_stratified_reduced_64_100_steps():
+    w = W.make(2, n=64)
+    r = _run_pair(w, 100)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[100][0].values()) <= MULTI_STEP, r[100][0]
+    assert r["cons1"].max() <= CONS
+
+
+def test_cfg3_blast_reduced_64_50_steps_L1():
+    w = W.make(3, n=64)
+    r = _run_pair(w, 50)
+    assert max(r[1][1].values()) <= L1_SHOCK, r[1][1]
+    assert max(r[50][1].values()) <= L1_SHOCK, r[50][1]
+    assert r["cons1"].max() <= CONS
+    gs, os_ = r["final"]
+    assert np.abs(os_[1:4]).max() > 3.0           # the Mach ~3 blast really ran
+    assert gs[5].min() >= 0.0 and gs[5].max() <= 1.0
+
+
+def test_cfg4_convection_reduced_64_20_steps():
+    w = W.make(4, n=64)
+    r = _run_pair(w, 20)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[20][0].values()) <= MULTI_STEP, r[20][0]
+    assert r["cons1"].max() <= CONS
+
+
+def test_ragged_grid_all_boundaries_and_orders():
+    """nx, ny, nz not multiples of anything (ragged tails of every tile), mixed boundaries, all six orders."""
+    PPM = _gpu()
+    from oracle import binding as ob
+    rng = np.random.default_rng(11)
+    nx, ny, nz = 37, 29, 23
+    f = np.zeros((15, nz, ny, nx), dtype=np.float32)
+    f[0] = 1.0 + 0.3 * rng.random((nz, ny, nx))
+    f[1:4] = 0.2 * rng.normal(size=(3, nz, ny, nx))
+    f[4] = 0.8 + 0.3 * rng.random((nz, ny, nx))
+    f[5] = 0.2 + 0.6 * rng.random((nz, ny, nx))
+    f[6:] = 0.02 * rng.normal(size=(9, nz, ny, nx))
+    P_, R_ = 0, 1
+    for bc in ((P_, P_, R_, R_, P_, P_), (R_, R_, P_, P_, R_, R_)):
+        o = ob.Oracle(nx, ny, nz, 0.03, 1.4, bc, None)
+        g = PPM(nx, ny, nz, 0.03, 1.4, bc)
+        o.set_state(f)
+        g.set_state(f)
+        for order in range(6):
+            dt = 0.4 * g.cfl_dt(0.8)
+            g.step(dt, order)
+            o.step(dt, order)
+        e = max_rel(g.get_state().cpu().numpy().astype(np.float64), o.get_state())
+        assert max(e.values()) <= MULTI_STEP, e
+        g.close()
+
+
+def test_hydrostatic_state_is_preserved_exactly_on_gpu():
+    PPM = _gpu()
+    for cfg, n in ((2, 32), (4, 32)):
+        w = W.make(cfg, n=n)
+        f = w.fields()
+        f[1:4] = 0.0
+        g = PPM.from_workload(w)
+        g.set_state(f.cuda())
+        s0 = g.get_state().cpu().numpy()
+        for s in range(3):
+            g.step(0.8 * w.dx, s)
+        s1 = g.get_state().cpu().numpy()
+        if cfg == 2:      # rho', p' are exactly 0: bit-for-bit well-balanced
+            assert np.array_equal(s0[:5], s1[:5])
+        else:             # rho', p' = fp32 rounding of the input (~3e-8): only that noise evolves
+            assert np.abs(s1[1:4]).max() < 2e-7 and np.abs(s1[0] - s0[0]).max() < 3e-7
+        g.close()
+
+
+# ---------------------------------------------------------------- full-size configs on windows --------
+def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max"):
+    PPM = _gpu()
+    w = W.make(cfg)
+    n = w.n
+    g = PPM.from_workload(w)
+    _load(g, w, nzs=nzs_load)
+    dts = []
+    for s in range(steps):
+        dt = g.cfl_dt(w.cfl)
+        dts.append(dt)
+        g.step(dt, 0 if s % 2 == 0 else 5)
+    g.sync()
+    apron = 4 * steps
+    worst = {}
+    pairs = []
+    for (c, size) in windows:
+        lo = [max(0, c[d] - size // 2 - apron) for d in range(3)]
+        hi = [min(n, c[d] + size // 2 + apron) for d in range(3)]
+        bc = []
+        for d in range(3):
+            bc += [w.bc[2 * d] if lo[d] == 0 and (w.bc[2 * d] == 1 or hi[d] == n) else 2,
+                   w.bc[2 * d + 1] if hi[d] == n and (w.bc[2 * d + 1] == 1 or lo[d] == 0) else 2]
+        o = _oracle(w, n=[hi[d] - lo[d] for d in range(3)], org=lo, bc=bc)
+        o.set_state(w.fields(lo, hi, device="cuda").cpu().numpy())
+        for s, dt in enumerate(dts):
+            o.step(dt, 0 if s % 2 == 0 else 5)
+        os_ = o.get_state()
+        # interior of the window: drop the apron on OPEN sides only
+        sl = [slice(apron if bc[2 * d] == 2 else 0, (hi[d] - lo[d]) - (apron if bc[2 * d + 1] == 2 else 0)) for d in range(3)]
+        zs = slice(lo[2] + sl[2].start, lo[2] + sl[2].stop)
+        gs = g.get_state(z0=zs.start, nzs=zs.stop - zs.start).cpu().numpy().astype(np.float64)
+        gs = gs[:, :, lo[1] + sl[1].start:lo[1] + sl[1].stop, lo[0] + sl[0].start:lo[0] + sl[0].stop]
+        os_ = os_[:, sl[2], sl[1], sl[0]]
+        pairs.append((gs, os_))
+    g.close()
+    scale = merge_scales([o_ for _, o_ in pairs])      # a window in a quiescent region has no scale of its own
+    for gs, os_ in pairs:
+        e = max_rel(gs, os_, scale) if norm == "max" else l1_rel(gs, os_)
+        for k, v in e.items():
+            worst[k] = max(worst.get(k, 0.0), v)
+    assert max(worst.values()) <= tol, worst
+    return worst
+
+
+def test_cfg2_full_128_windows():
+    n = 128
+    _window_check(2, 2, [((64, 64, 64), 24), ((64, 64, 77), 24), ((10, 64, 4), 24), ((64, 120, 124), 24)])
+
+
+def test_cfg3_full_256_windows_L1():
+    _window_check(3, 2, [((128, 128, 128), 32), ((128, 128, 100), 24), ((8, 8, 8), 24)], tol=L1_SHOCK, norm="l1")
+
+
+def test_cfg4_full_512_windows():
+    c = 256
+    r45 = int(0.45 * 512)
+    _window_check(4, 2, [((c, c, c), 24), ((c + 170, c, c), 24), ((c, c + r45, c), 24), ((c, c, c + int(0.48 * 512)), 24),
+                         ((c, 6, c), 24), ((6, 6, 6), 24)])
+
+
+@pytest.mark.skipif(not torch.cuda.is_available() or torch.cuda.get_device_properties(0).total_memory < 150e9,
+                    reason="1024^3 needs ~129 GB of HBM")
+def test_cfg5_full_1024_windows():
+    c = 512
+    _window_check(5, 1, [((c, c, c), 24), ((c + 340, c, c), 24), ((c, c + int(0.45 * 1024), c), 24), ((6, 6, 6), 24)], nzs_load=8)

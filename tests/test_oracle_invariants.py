@@ -326,3 +326,32 @@ def test_window_reproduces_full_grid():
     gf = full.get_state()[:, lo[2] + a:hi[2], lo[1] + a:hi[1] - a, lo[0]:hi[0] - a]
     gw = win.get_state()[:, a:, a:-a, :-a]
     assert np.array_equal(gf, gw)
+
+
+# ---------------------------------------------------------------- parity floor of an fp32 state ----
+def test_fp32_state_storage_sets_the_parity_floor():
+    """Evidence for DESIGN.md reading R20a.  Run the fp64 oracle twice on config 1, once rounding the STATE to
+    fp32 after every sweep (the state is fp32) and nothing else.  The hydro variables and FV
+    (scaled by max |m000|) stay ~1e-6 apart, but a coefficient that is ~0 by symmetry moves by >1e-5 of its
+    own maximum — so 'relative to the field's own maximum' is not a usable norm for the ten coefficients."""
+    from parity_norms import max_rel
+    w = W.make(1)
+    f = w.fields().numpy()
+    A = ob.Oracle(w.n, w.n, w.n, w.dx, w.gamma, w.bc, None)
+    B = ob.Oracle(w.n, w.n, w.n, w.dx, w.gamma, w.bc, None)
+    A.set_state(f)
+    B.set_state(f)
+    orders = [(0, 1, 2), (2, 1, 0)]
+    for s in range(5):
+        dt = A.cfl_dt(0.8)
+        A.step(dt, 0 if s % 2 == 0 else 5)
+        for d in orders[s % 2]:
+            B.sweep(d, dt)
+            for k in range(15):
+                r = B.raw_field(k)
+                r[:] = r.astype(np.float32).astype(np.float64)
+    a, b = A.get_state(), B.get_state()
+    e = max_rel(b, a)
+    assert max(e.values()) < 5e-6
+    own = max(np.abs(b[k] - a[k]).max() / np.abs(a[k]).max() for k in range(6, 15))
+    assert own > 1e-5
