@@ -18,7 +18,8 @@
  *  - pointers marked [host] / [device] say where the memory lives; pointers passed in arrays
  *    (fields[]) are borrowed for the duration of the call only.
  *
- * State: 15 fp32 fields per cell, each a dense [nz][ny][nx] array, x fastest (SoA planes):
+ * State at the boundary (ppm_set_state / ppm_get_state): 15 fp32 fields per cell, each a dense [nz][ny][nx]
+ * array, x fastest.  Inside the two borrowed buffers the library keeps them as SoA bricks.
  *   0 rho  1 ux  2 uy  3 uz  4 p   5..14 = m000 m100 m010 m001 m200 m020 m002 m110 m101 m011
  * where m_abc are the coefficients of FV in the cell-local Legendre basis P0=1, P1=s, P2=s^2-1/12
  * on [-1/2,1/2]^3 (m000 = cell mean; "cell average and its 9 lowest-order moments").
@@ -103,6 +104,17 @@ int ppm_sync(ppm_ctx *ctx);
 /* Tuning knob for benchmarks: cells marched per thread along the sweep axis before the pencil is
  * split into another chunk (0 = library default).  Results do not depend on it. */
 int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
+
+/* Options (results do not depend on them).
+ *  PPM_OPT_X_PATH : 0 = automatic (brick layout: the x sweep stages whole 256-byte bricks through shared
+ *                   memory with TMA), 1 = force the direct global-memory path.
+ *  PPM_OPT_LAYOUT : internal layout of the two borrowed buffers; 0 = automatic (SoA bricks of 4x4x4 cells
+ *                   when nx, ny, nz are multiples of 4, SoA planes otherwise), 1 = force SoA planes.  Only
+ *                   before the first ppm_set_state. */
+enum { PPM_OPT_X_PATH = 1, PPM_OPT_LAYOUT = 2 };
+int ppm_set_option(ppm_ctx *ctx, int option, int value);
+/* 1 if the next x sweep will take the TMA-staged path, 0 if the direct path. */
+int ppm_x_path(const ppm_ctx *ctx);
 
 /* Number of kernel launches the context has enqueued so far (bench.py reports it). */
 long long ppm_launch_count(const ppm_ctx *ctx);

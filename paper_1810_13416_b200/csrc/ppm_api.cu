@@ -65,8 +65,10 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { set_err(c, "ppm_create: no CUDA device (this library has no CPU fallback)"); return PPM_ECUDA; }
 
-    c = (ppm_ctx*)calloc(1, sizeof(ppm_ctx));
-    if (!c) { set_err(nullptr, "ppm_create: out of host memory"); return PPM_ENOMEM; }
+    void* mem = nullptr;
+    if (posix_memalign(&mem, 64, sizeof(ppm_ctx)) != 0 || !mem) { set_err(nullptr, "ppm_create: out of host memory"); return PPM_ENOMEM; }
+    memset(mem, 0, sizeof(ppm_ctx));
+    c = (ppm_ctx*)mem;
     c->prm = *prm;
     c->prm.grav.g = c->prm.grav.rho0 = c->prm.grav.p0 = nullptr;   // host arrays are not kept
     c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0;
@@ -74,6 +76,9 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c->nblocks_red = 148 * 4;
     c->chunk = 0;
     c->err[0] = 0;
+    // SoA bricks of 4x4x4 cells when every extent is a multiple of 4 (every sweep direction then touches
+    // whole 256-byte bricks); SoA planes otherwise
+    c->layout = (prm->nx % 4 == 0 && prm->ny % 4 == 0 && prm->nz % 4 == 0) ? 1 : 0;
     cudaError_t e;
 #define CUC(call) do { e = (call); if (e != cudaSuccess) { set_err(nullptr, "%s failed: %s", #call, cudaGetErrorString(e)); ppm_destroy(c); return e == cudaErrorMemoryAllocation ? PPM_ENOMEM : PPM_ECUDA; } } while (0)
     CUC(cudaMalloc(&c->flag, sizeof(int)));
@@ -94,6 +99,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
         CUC(cudaMemcpy(c->tab64, t64.data(), sizeof(double) * 3 * g.n, cudaMemcpyHostToDevice));
     }
 #undef CUC
+    ppm_make_xmaps(c);      // x-sweep TMA path when nx % 4 == 0; otherwise the direct path serves all three axes
     *out = c;
     return PPM_OK;
 }
@@ -126,10 +132,14 @@ extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS],
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_set_state: fields[%d] is NULL", f); return PPM_EINVAL; }
     const long long plane = (long long)c->prm.nx * c->prm.ny, ncell = plane * c->prm.nz;
     float* st = c->buf[c->cur];
+    float* scratch = c->buf[c->cur ^ 1];    // free between steps: stages the dense slab
+    (void)ncell;
+    const long long tot = plane * nzs;
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     for (int f = 0; f < PPM_NFIELDS; ++f)
-        CU(cudaMemcpyAsync(st + f * ncell + z0 * plane, fields[f], sizeof(float) * plane * nzs, kind, c->stream));
-    CU(ppm_launch_to_perturbation(c, st, z0, nzs));
+        CU(cudaMemcpyAsync(scratch + f * tot, fields[f], sizeof(float) * tot, kind, c->stream));
+    CU(ppm_launch_to_perturbation(c, scratch, st, z0, nzs));
+    c->layout_locked = 1;
     CU(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
     return PPM_OK;
 }
@@ -195,5 +205,22 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
     c->chunk = chunk_cells;
     return PPM_OK;
 }
+
+extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
+    if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
+    if (option == PPM_OPT_X_PATH && (value == 0 || value == 1)) { c->force_direct = value; return PPM_OK; }
+    if (option == PPM_OPT_LAYOUT && (value == 0 || value == 1)) {
+        if (c->layout_locked) { set_err(c, "ppm_set_option: the layout cannot change once a state is loaded"); return PPM_EINVAL; }
+        const ppm_params& p = c->prm;
+        if (value == 0 && (p.nx % 4 || p.ny % 4 || p.nz % 4)) { set_err(c, "ppm_set_option: bricks need extents that are multiples of 4"); return PPM_EINVAL; }
+        c->layout = value == 0 ? 1 : 0;
+        ppm_make_xmaps(c);
+        return PPM_OK;
+    }
+    set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
+    return PPM_EINVAL;
+}
+
+extern "C" int ppm_x_path(const ppm_ctx* c) { return (c && c->tma_ok && !c->force_direct) ? 1 : 0; }
 
 extern "C" long long ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }

@@ -11,7 +11,30 @@ struct AuxParams {
     int grav_kind, tab_n;
     double s0, ds, cx, cy, cz;
     const double* __restrict__ tab64;   // node k: g, rho0, p0 (3 doubles)
+    int layout, nbx, nby;               // 1 = 4x4x4 bricks (all extents multiples of 4)
 };
+
+// storage offset of cell (i,j,k) inside one field
+__device__ __forceinline__ long long cell_offset(const AuxParams& A, int i, int j, int k) {
+    if (A.layout == 0) return ((long long)k * A.ny + j) * A.nx + i;
+    return ((((long long)(k >> 2) * A.nby + (j >> 2)) * A.nbx + (i >> 2)) << 6) + ((k & 3) << 4 | (j & 3) << 2 | (i & 3));
+}
+// inverse: storage index t (0 .. ncell) -> (i,j,k); both layouts are dense (no padding)
+__device__ __forceinline__ void cell_of(const AuxParams& A, long long t, int& i, int& j, int& k) {
+    if (A.layout == 0) {
+        const long long plane = (long long)A.nx * A.ny;
+        k = (int)(t / plane);
+        const long long rem = t % plane;
+        j = (int)(rem / A.nx); i = (int)(rem % A.nx);
+    } else {
+        const int c = (int)(t & 63);
+        long long B = t >> 6;
+        const int bx = (int)(B % A.nbx); B /= A.nbx;
+        const int by = (int)(B % A.nby);
+        const int bz = (int)(B / A.nby);
+        i = bx * 4 + (c & 3); j = by * 4 + ((c >> 2) & 3); k = bz * 4 + (c >> 4);
+    }
+}
 
 // fp64 base state at a cell centre (same definition as the sweep's, evaluated in double: the
 // conversion full <-> perturbation must not add fp32 error of the size of the base state)
@@ -33,18 +56,23 @@ __device__ __forceinline__ void base64(const AuxParams& A, int i, int j, int k, 
     }
 }
 
-// in place: rho <- rho - rho0c, p <- p - p0c on z-planes [z0, z0+nzs)
-__global__ void __launch_bounds__(256) to_perturbation_kernel(AuxParams A, float* __restrict__ st, int z0, int nzs) {
+// state (layout order, perturbation form) <- dense slab [15][nzs][ny][nx] of full values, z-planes [z0, z0+nzs)
+__global__ void __launch_bounds__(256) to_perturbation_kernel(AuxParams A, const float* __restrict__ src, float* __restrict__ st, int z0, int nzs) {
     const long long plane = (long long)A.nx * A.ny, tot = plane * nzs;
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
         const int k = z0 + (int)(t / plane);
         const long long rem = t % plane;
         const int j = (int)(rem / A.nx), i = (int)(rem % A.nx);
-        const long long id = (long long)k * plane + rem;
+        const long long id = cell_offset(A, i, j, k);
         double r0, p0;
         base64(A, i, j, k, r0, p0);
-        st[id] = (float)((double)st[id] - r0);
-        st[4 * A.ncell + id] = (float)((double)st[4 * A.ncell + id] - p0);
+#pragma unroll
+        for (int f = 0; f < PPM_NFIELDS; ++f) {
+            float v = src[f * tot + t];
+            if (f == 0) v = (float)((double)v - r0);
+            if (f == 4) v = (float)((double)v - p0);
+            st[f * A.ncell + id] = v;
+        }
     }
 }
 
@@ -55,7 +83,7 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
         const int k = z0 + (int)(t / plane);
         const long long rem = t % plane;
         const int j = (int)(rem / A.nx), i = (int)(rem % A.nx);
-        const long long id = (long long)k * plane + rem;
+        const long long id = cell_offset(A, i, j, k);
         double r0, p0;
         base64(A, i, j, k, r0, p0);
 #pragma unroll
@@ -72,13 +100,11 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
 __device__ __forceinline__ unsigned int enc(float x) { return __float_as_uint(fmaxf(x, 0.f)); }
 
 __global__ void __launch_bounds__(256) cfl_kernel(AuxParams A, const float* __restrict__ st, unsigned int* __restrict__ out, int* flag) {
-    const long long plane = (long long)A.nx * A.ny;
     float vmax = 0.f;
     const float gam = (float)A.gamma;
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.ncell; t += (long long)gridDim.x * blockDim.x) {
-        const int k = (int)(t / plane);
-        const long long rem = t % plane;
-        const int j = (int)(rem / A.nx), i = (int)(rem % A.nx);
+        int i, j, k;
+        cell_of(A, t, i, j, k);
         double r0, p0;
         base64(A, i, j, k, r0, p0);
         const float rho = (float)(r0 + (double)st[t]), p = (float)(p0 + (double)st[4 * A.ncell + t]);
@@ -103,12 +129,10 @@ __global__ void __launch_bounds__(256) cfl_kernel(AuxParams A, const float* __re
 
 // conserved sums: fp64 accumulation, fixed assignment of cells to threads, fixed reduction trees
 __global__ void __launch_bounds__(256) conserved_kernel(AuxParams A, const float* __restrict__ st, double* __restrict__ partial) {
-    const long long plane = (long long)A.nx * A.ny;
     double acc[6] = {0, 0, 0, 0, 0, 0};
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.ncell; t += (long long)gridDim.x * blockDim.x) {
-        const int k = (int)(t / plane);
-        const long long rem = t % plane;
-        const int j = (int)(rem / A.nx), i = (int)(rem % A.nx);
+        int i, j, k;
+        cell_of(A, t, i, j, k);
         double r0, p0;
         base64(A, i, j, k, r0, p0);
         const double rho = r0 + (double)st[t], p = p0 + (double)st[4 * A.ncell + t];
@@ -150,6 +174,7 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.s0 = p.grav.s0; A.ds = p.grav.ds;
     A.cx = p.grav.center[0]; A.cy = p.grav.center[1]; A.cz = p.grav.center[2];
     A.tab64 = c->tab64;
+    A.layout = c->layout; A.nbx = (p.nx + 3) / 4; A.nby = (p.ny + 3) / 4;
     return A;
 }
 
@@ -162,9 +187,9 @@ int grid_for(long long n, int cap) {
 
 }  // namespace
 
-cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, float* state, int z0, int nzs) {
+cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs) {
     const long long tot = (long long)c->prm.nx * c->prm.ny * nzs;
-    to_perturbation_kernel<<<grid_for(tot, 148 * 16), 256, 0, c->stream>>>(make_aux(c), state, z0, nzs);
+    to_perturbation_kernel<<<grid_for(tot, 148 * 16), 256, 0, c->stream>>>(make_aux(c), dense_slab, state, z0, nzs);
     c->launches += 1;
     return cudaGetLastError();
 }

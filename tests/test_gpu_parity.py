@@ -85,6 +85,32 @@ def test_cfg1_full_32cubed_20_steps():
     assert fv.min() >= 0.0 and fv.max() <= 1.0
 
 
+def test_data_paths_agree():
+    """brick layout with the TMA-staged x sweep (default), brick layout with the direct x sweep, and the SoA-plane
+    fallback run the same marching body: the two brick paths are bit-identical; planes differ only through the
+    warp-uniform Newton exit (different pencils share a warp), i.e. by rounding."""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_LAYOUT, OPT_X_PATH
+    for cfg, n in ((1, 32), (4, 32), (3, 32)):
+        w = W.make(cfg, n=n)
+        f = w.fields().cuda()
+        res = []
+        for mode in ("tma", "direct", "planes"):
+            g = PPM.from_workload(w)
+            if mode == "planes":
+                g.set_option(OPT_LAYOUT, 1)
+            if mode == "direct":
+                g.set_option(OPT_X_PATH, 1)
+            assert g.x_path() == (1 if mode == "tma" else 0)
+            g.set_state(f)
+            for s in range(3):
+                g.step(g.cfl_dt(0.8), s * 2)
+            res.append(g.get_state().cpu().numpy().astype(np.float64))
+            g.close()
+        assert np.array_equal(res[0], res[1])
+        assert max(max_rel(res[2], res[0]).values()) < 2e-6
+
+
 @pytest.mark.parametrize("chunk", [8, 13])
 def test_pencil_chunking_does_not_change_results(chunk):
     PPM = _gpu()
