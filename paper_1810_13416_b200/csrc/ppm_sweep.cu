@@ -363,8 +363,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // Newton on p*' with the two-shock wave speeds W_K; at most 5 iterations (reading R7).  The loop
             // stops early only when EVERY lane's last update is below fp32 resolution of p* (warp-uniform
             // exit), i.e. when further iterations could not change the result beyond rounding.
-#pragma unroll 1
-            for (int it = 0; it < 5; ++it) {
+            auto newton = [&]() -> bool {
                 const float ps = p0fc + pps;
                 const float wl2 = fmaf(gpL, ps, gmL), wr2 = fmaf(gpR, ps, gmR);
                 const float iwl = rsqrtf(wl2), iwr = rsqrtf(wr2);
@@ -373,7 +372,14 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 const float izl = (wl2 + CL2) * (iwl * iwl * iwl), izr = (wr2 + CR2) * (iwr * iwr * iwr);
                 const float d = fdiv(2.0f * (usr - usl), izl + izr);
                 pps = fmaxf(pfl, pps - d);
-                if (__all_sync(wmask, fabsf(d) <= 6e-8f * ps)) break;
+                return fabsf(d) <= 6e-8f * ps;
+            };
+            // first iteration in straight-line code (the scheduler can overlap it with independent work); the
+            // remaining ones only while some lane still moves (rare at low Mach: the acoustic guess is nearly exact)
+            if (!__all_sync(wmask, newton())) {
+#pragma unroll 1
+                for (int it = 1; it < 5; ++it)
+                    if (__all_sync(wmask, newton())) break;
             }
             const float ps = p0fc + pps;
             const float wl2 = fmaf(gpL, ps, gmL), wr2 = fmaf(gpR, ps, gmR);
@@ -465,18 +471,19 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 // =====================================================================================================
 // IoDirect: straight global loads / stores, lanes along a contiguous axis; next plane prefetched.
 // =====================================================================================================
-__device__ __forceinline__ long long axis_off(const SweepParams& P, int j) { return (long long)(j >> 2) * P.SBd + (j & 3) * P.SId; }
+__device__ __forceinline__ unsigned axis_off(const SweepParams& P, int j) { return (unsigned)(j >> 2) * (unsigned)P.SBd + (unsigned)(j & 3) * (unsigned)P.SId; }
 
 template <int DIR>
 struct IoDirect {
     const SweepParams& P;
-    const long long pbase;
+    const unsigned pbase;    // element offsets inside one field fit 32 bits (ppm_create checks)
     float nx5[5];            // plane n+1, already in flight
-    int jn; float sn;
-    __device__ __forceinline__ IoDirect(const SweepParams& P_, long long pb, int n0) : P(P_), pbase(pb) { fetch(n0); }
+    float nm[10];            // PPB coefficients of the next cell, already in flight
+    int jn; float sn, snm;
+    __device__ __forceinline__ IoDirect(const SweepParams& P_, unsigned pb, int n0, int c0) : P(P_), pbase(pb) { fetch(n0); fetch_ppb(c0 - 1); }
     __device__ __forceinline__ void fetch(int n) {
         jn = image_cell(n, P.n, P.bc_lo, P.bc_hi, sn);
-        const long long id = pbase + axis_off(P, jn);
+        const unsigned id = pbase + axis_off(P, jn);
         nx5[0] = __ldg(P.inf[0] + id);
         nx5[1] = __ldg(P.inf[Dir<DIR>::U] + id);
         nx5[2] = __ldg(P.inf[Dir<DIR>::V] + id);
@@ -491,16 +498,20 @@ struct IoDirect {
         v[1] *= sgn;
         fetch(n + 1);        // overshoots by one plane at the end of the pencil: still a valid image cell
     }
-    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
-        float sgn;
-        const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, sgn);
-        const long long id = pbase + axis_off(P, j);
+    __device__ __forceinline__ void fetch_ppb(int c) {
+        const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, snm);
+        const unsigned id = pbase + axis_off(P, j);
 #pragma unroll
-        for (int k = 0; k < 10; ++k) m[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
-        m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
+        for (int k = 0; k < 10; ++k) nm[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
+    }
+    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
+#pragma unroll
+        for (int k = 0; k < 10; ++k) m[k] = nm[k];
+        m[1] *= snm; m[4] *= snm; m[6] *= snm;
+        fetch_ppb(c + 1);    // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
     }
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
-        const long long id = pbase + axis_off(P, i);
+        const unsigned id = pbase + axis_off(P, i);
         P.outf[0][id] = h[0];
         P.outf[Dir<DIR>::U][id] = h[1];
         P.outf[Dir<DIR>::V][id] = h[2];
@@ -528,8 +539,8 @@ __global__ void __launch_bounds__(128, 3) ppm_sweep_kernel(const SweepParams P) 
     const unsigned wmask = __activemask();
     const int c0 = blockIdx.z * P.chunk;
     const int c1 = min(c0 + P.chunk, P.n);
-    const long long tb = (long long)(a >> 2) * P.SBa + (a & 3) * P.SIa + (long long)(b >> 2) * P.SBb + (b & 3) * P.SIb;
-    IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST);
+    const unsigned tb = (unsigned)(a >> 2) * (unsigned)P.SBa + (unsigned)(a & 3) * (unsigned)P.SIa + (unsigned)(b >> 2) * (unsigned)P.SBb + (unsigned)(b & 3) * (unsigned)P.SIb;
+    IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     march<DIR, GRAV>(P, io, a, b, c0, c1, true, wmask);
 }
 
@@ -803,7 +814,6 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     } else {
         const long long str[3] = {1, nx, nx * ny};
         for (int d = 0; d < 3; ++d) { SB[d] = 4 * str[d]; SI[d] = (int)str[d]; }
-        if (nx * ny >= (1LL << 31)) return cudaErrorInvalidValue;
     }
     P.SBd = SB[axis]; P.SBa = SB[ia]; P.SBb = SB[ib];
     P.SId = SI[axis]; P.SIa = SI[ia]; P.SIb = SI[ib];
