@@ -451,3 +451,25 @@ def test_p4_mass_conservation_on_a_ring():
 def test_p4_degenerate_new_mass_leaves_cell_unchanged():
     out, ok = ob.p4_remap(2, [[1, 0, 0], [0.3, 0.2, 0.1], [0, 0, 0]], [1, 1, 1], 0.0, 1.0)
     assert ok == 0 and out == pytest.approx([0.3, 0.2, 0.1])
+
+
+# ---------------------------------------------------------------- the paper's printed arithmetic ----
+def test_paper_printed_arithmetic():
+    """tests/golden/paper_arithmetic.txt holds the numbers PAPER.md prints at L149/L118.  They pin reading R18
+    (the garbled brick-cost formula) and the record/flop arithmetic DESIGN.md quotes: 64 cells x 16 vars x 4 B,
+    2 x 1300 x 32 flops per briquette (L124: 1300-1400 flops per 32-cell half-briquette)."""
+    import os
+    vals = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_arithmetic.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            vals[line[0]] = float(line[1])
+    cost = lambda M: (M + 1) * ((M + 2) ** 2 + (M + 2) * M + M * M)          # R18
+    assert cost(40) == vals["brick_updates_M40"] and cost(80) == vals["brick_updates_M80"]
+    assert 4 * 4 * 4 * 16 * 4 == vals["briquette_bytes"]
+    assert 2 * 1300 * 32 == vals["flops_per_briquette"]
+    halo = lambda M: ((M + 2) ** 3 - M ** 3) * 4000 / 1e6       # the paper rounds the 4096-byte record to "4 KB" = 4000 B here
+    assert halo(40) == pytest.approx(vals["halo_mbytes_M40"], rel=2e-3)
+    assert halo(80) == pytest.approx(vals["halo_mbytes_M80"], rel=2e-3)
+    assert cost(40) * vals["flops_per_briquette"] / 1e9 == pytest.approx(vals["gflop_M40"], rel=2e-3)
+    assert cost(80) * vals["flops_per_briquette"] / 1e9 == pytest.approx(vals["gflop_M80"], rel=2e-3)
