@@ -40,7 +40,13 @@
 
 #include "ppm_internal.h"
 
+#ifndef PPM_MARCH_UNROLL
+#define PPM_MARCH_UNROLL 1
+#endif
+
 namespace {
+
+constexpr int MARCH_UNROLL = PPM_MARCH_UNROLL;   // iterations of the marching loop per loop body
 
 // ---- field permutations per sweep direction ----------------------------------------------------
 template <int DIR> struct Dir;
@@ -246,6 +252,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 #pragma unroll
         for (int k = 0; k < 10; ++k) mw[s][k] = 0.f;
 
+#pragma unroll MARCH_UNROLL
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
         io.begin(n);
         // ---- shift windows, take plane n ---------------------------------------------------------------
