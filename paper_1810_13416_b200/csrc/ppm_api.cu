@@ -91,7 +91,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
         std::vector<float4> t32(g.n);
         std::vector<double> t64(3 * (size_t)g.n);
         for (int k = 0; k < g.n; ++k) {
-            t32[k] = make_float4(g.g[k], g.rho0[k], g.p0[k], 0.f);
+            t32[k] = make_float4(g.rho0[k], g.p0[k], g.g[k], 0.f);   // (rho0, p0) is an aligned pair for the packed lerp
             t64[3 * k] = g.g[k]; t64[3 * k + 1] = g.rho0[k]; t64[3 * k + 2] = g.p0[k];
         }
         CUC(cudaMalloc(&c->tab, sizeof(float4) * g.n));

@@ -31,7 +31,7 @@ struct SweepParams {
     int tab_n;
     float s0, inv_ds;
     float cen_d, cen_a, cen_b;      // RADIAL centre along (sweep, a, b) axes
-    const float4* __restrict__ tab; // node k: {g, rho0, p0, 0}
+    const float4* __restrict__ tab; // node k: {rho0, p0, g, 0}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
 };
 

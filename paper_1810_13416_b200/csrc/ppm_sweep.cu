@@ -66,26 +66,63 @@ __device__ __forceinline__ float rcp(float x) { return __fdividef(1.0f, x); }
 __device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
 __device__ __forceinline__ float fsqrt(float x) { return x * rsqrtf(fmaxf(x, 1e-37f)); }
 
+// ---- packed fp32 pairs (sm_100a FADD2 / FMUL2 / FFMA2) --------------------------------------------------
+// The sweep is bound by instruction issue, not by the FP32 lanes: one f32x2 instruction does the work of two
+// scalar ones in one issue slot.  A v2 lives in an aligned register pair; ptxas folds negation, |x|, the
+// (-,+) / (+,-) sign patterns, half swaps and scalar broadcasts into operand modifiers, and min/max/select on
+// a half are ordinary scalar instructions on that register — so packing costs no extra moves.
+struct v2 { float x, y; };
+__device__ __forceinline__ unsigned long long pk(v2 a) { unsigned long long r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a.x), "f"(a.y)); return r; }
+__device__ __forceinline__ v2 up(unsigned long long a) { v2 r; asm("mov.b64 {%0,%1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(a)); return r; }
+__device__ __forceinline__ v2 operator+(v2 a, v2 b) { unsigned long long r; asm("add.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b))); return up(r); }
+__device__ __forceinline__ v2 operator-(v2 a, v2 b) { unsigned long long r; asm("sub.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b))); return up(r); }
+__device__ __forceinline__ v2 operator*(v2 a, v2 b) { unsigned long long r; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b))); return up(r); }
+__device__ __forceinline__ v2 fma2(v2 a, v2 b, v2 c) { unsigned long long r; asm("fma.rn.ftz.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c))); return up(r); }
+__device__ __forceinline__ v2 mk(float x, float y) { v2 r; r.x = x; r.y = y; return r; }
+__device__ __forceinline__ v2 bc(float s) { return mk(s, s); }                 // broadcast
+__device__ __forceinline__ v2 operator*(v2 a, float s) { return a * bc(s); }
+__device__ __forceinline__ v2 operator-(v2 a) { return mk(-a.x, -a.y); }
+__device__ __forceinline__ v2 np(v2 a) { return mk(-a.x, a.y); }              // (-,+) sign pattern
+__device__ __forceinline__ v2 swp(v2 a) { return mk(a.y, a.x); }
+__device__ __forceinline__ v2 abs2(v2 a) { return mk(fabsf(a.x), fabsf(a.y)); }
+__device__ __forceinline__ float hsum(v2 a) { return a.x + a.y; }
+
+// the five interpolated variables of a cell: A = (rho', p'), B = (v, w) transverse, u normal
+struct V5 { v2 A, B; float u; };
+__device__ __forceinline__ V5 operator+(const V5& a, const V5& b) { V5 r; r.A = a.A + b.A; r.B = a.B + b.B; r.u = a.u + b.u; return r; }
+__device__ __forceinline__ V5 operator-(const V5& a, const V5& b) { V5 r; r.A = a.A - b.A; r.B = a.B - b.B; r.u = a.u - b.u; return r; }
+__device__ __forceinline__ V5 operator*(const V5& a, const V5& b) { V5 r; r.A = a.A * b.A; r.B = a.B * b.B; r.u = a.u * b.u; return r; }
+__device__ __forceinline__ V5 operator*(const V5& a, float s) { V5 r; r.A = a.A * bc(s); r.B = a.B * bc(s); r.u = a.u * s; return r; }
+__device__ __forceinline__ V5 fma5(const V5& a, const V5& b, const V5& c) { V5 r; r.A = fma2(a.A, b.A, c.A); r.B = fma2(a.B, b.B, c.B); r.u = fmaf(a.u, b.u, c.u); return r; }
+__device__ __forceinline__ V5 fma5(const V5& a, float s, const V5& c) { V5 r; r.A = fma2(a.A, bc(s), c.A); r.B = fma2(a.B, bc(s), c.B); r.u = fmaf(a.u, s, c.u); return r; }
+__device__ __forceinline__ V5 abs5(const V5& a) { V5 r; r.A = abs2(a.A); r.B = abs2(a.B); r.u = fabsf(a.u); return r; }
+__device__ __forceinline__ V5 bc5(float s) { V5 r; r.A = bc(s); r.B = bc(s); r.u = s; return r; }
+__device__ __forceinline__ V5 zero5() { V5 r; r.A = bc(0.f); r.B = bc(0.f); r.u = 0.f; return r; }
+template <class F> __device__ __forceinline__ V5 map3(const V5& a, const V5& b, const V5& c, F f) {
+    V5 r; r.A = mk(f(a.A.x, b.A.x, c.A.x), f(a.A.y, b.A.y, c.A.y)); r.B = mk(f(a.B.x, b.B.x, c.B.x), f(a.B.y, b.B.y, c.B.y)); r.u = f(a.u, b.u, c.u); return r;
+}
+
 // image of a cell / face index outside [0, n) under the boundary condition (C3)
 __device__ __forceinline__ int image_cell(int i, int n, int bc_lo, int bc_hi, float& sgn) {
     sgn = 1.0f;
     if (i >= 0 && i < n) return i;
-    const int bc = (i < 0) ? bc_lo : bc_hi;
-    if (bc == PPM_BC_PERIODIC) return ((i % n) + n) % n;
+    const int bcx = (i < 0) ? bc_lo : bc_hi;
+    if (bcx == PPM_BC_PERIODIC) return ((i % n) + n) % n;
     sgn = -1.0f;
     int s = (i < 0) ? (-1 - i) : (2 * n - 1 - i);
     return min(max(s, 0), n - 1);
 }
 __device__ __forceinline__ int image_face(int f, int n, int bc_lo, int bc_hi) {
     if (f >= 0 && f <= n) return (f == n && bc_hi == PPM_BC_PERIODIC) ? 0 : f;
-    const int bc = (f < 0) ? bc_lo : bc_hi;
-    if (bc == PPM_BC_PERIODIC) return ((f % n) + n) % n;
+    const int bcx = (f < 0) ? bc_lo : bc_hi;
+    if (bcx == PPM_BC_PERIODIC) return ((f % n) + n) % n;
     int s = (f < 0) ? -f : 2 * n - f;
     return min(max(s, 0), n);
 }
 
 // ---- base state (C1) -----------------------------------------------------------------------------
-struct Base { float r0, p0, g; };
+// table node k: {rho0, p0, g, 0} — (rho0, p0) is an aligned pair
+struct Base { v2 rp; float g; };
 
 __device__ __forceinline__ Base table_at(const SweepParams& P, float s) {
     float t = (s - P.s0) * P.inv_ds;
@@ -94,9 +131,9 @@ __device__ __forceinline__ Base table_at(const SweepParams& P, float s) {
     float w = t - (float)k;
     float4 a = __ldg(P.tab + k), b = __ldg(P.tab + k + 1);
     Base o;
-    o.g = fmaf(w, b.x - a.x, a.x);
-    o.r0 = fmaf(w, b.y - a.y, a.y);
-    o.p0 = fmaf(w, b.z - a.z, a.z);
+    const v2 ra = mk(a.x, a.y), rb = mk(b.x, b.y);
+    o.rp = fma2(bc(w), rb - ra, ra);
+    o.g = fmaf(w, b.z - a.z, a.z);
     return o;
 }
 
@@ -105,20 +142,20 @@ template <int DIR, int GRAV> struct Geo {
     float t2;      // RADIAL: squared transverse distance from the centre
     Base cst;      // CONST_Z, DIR != 2: the base state is constant along the pencil
     __device__ __forceinline__ void init(const SweepParams& P, int a, int b) {
-        t2 = 0.f; cst.r0 = cst.p0 = cst.g = 0.f;
+        t2 = 0.f; cst.rp = bc(0.f); cst.g = 0.f;
         if (GRAV == PPM_GRAV_RADIAL) {
             float xa = ((float)a + 0.5f) * P.dx - P.cen_a, xb = ((float)b + 0.5f) * P.dx - P.cen_b;
             t2 = xa * xa + xb * xb;
         } else if (GRAV == PPM_GRAV_CONST_Z && DIR != 2) {
             float4 v = __ldg(P.tab + 2 * b + 2 * PPM_NGHOST + 1);   // b is the z index for x- and y-sweeps
-            cst.r0 = v.y; cst.p0 = v.z; cst.g = 0.f;                // no acceleration along x or y
+            cst.rp = mk(v.x, v.y); cst.g = 0.f;                     // no acceleration along x or y
         }
     }
     // cell centre with image index j (sign sgn for the odd normal acceleration)
     __device__ __forceinline__ Base cell(const SweepParams& P, int j, float sgn) const {
-        Base o; o.r0 = o.p0 = o.g = 0.f;
+        Base o; o.rp = bc(0.f); o.g = 0.f;
         if (GRAV == PPM_GRAV_CONST_Z) {
-            if (DIR == 2) { float4 v = __ldg(P.tab + 2 * j + 2 * PPM_NGHOST + 1); o.g = sgn * v.x; o.r0 = v.y; o.p0 = v.z; }
+            if (DIR == 2) { float4 v = __ldg(P.tab + 2 * j + 2 * PPM_NGHOST + 1); o.g = sgn * v.z; o.rp = mk(v.x, v.y); }
             else o = cst;
         } else if (GRAV == PPM_GRAV_RADIAL) {
             float xd = ((float)j + 0.5f) * P.dx - P.cen_d;
@@ -129,94 +166,116 @@ template <int DIR, int GRAV> struct Geo {
         }
         return o;
     }
-    // face with image index f (position f*dx along the sweep axis)
-    __device__ __forceinline__ void face(const SweepParams& P, int f, float& r0, float& p0) const {
-        r0 = 0.f; p0 = 0.f;
+    // face with image index f (position f*dx along the sweep axis): (rho0, p0)
+    __device__ __forceinline__ v2 face(const SweepParams& P, int f) const {
+        v2 o = bc(0.f);
         if (GRAV == PPM_GRAV_CONST_Z) {
-            if (DIR == 2) { float4 v = __ldg(P.tab + 2 * f + 2 * PPM_NGHOST); r0 = v.y; p0 = v.z; }
-            else { r0 = cst.r0; p0 = cst.p0; }
+            if (DIR == 2) { float4 v = __ldg(P.tab + 2 * f + 2 * PPM_NGHOST); o = mk(v.x, v.y); }
+            else o = cst.rp;
         } else if (GRAV == PPM_GRAV_RADIAL) {
             float xd = (float)f * P.dx - P.cen_d;
             float r2 = fmaf(xd, xd, t2);
-            Base o = table_at(P, fsqrt(r2));
-            r0 = o.r0; p0 = o.p0;
+            o = table_at(P, fsqrt(r2)).rp;
         }
+        return o;
     }
 };
 
 // ---- H2 + H3: limited parabola blended with the unlimited one ------------------------------------
-// Lc, Rc: face values already clamped between the neighbouring cell means (per-face medians)
-__device__ __forceinline__ void parabola(float q0, float Lc, float Rc, float fl, float fr, float om, float& L, float& R) {
-    const bool ext = (Rc - q0) * (q0 - Lc) <= 0.0f;
-    const float D = Rc - Lc, q6 = 6.0f * (q0 - 0.5f * (Lc + Rc));
-    const float Dq6 = D * q6, D2 = D * D;
-    float L2 = (Dq6 > D2) ? fmaf(-2.0f, Rc, 3.0f * q0) : Lc;
-    float R2 = (Dq6 < -D2) ? fmaf(-2.0f, Lc, 3.0f * q0) : Rc;
-    L2 = ext ? q0 : L2;
-    R2 = ext ? q0 : R2;
-    L = fmaf(om, L2 - fl, fl);
-    R = fmaf(om, R2 - fr, fr);
+// Lc, Rc: face values already clamped between the neighbouring cell means (per-face medians); fl, fr the
+// unlimited faces; om the smoothness weight.  With a = Rc - q0, b = q0 - Lc (same sign unless the cell is an
+// extremum): Delta = a + b, q6 = 3(b - a), so the Colella-Woodward overshoot tests Delta*q6 > Delta^2 and
+// Delta*q6 < -Delta^2 are |b| > 2|a| and |a| > 2|b|, and the corrected faces are q0 - 2a and q0 + 2b.
+__device__ __forceinline__ void parabola(const V5& q0, const V5& Lc, const V5& Rc, const V5& fl, const V5& fr, const V5& om, V5& L, V5& R) {
+    const V5 a = Rc - q0, b = q0 - Lc;
+    const V5 pr = a * b;
+    const V5 a2 = a + a, b2 = b + b;
+    const V5 La = q0 - a2, Ra = q0 + b2;
+    // L2: extremum -> q0; |b| > |2a| -> q0 - 2a; else Lc.   (selects are per element)
+    V5 L2, R2;
+#define PPM_SEL(E) \
+    { const bool ext = pr.E <= 0.0f; \
+      const float l = (fabsf(b.E) > fabsf(a2.E)) ? La.E : Lc.E; \
+      const float r = (fabsf(a.E) > fabsf(b2.E)) ? Ra.E : Rc.E; \
+      L2.E = ext ? q0.E : l; R2.E = ext ? q0.E : r; }
+    PPM_SEL(A.x) PPM_SEL(A.y) PPM_SEL(B.x) PPM_SEL(B.y) PPM_SEL(u)
+#undef PPM_SEL
+    L = fma5(om, L2 - fl, fl);
+    R = fma5(om, R2 - fr, fr);
 }
 
-// ---- H5: A+(s) = qR - F+(q;s),  A-(s) = F-(q;s) - qL ------------------------------------------------
-__device__ __forceinline__ float Aplus(float dq, float q6, float s) { return 0.5f * s * (dq - (1.0f - (2.0f / 3.0f) * s) * q6); }
-__device__ __forceinline__ float Aminus(float dq, float q6, float s) { return 0.5f * s * (dq + (1.0f - (2.0f / 3.0f) * s) * q6); }
-
 // ---- P4: exact projection of up to three pieces onto the Legendre basis ---------------------------
-// S[s][0..9]: pre-limited coefficients (local family order) of cells i-1, i, i+1; rm,r0,rp their masses
-// per dx; dl, dr = mass per dx through the left / right face (positive rightward).
-__device__ __forceinline__ void ppb_remap(const float (&S)[3][10], float rm, float r0, float rp, float dl, float dr,
-                                          float (&out)[10]) {
+// pre-limited coefficients of one cell in local family order, stored as the pairs the remap uses
+struct PpbCell { float a0, a1, a2; v2 bc0, bc1, de; float f; };   // bc0 = (b0, c0), bc1 = (b1, c1), de = (d0, e0)
+
+// S[0..2]: cells i-1, i, i+1; rm,r0,rp their masses per dx; dl, dr = mass per dx through the left / right
+// face (positive rightward).  The two donor pieces (from i-1 and from i+1) run as one packed computation for
+// the degree-2 family; the (b,c) and (d,e) families are packed inside every piece.
+__device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float rm, float r0, float rp, float dl, float dr, float (&out)[10]) {
     const float rn = r0 - dr + dl;
     const bool ok = rn > PPM_TINY;
     const float irn = rcp(fmaxf(rn, PPM_TINY));
-    const float dlp = fmaxf(dl, 0.f), dln = fmaxf(-dl, 0.f), drp = fmaxf(dr, 0.f), drn = fmaxf(-dr, 0.f);
-    const float irm = rcp(rm), ir0 = rcp(r0), irp = rcp(rp);
-    const float w1 = dlp * irn, w3 = drn * irn;          // widths of the donor pieces in the new cell
-    // piece geometry: new-coordinate midpoint xm, half width h; old-coordinate midpoint sm, slope beta
-    float xm[3], h[3], sm[3], be[3];
-    h[0] = 0.5f * w1;              xm[0] = -0.5f + h[0];          sm[0] = 0.5f - 0.5f * dlp * irm;   be[0] = rn * irm;
-    h[2] = 0.5f * w3;              xm[2] = 0.5f - h[2];           sm[2] = -0.5f + 0.5f * drn * irp;  be[2] = rn * irp;
-    h[1] = 0.5f - h[0] - h[2];     xm[1] = h[0] - h[2];           sm[1] = 0.5f * (dln - drp) * ir0;  be[1] = rn * ir0;
+    const float dln = fmaxf(-dl, 0.f), drp = fmaxf(dr, 0.f);
+    const v2 dD = mk(fmaxf(dl, 0.f), fmaxf(-dr, 0.f));      // donated mass: from the left cell, from the right cell
+    const v2 irD = mk(rcp(rm), rcp(rp));
+    const float ir0 = rcp(r0);
+    // piece geometry: new-coordinate midpoint x, half width h; old-coordinate midpoint s, slope beta
+    const v2 hD = dD * bc(0.5f * irn);                       // half widths of the donor pieces in the new cell
+    const v2 xD = fma2(hD, mk(1.f, -1.f), mk(-0.5f, 0.5f));
+    const v2 sD = fma2(dD * irD, mk(-0.5f, 0.5f), mk(0.5f, -0.5f));
+    const v2 bD = irD * bc(rn);
+    const float h1 = 0.5f - hD.x - hD.y, x1 = hD.x - hD.y, s1 = 0.5f * (dln - drp) * ir0, b1 = rn * ir0;
+    // powers of the half width: w = 2h, w2 = 2h^3/3, w4 = 2h^5/5
+    const v2 h2D = hD * hD, wD = hD + hD, w2D = (wD * h2D) * bc(1.0f / 3.0f), w4D = (w2D * h2D) * bc(0.6f);
+    const float h21 = h1 * h1, w1 = h1 + h1, w21 = w1 * h21 * (1.0f / 3.0f), w41 = w21 * h21 * 0.6f;
+    const v2 x2D = fma2(xD, xD, bc(-1.0f / 12.0f)), s2D = fma2(sD, sD, bc(-1.0f / 12.0f));
+    const float x21 = fmaf(x1, x1, -1.0f / 12.0f), s21 = fmaf(s1, s1, -1.0f / 12.0f);
     // reference constants (own cell's degree-0 coefficients): projecting a constant is exact, so only
     // deviations from it are integrated (keeps fp32 round-off at the size of the variation)
-    const float refA = S[1][0], refB = S[1][3], refC = S[1][5];
-    float a0 = 0.f, a1 = 0.f, a2 = 0.f, b0 = 0.f, b1 = 0.f, c0 = 0.f, c1 = 0.f, d0 = 0.f, e0 = 0.f, f0 = 0.f;
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const float hh = h[k], h2 = hh * hh, w = 2.0f * hh;
-        const float h23 = h2 * (1.0f / 3.0f), h45 = h2 * h2 * 0.2f;
-        const float x = xm[k], x2 = fmaf(x, x, -1.0f / 12.0f);
-        const float s = sm[k], s2 = fmaf(s, s, -1.0f / 12.0f), b = be[k];
-        const float* c = S[k];
-        {   // degree-2 family
-            const float E2 = c[2] * b * b, E1 = b * fmaf(2.0f * c[2], s, c[1]);
-            const float E0 = (c[0] - refA) + fmaf(c[1], s, c[2] * s2);
-            const float J0 = w * fmaf(E2, h23, E0), J1 = w * E1 * h23, J2 = w * fmaf(E0, h23, E2 * h45);
-            a0 += J0;
-            a1 += fmaf(x, J0, J1);
-            a2 += fmaf(x2, J0, fmaf(2.0f * x, J1, J2));
-        }
-        {   // the two degree-1 families
-            const float E0b = (c[3] - refB) + c[4] * s, E1b = b * c[4];
-            const float J0b = w * E0b, J1b = w * E1b * h23;
-            b0 += J0b; b1 += fmaf(x, J0b, J1b);
-            const float E0c = (c[5] - refC) + c[6] * s, E1c = b * c[6];
-            const float J0c = w * E0c, J1c = w * E1c * h23;
-            c0 += J0c; c1 += fmaf(x, J0c, J1c);
-        }
-        d0 = fmaf(w, c[7], d0); e0 = fmaf(w, c[8], e0); f0 = fmaf(w, c[9], f0);
+    const float refA = S[1].a0;
+    const v2 refBC = S[1].bc0;
+    // ---- degree-2 family: donors packed (x = from i-1, y = from i+1), own piece scalar
+    float a0, a1, a2;
+    {
+        const v2 c0 = mk(S[0].a0, S[2].a0), c1 = mk(S[0].a1, S[2].a1), c2 = mk(S[0].a2, S[2].a2);
+        const v2 E2 = (c2 * bD) * bD, E1 = bD * fma2(c2 + c2, sD, c1);
+        const v2 E0 = (c0 - bc(refA)) + fma2(c1, sD, c2 * s2D);
+        const v2 J0 = fma2(w2D, E2, wD * E0), J1 = w2D * E1, J2 = fma2(w4D, E2, w2D * E0);
+        const v2 A1 = fma2(xD, J0, J1), A2 = fma2(x2D, J0, fma2(xD + xD, J1, J2));
+        const float d1 = S[1].a1, d2 = S[1].a2;
+        const float e2 = d2 * b1 * b1, e1 = b1 * fmaf(2.0f * d2, s1, d1);
+        const float e0 = fmaf(d1, s1, d2 * s21);
+        const float j0 = fmaf(w21, e2, w1 * e0), j1 = w21 * e1, j2 = fmaf(w41, e2, w21 * e0);
+        a0 = hsum(J0) + j0;
+        a1 = hsum(A1) + fmaf(x1, j0, j1);
+        a2 = hsum(A2) + fmaf(x21, j0, fmaf(2.0f * x1, j1, j2));
     }
-    out[0] = ok ? refA + a0 : S[1][0];
-    out[1] = ok ? 12.0f * a1 : S[1][1];
-    out[2] = ok ? 180.0f * a2 : S[1][2];
-    out[3] = ok ? refB + b0 : S[1][3];
-    out[4] = ok ? 12.0f * b1 : S[1][4];
-    out[5] = ok ? refC + c0 : S[1][5];
-    out[6] = ok ? 12.0f * c1 : S[1][6];
-    out[7] = ok ? d0 : S[1][7];
-    out[8] = ok ? e0 : S[1][8];
-    out[9] = ok ? f0 : S[1][9];
+    // ---- the two degree-1 families (b, c) and the degree-0 pair (d, e), packed per piece; f scalar
+    v2 g0, g1, de;
+    float f0;
+    {
+        // donor from i-1 (geometry = x halves), own piece, donor from i+1 (y halves)
+        const v2 E0m = (S[0].bc0 - refBC) + S[0].bc1 * bc(sD.x), E1m = S[0].bc1 * bc(bD.x);
+        const v2 E0o = S[1].bc1 * bc(s1), E1o = S[1].bc1 * bc(b1);
+        const v2 E0p = (S[2].bc0 - refBC) + S[2].bc1 * bc(sD.y), E1p = S[2].bc1 * bc(bD.y);
+        const v2 J0m = E0m * bc(wD.x), J1m = E1m * bc(w2D.x);
+        const v2 J0o = E0o * bc(w1), J1o = E1o * bc(w21);
+        const v2 J0p = E0p * bc(wD.y), J1p = E1p * bc(w2D.y);
+        g0 = (J0m + J0o) + J0p;
+        g1 = (fma2(bc(xD.x), J0m, J1m) + fma2(bc(x1), J0o, J1o)) + fma2(bc(xD.y), J0p, J1p);
+        de = fma2(bc(wD.x), S[0].de, fma2(bc(w1), S[1].de, S[2].de * bc(wD.y)));
+        f0 = fmaf(wD.x, S[0].f, fmaf(w1, S[1].f, wD.y * S[2].f));
+    }
+    out[0] = ok ? refA + a0 : S[1].a0;
+    out[1] = ok ? 12.0f * a1 : S[1].a1;
+    out[2] = ok ? 180.0f * a2 : S[1].a2;
+    out[3] = ok ? refBC.x + g0.x : S[1].bc0.x;
+    out[4] = ok ? 12.0f * g1.x : S[1].bc1.x;
+    out[5] = ok ? refBC.y + g0.y : S[1].bc0.y;
+    out[6] = ok ? 12.0f * g1.y : S[1].bc1.y;
+    out[7] = ok ? de.x : S[1].de.x;
+    out[8] = ok ? de.y : S[1].de.y;
+    out[9] = ok ? f0 : S[1].f;
 }
 
 // =====================================================================================================
@@ -226,65 +285,58 @@ __device__ __forceinline__ void ppb_remap(const float (&S)[3][10], float rm, flo
 template <int DIR, int GRAV, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
                                       const bool valid, const unsigned wmask) {
-    const float gam = P.gamma, gp = 0.5f * (gam + 1.0f), gm = 0.5f * (gam - 1.0f), g_gm1 = gam * rcp(gam - 1.0f);
+    const float gam = P.gamma, gp = 0.5f * (gam + 1.0f), gmg = 0.5f * (gam - 1.0f) * rcp(gam), g_gm1 = gam * rcp(gam - 1.0f);
     const float dtdx = P.dtdx, hdt = 0.5f * P.dt;
 
     Geo<DIR, GRAV> geo;
     geo.init(P, a, b);
 
-    // sliding windows (registers).  q[k][s]: cell n-4+s;  k = rho', u, v, w, p'
-    float q[5][5], pf[5], rf[6], gw[5];
+    // sliding windows (registers).  q[s]: cell n-4+s
+    V5 q[5];
+    float pf[5], rf[6], gw[5];
 #pragma unroll
-    for (int s = 0; s < 5; ++s) {
-#pragma unroll
-        for (int k = 0; k < 5; ++k) q[k][s] = 0.f;
-        pf[s] = 1.f; gw[s] = 0.f;
-    }
+    for (int s = 0; s < 5; ++s) { q[s] = zero5(); pf[s] = 1.f; gw[s] = 0.f; }
 #pragma unroll
     for (int s = 0; s < 6; ++s) rf[s] = 1.f;
-    float d2a[5], d2b[5], Fc[5], Fcl[5], parL[5], parR[5], WLc[5], Fl[5];
+    V5 d2a = zero5(), d2b = zero5(), Fc = zero5(), Fcl = zero5(), parL = zero5(), parR = zero5();
+    float WLr = 0.f, WLu = 0.f, WLp = 0.f, WLv = 0.f, WLw = 0.f;      // left state of the face being solved (from cell n-4)
+    float Flm = 0.f, Fln = 0.f, FlE = 0.f;                              // fluxes through the left face of cell n-4
+    v2 FlB = bc(0.f);
+    float ft0 = 0.f, ft1 = 0.f, cs = 1.f;
+    v2 b0fc = bc(0.f);                                                  // (rho0, p0) at the face being solved
+    PpbCell mw[3];
 #pragma unroll
-    for (int k = 0; k < 5; ++k) { d2a[k] = d2b[k] = Fc[k] = Fcl[k] = parL[k] = parR[k] = WLc[k] = Fl[k] = 0.f; }
-    float ft0 = 0.f, ft1 = 0.f, cs = 1.f, r0fc = 0.f, p0fc = 0.f;
-    float mw[3][10];
-#pragma unroll
-    for (int s = 0; s < 3; ++s)
-#pragma unroll
-        for (int k = 0; k < 10; ++k) mw[s][k] = 0.f;
+    for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
 
 #pragma unroll MARCH_UNROLL
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
         io.begin(n);
         // ---- shift windows, take plane n ---------------------------------------------------------------
 #pragma unroll
-        for (int s = 0; s < 4; ++s) {
-#pragma unroll
-            for (int k = 0; k < 5; ++k) q[k][s] = q[k][s + 1];
-            pf[s] = pf[s + 1]; gw[s] = gw[s + 1];
-        }
+        for (int s = 0; s < 4; ++s) { q[s] = q[s + 1]; pf[s] = pf[s + 1]; gw[s] = gw[s + 1]; }
 #pragma unroll
         for (int s = 0; s < 5; ++s) rf[s] = rf[s + 1];
         {
             float sgn, v[5];
             int j;
             io.hydro(n, j, sgn, v);
-#pragma unroll
-            for (int k = 0; k < 5; ++k) q[k][4] = v[k];
+            q[4].A = mk(v[0], v[4]); q[4].B = mk(v[2], v[3]); q[4].u = v[1];
             const Base bs = geo.cell(P, j, sgn);
-            rf[5] = bs.r0 + q[0][4];
-            pf[4] = bs.p0 + q[4][4];
+            const v2 full = bs.rp + q[4].A;
+            rf[5] = full.x;
+            pf[4] = full.y;
             gw[4] = bs.g;
         }
         // ---- A, B, C, D: interpolation of cell n-2 ----------------------------------------------------
-        float d2n[5], Fn[5], Fnl[5], pLn[5], pRn[5];
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            d2n[k] = q[k][4] - 2.0f * q[k][3] + q[k][2];
-            Fn[k] = (7.0f / 12.0f) * (q[k][2] + q[k][3]) - (1.0f / 12.0f) * (q[k][1] + q[k][4]);
-            Fnl[k] = med3(q[k][2], Fn[k], q[k][3]);                      // H2: clamp between the adjacent means
-            const float S = fdiv(fabsf(d2n[k] - d2a[k]), fabsf(d2a[k]) + 2.0f * fabsf(d2b[k]) + fabsf(d2n[k]) + PPM_TINY);
-            const float om = sat((S - 0.1f) * 5.0f);
-            parabola(q[k][2], Fcl[k], Fnl[k], Fc[k], Fn[k], om, pLn[k], pRn[k]);
+        const V5 d2n = fma5(q[3], -2.0f, q[4]) + q[2];                                           // d2_{n-1}
+        const V5 Fn = fma5(q[1] + q[4], -1.0f / 12.0f, (q[2] + q[3]) * (7.0f / 12.0f));          // face (n-2)+1/2 (H1)
+        const V5 Fnl = map3(q[2], Fn, q[3], [](float x, float y, float z) { return med3(x, y, z); });   // H2: clamp
+        V5 pLn, pRn;
+        {
+            const V5 num = d2n - d2a;
+            const V5 den = fma5(abs5(d2b), 2.0f, abs5(d2a)) + (abs5(d2n) + bc5(PPM_TINY));
+            const V5 om = map3(num, den, den, [](float x, float y, float) { return sat(fmaf(fabsf(x) * rcp(y), 5.0f, -0.5f)); });   // H3
+            parabola(q[2], Fcl, Fnl, Fc, Fn, om, pLn, pRn);
         }
         // ---- E, F: flattening ---------------------------------------------------------------------------
         const float cn2 = fsqrt(gam * pf[2] * rcp(rf[3]));          // c_{n-2}
@@ -293,91 +345,92 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const float d1 = pf[3] - pf[1], dd2 = pf[4] - pf[0];
             const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
             const float jump = sat(fdiv(3.0f * fabsf(d1), fminf(pf[3], pf[1])) - 1.0f);
-            const float conv = sat(fdiv(q[1][1] - q[1][3], 0.05f * cn2));
+            const float conv = sat(fdiv(q[1].u - q[3].u, 0.05f * cn2));
             ftn = steep * jump * conv;
         }
         const float fl3 = fmaxf(ft0, fmaxf(ft1, ftn));              // f_{n-3}
         // ---- G, H: flattened parabola and characteristic tracing of cell n-3 ---------------------------
-        float WL[5], WR[5];
-        float r0fn, p0fn;
+        // Each traced quantity is a pair W = (left of face (n-3)+1/2, right of face (n-3)-1/2): the two states
+        // are mirror images, F+ and F- differ only in the sign of the q6 term.
+        v2 Wr, Wu, Wp, Wv, Ww;
+        v2 b0fn;
         {
             const int fi = image_face(n - 2, P.n, P.bc_lo, P.bc_hi);
-            geo.face(P, fi, r0fn, p0fn);
+            b0fn = geo.face(P, fi);
         }
         {
-            float qL[5], dq[5], q6[5];
-#pragma unroll
-            for (int k = 0; k < 5; ++k) {
-                const float qc = q[k][1];
-                const float L = fmaf(fl3, qc - parL[k], parL[k]);
-                const float R = fmaf(fl3, qc - parR[k], parR[k]);
-                qL[k] = L; dq[k] = R - L; q6[k] = 6.0f * (qc - 0.5f * (L + R));
-            }
-            const float rho = rf[2], c = cs, u = q[1][1];
-            const float rc = rho * c, ic2h = 0.5f * rcp(c * c), cor = fdiv(c, rho);   // 1/(2c^2), c/rho
+            const V5 qc = q[1];
+            const V5 L = fma5(qc - parL, fl3, parL);
+            const V5 R = fma5(qc - parR, fl3, parR);
+            const V5 dq = R - L;
+            const V5 q6 = fma5(L + R, -3.0f, qc * 6.0f);
+            const float rho = rf[2], c = cs, u = qc.u;
+            const float c2 = c * c, rc = rho * c, ic2 = rcp(c2), ic2h = 0.5f * ic2, cor = fdiv(c, rho);
             const float s_m = (u - c) * dtdx, s_0 = u * dtdx, s_p = (u + c) * dtdx;
             // Each wave family k takes its amplitude from its own domain of dependence max(+-sigma^k, 0); a
             // wave moving away from the face has the zero-width domain, i.e. the edge value (reading R8',
             // DESIGN.md).  No switch on sign(lambda^k): the traced states are continuous in the data.
-            // left of face (n-3)+1/2 : W~ = qR - A+(max(s_p,0));  delta^k = W~ - F+(s_k) = A+(s_k) - A+(sp)
-            {
-                const float sp = fmaxf(s_p, 0.f), smk = fmaxf(s_m, 0.f), s0k = fmaxf(s_0, 0.f);
-                const float Ar = Aplus(dq[0], q6[0], sp), Au = Aplus(dq[1], q6[1], sp), Ap = Aplus(dq[4], q6[4], sp);
-                const float du_m = Aplus(dq[1], q6[1], smk) - Au, dp_m = Aplus(dq[4], q6[4], smk) - Ap;
-                const float am = (dp_m - rc * du_m) * ic2h;
-                const float dr_0 = Aplus(dq[0], q6[0], s0k) - Ar, dp_0 = Aplus(dq[4], q6[4], s0k) - Ap;
-                const float a0 = dr_0 - dp_0 * (2.0f * ic2h);
-                const float R0 = qL[0] + dq[0], R1 = qL[1] + dq[1], R4 = qL[4] + dq[4];
-                WL[0] = R0 - Ar - am - a0;
-                WL[1] = R1 - Au + cor * am;
-                WL[4] = R4 - Ap - c * c * am;
-                WL[2] = qL[2] + dq[2] - Aplus(dq[2], q6[2], s0k);
-                WL[3] = qL[3] + dq[3] - Aplus(dq[3], q6[3], s0k);
-            }
-            // right of face (n-3)-1/2 : W~ = qL + A-(max(-s_m,0));  delta^k = A-(sm) - A-(max(-s_k,0))
-            {
-                const float sm = fmaxf(-s_m, 0.f), spk = fmaxf(-s_p, 0.f), s0k = fmaxf(-s_0, 0.f);
-                const float Ar = Aminus(dq[0], q6[0], sm), Au = Aminus(dq[1], q6[1], sm), Ap = Aminus(dq[4], q6[4], sm);
-                const float du_p = Au - Aminus(dq[1], q6[1], spk), dp_p = Ap - Aminus(dq[4], q6[4], spk);
-                const float ap = (dp_p + rc * du_p) * ic2h;
-                const float dr_0 = Ar - Aminus(dq[0], q6[0], s0k), dp_0 = Ap - Aminus(dq[4], q6[4], s0k);
-                const float a0 = dr_0 - dp_0 * (2.0f * ic2h);
-                WR[0] = qL[0] + Ar - ap - a0;
-                WR[1] = qL[1] + Au - cor * ap;
-                WR[4] = qL[4] + Ap - c * c * ap;
-                WR[2] = qL[2] + Aminus(dq[2], q6[2], s0k);
-                WR[3] = qL[3] + Aminus(dq[3], q6[3], s0k);
-            }
+            // domains (left state, right state): fastest wave toward the face, the opposite acoustic wave, the entropy wave
+            const v2 sf = mk(fmaxf(s_p, 0.f), fmaxf(-s_m, 0.f));
+            const v2 so = mk(fmaxf(s_m, 0.f), fmaxf(-s_p, 0.f));
+            const v2 se = mk(fmaxf(s_0, 0.f), fmaxf(-s_0, 0.f));
+            // H5: A(s) = (s/2) (dq -+ (1 - 2s/3) q6)   (- for the left state = qR - F+, + for the right = F- - qL)
+            const v2 K23 = mk(2.0f / 3.0f, -2.0f / 3.0f), Km1 = mk(-1.0f, 1.0f);
+            const v2 hf = sf * 0.5f, tf = fma2(sf, K23, Km1);
+            const v2 ho = so * 0.5f, to = fma2(so, K23, Km1);
+            const v2 he = se * 0.5f, te = fma2(se, K23, Km1);
+#define PPM_AV(dq_, q6_, h_, t_) ((h_) * fma2((t_), bc(q6_), bc(dq_)))
+            const v2 Ar = PPM_AV(dq.A.x, q6.A.x, hf, tf), Au = PPM_AV(dq.u, q6.u, hf, tf), Ap = PPM_AV(dq.A.y, q6.A.y, hf, tf);
+            const v2 Ou = PPM_AV(dq.u, q6.u, ho, to), Op = PPM_AV(dq.A.y, q6.A.y, ho, to);
+            const v2 Er = PPM_AV(dq.A.x, q6.A.x, he, te), Ep = PPM_AV(dq.A.y, q6.A.y, he, te);
+            const v2 Ev = PPM_AV(dq.B.x, q6.B.x, he, te), Ew = PPM_AV(dq.B.y, q6.B.y, he, te);
+#undef PPM_AV
+            // acoustic amplitude of the opposite family: beta = (am, -ap);  entropy amplitude al0 = (a0L, -a0R)
+            const v2 du = Ou - Au, dp = Op - Ap;
+            const v2 beta = fma2(np(du), bc(rc), dp) * ic2h;
+            const v2 al0 = fma2(Ep - Ap, bc(-ic2), Er - Ar);
+            // W = (qR, qL) + (-,+) * (...)
+            const v2 K10 = mk(1.0f, 0.0f);
+            const v2 Br = fma2(bc(dq.A.x), K10, bc(L.A.x)), Bu = fma2(bc(dq.u), K10, bc(L.u)), Bp = fma2(bc(dq.A.y), K10, bc(L.A.y));
+            const v2 Bv = fma2(bc(dq.B.x), K10, bc(L.B.x)), Bw = fma2(bc(dq.B.y), K10, bc(L.B.y));
+            Wr = Br + np((Ar + beta) + al0);
+            Wu = (Bu + np(Au)) + beta * cor;
+            Wp = Bp + np(fma2(beta, bc(c2), Ap));
+            Wv = Bv + np(Ev);
+            Ww = Bw + np(Ew);
             if (GRAV != PPM_GRAV_NONE) {   // half-step sources of the perturbation equations (H6)
-                const float sr = hdt * (-u * (r0fn - r0fc) * P.inv_dx);
-                const float sp_ = hdt * (-u * (p0fn - p0fc) * P.inv_dx);
-                const float su = hdt * gw[1] * fdiv(q[0][1], rho);
-                WL[0] += sr; WR[0] += sr; WL[4] += sp_; WR[4] += sp_; WL[1] += su; WR[1] += su;
+                const v2 db = b0fn - b0fc;
+                const float k = -hdt * u * P.inv_dx;
+                const float su = hdt * gw[1] * fdiv(qc.A.x, rho);
+                Wr = Wr + bc(k * db.x); Wp = Wp + bc(k * db.y); Wu = Wu + bc(su);
             }
         }
-        // ---- I: Riemann problem at face (n-4)+1/2 : L = WLc (cell n-4), R = WR (cell n-3) -------------
-        float Fr[5];
+        // ---- I: Riemann problem at face (n-4)+1/2 : L = left state carried from cell n-4, R = right state of cell n-3
+        float Frm, Frn, FrE;
+        v2 FrB;
         {
-            const float rL = fmaxf(r0fc + WLc[0], P.rho_floor), rR = fmaxf(r0fc + WR[0], P.rho_floor);
-            const float pfl = P.p_floor - p0fc;
-            const float ppL = fmaxf(WLc[4], pfl), ppR = fmaxf(WR[4], pfl);           // p' (floored)
-            const float pL = p0fc + ppL, pR = p0fc + ppR;
-            const float uL = WLc[1], uR = WR[1];
-            const float CL2 = gam * pL * rL, CR2 = gam * pR * rR;
-            const float CL = fsqrt(CL2), CR = fsqrt(CR2);
-            float pps = fmaxf(pfl, fdiv(CR * ppL + CL * ppR + CL * CR * (uL - uR), CL + CR));   // p*' acoustic guess
-            const float gpL = gp * rL, gpR = gp * rR, gmL = gm * pL * rL, gmR = gm * pR * rR;
+            const float r0f = b0fc.x, p0f = b0fc.y;
+            const float pfl = P.p_floor - p0f;
+            const v2 Zu = mk(WLu, Wu.y);
+            v2 r = bc(r0f) + mk(WLr, Wr.y);
+            r = mk(fmaxf(r.x, P.rho_floor), fmaxf(r.y, P.rho_floor));
+            const v2 pp = mk(fmaxf(WLp, pfl), fmaxf(Wp.y, pfl));              // p' (floored)
+            const v2 p = bc(p0f) + pp;
+            const v2 C2 = (p * gam) * r;
+            const v2 C = C2 * mk(rsqrtf(fmaxf(C2.x, 1e-37f)), rsqrtf(fmaxf(C2.y, 1e-37f)));
+            const float CLR = C.x * C.y;
+            float pps = fmaxf(pfl, fdiv(hsum(swp(C) * pp) + CLR * (Zu.x - Zu.y), C.x + C.y));   // p*' acoustic guess
+            const v2 gpr = r * gp, gmr = C2 * gmg;
             // Newton on p*' with the two-shock wave speeds W_K; at most 5 iterations (reading R7).  The loop
             // stops early only when EVERY lane's last update is below fp32 resolution of p* (warp-uniform
             // exit), i.e. when further iterations could not change the result beyond rounding.
             auto newton = [&]() -> bool {
-                const float ps = p0fc + pps;
-                const float wl2 = fmaf(gpL, ps, gmL), wr2 = fmaf(gpR, ps, gmR);
-                const float iwl = rsqrtf(wl2), iwr = rsqrtf(wr2);
-                const float usl = uL - (pps - ppL) * iwl, usr = uR + (pps - ppR) * iwr;
-                // 1/Z_K = (W^2 + C^2) / (2 W^3)
-                const float izl = (wl2 + CL2) * (iwl * iwl * iwl), izr = (wr2 + CR2) * (iwr * iwr * iwr);
-                const float d = fdiv(2.0f * (usr - usl), izl + izr);
+                const float ps = p0f + pps;
+                const v2 w2 = fma2(gpr, bc(ps), gmr);
+                const v2 iw = mk(rsqrtf(w2.x), rsqrtf(w2.y));
+                const v2 us = fma2(np(bc(pps) - pp), iw, Zu);               // u*_L = uL - (p*-pL)/W_L, u*_R = uR + (p*-pR)/W_R
+                const v2 iz = (w2 + C2) * ((iw * iw) * iw);                   // 1/Z_K = (W^2 + C^2) / (2 W^3), times 2
+                const float d = fdiv(2.0f * (us.y - us.x), hsum(iz));
                 pps = fmaxf(pfl, pps - d);
                 return fabsf(d) <= 6e-8f * ps;
             };
@@ -388,16 +441,16 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 for (int it = 1; it < 5; ++it)
                     if (__all_sync(wmask, newton())) break;
             }
-            const float ps = p0fc + pps;
-            const float wl2 = fmaf(gpL, ps, gmL), wr2 = fmaf(gpR, ps, gmR);
-            const float WLs = fsqrt(wl2), WRs = fsqrt(wr2);
-            const float us = fdiv(WLs * uL + WRs * uR + (ppL - ppR), WLs + WRs);
+            const float ps = p0f + pps;
+            const v2 w2 = fma2(gpr, bc(ps), gmr);
+            const v2 Ws = w2 * mk(rsqrtf(fmaxf(w2.x, 1e-37f)), rsqrtf(fmaxf(w2.y, 1e-37f)));
+            const float us = fdiv(hsum(Ws * Zu) + (pp.x - pp.y), hsum(Ws));
             // sampling at x/t = 0 in the frame mirrored so that the upwind side K is on the left
             const bool left = us >= 0.f;
             const float sg = left ? 1.f : -1.f;
-            const float rK = left ? rL : rR, uK = left ? uL : uR, pK = left ? pL : pR, ppK = left ? ppL : ppR;
-            const float wk2 = left ? wl2 : wr2, WK = left ? WLs : WRs;
-            const float vK = left ? WLc[2] : WR[2], wK = left ? WLc[3] : WR[3];
+            const float rK = left ? r.x : r.y, uK = left ? Zu.x : Zu.y, pK = left ? p.x : p.y, ppK = left ? pp.x : pp.y;
+            const float wk2 = left ? w2.x : w2.y, WK = left ? Ws.x : Ws.y;
+            const v2 vw = mk(left ? WLv : Wv.y, left ? WLw : Ww.y);
             float rs = fdiv(rK * wk2, wk2 - rK * (pps - ppK));                 // 1/(1/rK - (p*-pK)/WK^2)
             rs = fmaxf(rs, P.rho_floor);
             const float irK = rcp(rK);
@@ -410,66 +463,66 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const float rh = fmaf(th, rs - rK, rK);
             const float uh = fmaf(th, us - uK, uK);
             const float pph = fmaf(th, pps - ppK, ppK);
-            const float ph = p0fc + pph;
+            const float ph = p0f + pph;
             const float Fm = rh * uh;
-            Fr[0] = Fm;
-            Fr[1] = fmaf(Fm, uh, pph);
-            Fr[2] = Fm * vK;
-            Fr[3] = Fm * wK;
-            Fr[4] = uh * fmaf(g_gm1, ph, 0.5f * rh * (uh * uh + vK * vK + wK * wK));
+            Frm = Fm;
+            Frn = fmaf(Fm, uh, pph);
+            FrB = vw * Fm;
+            FrE = uh * fmaf(g_gm1, ph, 0.5f * rh * fmaf(uh, uh, hsum(vw * vw)));
         }
         // ---- K (first half): PPB coefficients of cell n-3, pre-limited (P2) ---------------------------
-#pragma unroll
-        for (int k = 0; k < 10; ++k) { mw[0][k] = mw[1][k]; mw[1][k] = mw[2][k]; }
+        mw[0] = mw[1]; mw[1] = mw[2];
         if (n - 3 >= c0 - 1) {
             float m[10];
             io.ppb(n - 3, m);
             // bound B: first-order terms 1/2, pure second-order 1/6, mixed 1/4.
             // local order: a1,b0,c0 are P1 terms; a2,d0,e0 are P2 terms; b1,c1,f0 are mixed P1P1 terms.
-            const float B = 0.5f * (fabsf(m[1]) + fabsf(m[3]) + fabsf(m[5])) + (1.0f / 6.0f) * (fabsf(m[2]) + fabsf(m[7]) + fabsf(m[8]))
-                          + 0.25f * (fabsf(m[4]) + fabsf(m[6]) + fabsf(m[9]));
+            const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
+            const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
+            const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
             const float th = fminf(1.0f, fdiv(fmaxf(0.f, fminf(m[0], 1.0f - m[0])), fmaxf(B, PPM_TINY)));
-            mw[2][0] = m[0];
-#pragma unroll
-            for (int k = 1; k < 10; ++k) mw[2][k] = m[k] * th;
+            // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
+            asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
+            mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+            mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
+            io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
         }
         // ---- J, K, L: finish cell n-4 ---------------------------------------------------------------------
         const int i = n - PPM_NGHOST;
         if (i >= c0) {
-            const float r_old = rf[1], rp_old = q[0][0], u0 = q[1][0], v0 = q[2][0], w0 = q[3][0], g = gw[0];
-            float drho = -dtdx * (Fr[0] - Fl[0]);
+            const float r_old = rf[1], rp_old = q[0].A.x, pp_old = q[0].A.y, u0 = q[0].u, g = gw[0];
+            const v2 vw0 = q[0].B;
+            float drho = -dtdx * (Frm - Flm);
             int bad = 0;
             if (!(r_old + drho > P.rho_floor)) { drho = P.rho_floor - r_old; bad = 1; }
             const float r_new = r_old + drho;
             const float rp_new = rp_old + drho;
             const float mu0 = r_old * u0;
-            float mu1 = mu0 - dtdx * (Fr[1] - Fl[1]);
-            float dE = -dtdx * (Fr[4] - Fl[4]);
+            float mu1 = mu0 - dtdx * (Frn - Fln);
+            float dE = -dtdx * (FrE - FlE);
             if (GRAV != PPM_GRAV_NONE) {
                 mu1 += P.dt * 0.5f * (rp_old + rp_new) * g;
                 dE += P.dt * 0.5f * (mu0 + mu1) * g;
             }
-            const float mv1 = r_old * v0 - dtdx * (Fr[2] - Fl[2]);
-            const float mw1 = r_old * w0 - dtdx * (Fr[3] - Fl[3]);
+            const v2 mB = fma2(FrB - FlB, bc(-dtdx), vw0 * r_old);
             const float irn = rcp(r_new);
             float ho[5], mo[10];
-            const float u1 = mu1 * irn, v1 = mv1 * irn, w1 = mw1 * irn;
-            const float dKE = 0.5f * (r_new * (u1 * u1 + v1 * v1 + w1 * w1) - r_old * (u0 * u0 + v0 * v0 + w0 * w0));
-            float pp_new = q[4][0] + (gam - 1.0f) * (dE - dKE);
-            const float p0c = pf[0] - q[4][0];
+            const float u1 = mu1 * irn;
+            const v2 vw1 = mB * irn;
+            const float dKE = 0.5f * (r_new * fmaf(u1, u1, hsum(vw1 * vw1)) - r_old * fmaf(u0, u0, hsum(vw0 * vw0)));
+            float pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
+            const float p0c = pf[0] - pp_old;
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
-            ho[0] = rp_new; ho[1] = u1; ho[2] = v1; ho[3] = w1; ho[4] = pp_new;
-            ppb_remap(mw, rf[0], rf[1], rf[2], dtdx * Fl[0], dtdx * Fr[0], mo);
+            ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
+            ppb_remap(mw, rf[0], rf[1], rf[2], dtdx * Flm, dtdx * Frm, mo);
             io.store(i, ho, mo);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
-#pragma unroll
-        for (int k = 0; k < 5; ++k) {
-            d2a[k] = d2b[k]; d2b[k] = d2n[k]; Fc[k] = Fn[k]; Fcl[k] = Fnl[k]; parL[k] = pLn[k]; parR[k] = pRn[k];
-            WLc[k] = WL[k]; Fl[k] = Fr[k];
-        }
-        ft0 = ft1; ft1 = ftn; cs = cn2; r0fc = r0fn; p0fc = p0fn;
+        d2a = d2b; d2b = d2n; Fc = Fn; Fcl = Fnl; parL = pLn; parR = pRn;
+        WLr = Wr.x; WLu = Wu.x; WLp = Wp.x; WLv = Wv.x; WLw = Ww.x;
+        Flm = Frm; Fln = Frn; FlE = FrE; FlB = FrB;
+        ft0 = ft1; ft1 = ftn; cs = cn2; b0fc = b0fn;
         io.end(n);
     }
     io.finish();
@@ -511,11 +564,22 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) nm[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
     }
-    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
+    __device__ __forceinline__ void ppb(int, float (&m)[10]) {
 #pragma unroll
         for (int k = 0; k < 10; ++k) m[k] = nm[k];
         m[1] *= snm; m[4] *= snm; m[6] *= snm;
-        fetch_ppb(c + 1);    // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
+    }
+    // Issues the loads of cell c one iteration ahead of their use.  `used` = the values computed from the
+    // previous prefetch: the empty asm orders the new loads after them, so the loads land in the very
+    // registers the old values just left (otherwise ptxas hoists the loads above the last use, renames them,
+    // and parks a register copy — which waits for DRAM — right behind the loads).
+    __device__ __forceinline__ void ppb_prefetch(int c, const PpbCell& used) {
+        const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, snm);
+        unsigned id = pbase + axis_off(P, j);
+        asm volatile("" : "+r"(id) : "f"(used.a0), "f"(used.a1), "f"(used.a2), "f"(used.f), "f"(used.bc0.x), "f"(used.bc0.y),
+                     "f"(used.bc1.x), "f"(used.bc1.y), "f"(used.de.x), "f"(used.de.y));
+#pragma unroll
+        for (int k = 0; k < 10; ++k) nm[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
     }
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
         const unsigned id = pbase + axis_off(P, i);
@@ -676,6 +740,7 @@ struct IoTmaX {
         for (int q = 0; q < 10; ++q) m[q] = src[PPB_PERM[0][q] * TX_ROWS * TX_CH];
         m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
     }
+    __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
         const int s = i & 3;
         if (s == 0 && store_pending) {                         // the previous chunk's TMA store must have read outb
