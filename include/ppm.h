@@ -19,7 +19,8 @@
  *    (fields[]) are borrowed for the duration of the call only.
  *
  * State at the boundary (ppm_set_state / ppm_get_state): 15 fp32 fields per cell, each a dense [nz][ny][nx]
- * array, x fastest.  Inside the two borrowed buffers the library keeps them as SoA bricks.
+ * array, x fastest.  Inside the two borrowed buffers the library keeps them as brick records: 4x4x4 cells x
+ * 15 fields per 3840-byte brick, extents rounded up to whole bricks.
  *   0 rho  1 ux  2 uy  3 uz  4 p   5..14 = m000 m100 m010 m001 m200 m020 m002 m110 m101 m011
  * where m_abc are the coefficients of FV in the cell-local Legendre basis P0=1, P1=s, P2=s^2-1/12
  * on [-1/2,1/2]^3 (m000 = cell mean; "cell average and its 9 lowest-order moments").
@@ -68,8 +69,13 @@ typedef struct {
     void *stream; /* cudaStream_t the library enqueues on (0 = default stream) */
 } ppm_params;
 
+/* Number of floats each of the two state buffers must hold for an nx x ny x nz grid:
+ * 15 * 64 * ceil(nx/4) * ceil(ny/4) * ceil(nz/4)  (= 15*nx*ny*nz when the extents are multiples of 4).
+ * Returns 0 for a non-positive extent.  Pure host arithmetic; needs no device. */
+size_t ppm_state_floats(int nx, int ny, int nz);
+
 /* Creates a context.  dev_buf_a, dev_buf_b: [device] two caller-owned buffers of
- * 15*nx*ny*nz floats each, 16-byte aligned (e.g. torch tensors).  The library BORROWS them for the
+ * ppm_state_floats(nx,ny,nz) floats each, 128-byte aligned (e.g. torch tensors).  The library BORROWS them for the
  * life of the context: the state lives in one, the other is sweep scratch, and they ping-pong.  It
  * never frees them.  Contents are undefined until ppm_set_state has covered every z-slab. */
 int ppm_create(ppm_ctx **out, const ppm_params *prm, float *dev_buf_a, float *dev_buf_b);
@@ -106,12 +112,9 @@ int ppm_sync(ppm_ctx *ctx);
 int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
 
 /* Options (results do not depend on them).
- *  PPM_OPT_X_PATH : 0 = automatic (brick layout: the x sweep stages whole 256-byte bricks through shared
- *                   memory with TMA), 1 = force the direct global-memory path.
- *  PPM_OPT_LAYOUT : internal layout of the two borrowed buffers; 0 = automatic (SoA bricks of 4x4x4 cells
- *                   when nx, ny, nz are multiples of 4, SoA planes otherwise), 1 = force SoA planes.  Only
- *                   before the first ppm_set_state. */
-enum { PPM_OPT_X_PATH = 1, PPM_OPT_LAYOUT = 2 };
+ *  PPM_OPT_X_PATH : 0 = automatic (nx a multiple of 4: the x sweep stages whole bricks through shared
+ *                   memory with TMA), 1 = force the direct global-memory path. */
+enum { PPM_OPT_X_PATH = 1 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* 1 if the next x sweep will take the TMA-staged path, 0 if the direct path. */
 int ppm_x_path(const ppm_ctx *ctx);

@@ -13,7 +13,8 @@ import numpy as np
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libppm_b200.so")
+# PPM_B200_LIB: load another build of the same library (e.g. one compiled with different tuning knobs)
+LIB_PATH = os.environ.get("PPM_B200_LIB") or os.path.join(HERE, "libppm_b200.so")
 
 PPM_OK, PPM_EINVAL, PPM_ENOMEM, PPM_ECUDA, PPM_ESTATE = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_REFLECT = 0, 1
@@ -21,8 +22,8 @@ GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_x_path", "ppm_launch_count",
-           "ppm_destroy", "ppm_last_error")
-OPT_X_PATH, OPT_LAYOUT = 1, 2
+           "ppm_state_floats", "ppm_destroy", "ppm_last_error")
+OPT_X_PATH = 1
 
 
 class ppm_gravity(C.Structure):
@@ -49,6 +50,8 @@ def lib():
                               "(there is no CPU fallback)")
         L = C.CDLL(LIB_PATH)
         fpp = C.POINTER(C.POINTER(C.c_float))
+        L.ppm_state_floats.argtypes = [C.c_int, C.c_int, C.c_int]
+        L.ppm_state_floats.restype = C.c_size_t
         L.ppm_create.argtypes = [C.POINTER(C.c_void_p), C.POINTER(ppm_params), C.c_void_p, C.c_void_p]
         L.ppm_set_state.argtypes = [C.c_void_p, fpp, C.c_int, C.c_int, C.c_int]
         L.ppm_get_state.argtypes = [C.c_void_p, fpp, C.c_int, C.c_int, C.c_int]
@@ -111,9 +114,10 @@ class PPM:
         self.n = (int(nx), int(ny), int(nz))
         self.ncell = int(nx) * int(ny) * int(nz)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        nfl = int(lib().ppm_state_floats(int(nx), int(ny), int(nz)))
         with torch.cuda.device(self.device):
-            self.buf_a = torch.empty(NF * self.ncell, dtype=torch.float32, device=self.device)
-            self.buf_b = torch.empty(NF * self.ncell, dtype=torch.float32, device=self.device)
+            self.buf_a = torch.empty(nfl, dtype=torch.float32, device=self.device)
+            self.buf_b = torch.empty(nfl, dtype=torch.float32, device=self.device)
         prm, keep = make_params(nx, ny, nz, dx, gamma, bc, grav, rho_floor, p_floor, self.stream.cuda_stream)
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):

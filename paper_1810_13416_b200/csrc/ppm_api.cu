@@ -31,6 +31,11 @@ static const int ORDERS[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2,
 
 extern "C" const char* ppm_last_error(const ppm_ctx* c) { return c ? c->err : g_err; }
 
+extern "C" size_t ppm_state_floats(int nx, int ny, int nz) {
+    if (nx < 1 || ny < 1 || nz < 1) return 0;
+    return (size_t)((nx + 3) / 4) * (size_t)((ny + 3) / 4) * (size_t)((nz + 3) / 4) * PPM_BRICK_FLOATS;
+}
+
 extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a, float* dev_buf_b) {
     ppm_ctx* c = nullptr;
     if (!out) { set_err(c, "ppm_create: out is NULL"); return PPM_EINVAL; }
@@ -38,11 +43,11 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     if (!prm || !dev_buf_a || !dev_buf_b || dev_buf_a == dev_buf_b) { set_err(c, "ppm_create: NULL or aliased argument"); return PPM_EINVAL; }
     if (prm->struct_size != sizeof(ppm_params)) { set_err(c, "ppm_create: struct_size %zu != %zu", prm->struct_size, sizeof(ppm_params)); return PPM_EINVAL; }
     if (prm->nx < 1 || prm->ny < 1 || prm->nz < 1) { set_err(c, "ppm_create: grid dims must be >= 1"); return PPM_EINVAL; }
-    if ((long long)prm->nx * prm->ny * prm->nz >= (1LL << 31)) { set_err(c, "ppm_create: more than 2^31 - 1 cells (32-bit in-field offsets; 2 x 15 such fields would not fit one GPU anyway)"); return PPM_EINVAL; }
+    if ((long long)prm->nx * prm->ny * prm->nz >= (1LL << 31)) { set_err(c, "ppm_create: more than 2^31 - 1 cells (2 x 15 such fields would not fit one GPU anyway)"); return PPM_EINVAL; }
     if (!(prm->dx > 0.0) || !(prm->gamma > 1.0) || !(prm->rho_floor > 0.0) || !(prm->p_floor > 0.0)) {
         set_err(c, "ppm_create: need dx > 0, gamma > 1, floors > 0"); return PPM_EINVAL;
     }
-    if (((uintptr_t)dev_buf_a | (uintptr_t)dev_buf_b) & 15) { set_err(c, "ppm_create: device buffers must be 16-byte aligned"); return PPM_EINVAL; }
+    if (((uintptr_t)dev_buf_a | (uintptr_t)dev_buf_b) & 127) { set_err(c, "ppm_create: device buffers must be 128-byte aligned"); return PPM_EINVAL; }
     const int ext[3] = {prm->nx, prm->ny, prm->nz};
     for (int d = 0; d < 3; ++d) {
         const int lo = prm->bc[2 * d], hi = prm->bc[2 * d + 1];
@@ -77,9 +82,8 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c->nblocks_red = 148 * 4;
     c->chunk = 0;
     c->err[0] = 0;
-    // SoA bricks of 4x4x4 cells when every extent is a multiple of 4 (every sweep direction then touches
-    // whole 256-byte bricks); SoA planes otherwise
-    c->layout = (prm->nx % 4 == 0 && prm->ny % 4 == 0 && prm->nz % 4 == 0) ? 1 : 0;
+    // brick records of 4x4x4 cells x 15 fields; extents are rounded up to whole bricks (ppm_state_floats)
+    c->nbx = (prm->nx + 3) / 4; c->nby = (prm->ny + 3) / 4; c->nbz = (prm->nz + 3) / 4;
     cudaError_t e;
 #define CUC(call) do { e = (call); if (e != cudaSuccess) { set_err(nullptr, "%s failed: %s", #call, cudaGetErrorString(e)); ppm_destroy(c); return e == cudaErrorMemoryAllocation ? PPM_ENOMEM : PPM_ECUDA; } } while (0)
     CUC(cudaMalloc(&c->flag, sizeof(int)));
@@ -131,16 +135,14 @@ extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS],
     int rc = check_slab(c, fields, z0, nzs, "ppm_set_state");
     if (rc) return rc;
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_set_state: fields[%d] is NULL", f); return PPM_EINVAL; }
-    const long long plane = (long long)c->prm.nx * c->prm.ny, ncell = plane * c->prm.nz;
+    const long long plane = (long long)c->prm.nx * c->prm.ny;
     float* st = c->buf[c->cur];
     float* scratch = c->buf[c->cur ^ 1];    // free between steps: stages the dense slab
-    (void)ncell;
     const long long tot = plane * nzs;
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     for (int f = 0; f < PPM_NFIELDS; ++f)
         CU(cudaMemcpyAsync(scratch + f * tot, fields[f], sizeof(float) * tot, kind, c->stream));
     CU(ppm_launch_to_perturbation(c, scratch, st, z0, nzs));
-    c->layout_locked = 1;
     CU(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
     return PPM_OK;
 }
@@ -210,14 +212,6 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
     if (option == PPM_OPT_X_PATH && (value == 0 || value == 1)) { c->force_direct = value; return PPM_OK; }
-    if (option == PPM_OPT_LAYOUT && (value == 0 || value == 1)) {
-        if (c->layout_locked) { set_err(c, "ppm_set_option: the layout cannot change once a state is loaded"); return PPM_EINVAL; }
-        const ppm_params& p = c->prm;
-        if (value == 0 && (p.nx % 4 || p.ny % 4 || p.nz % 4)) { set_err(c, "ppm_set_option: bricks need extents that are multiples of 4"); return PPM_EINVAL; }
-        c->layout = value == 0 ? 1 : 0;
-        ppm_make_xmaps(c);
-        return PPM_OK;
-    }
     set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
     return PPM_EINVAL;
 }

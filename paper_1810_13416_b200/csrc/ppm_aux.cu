@@ -6,34 +6,28 @@ namespace {
 
 struct AuxParams {
     int nx, ny, nz;
-    long long ncell;
+    long long nslots;                   // storage slots = bricks * 64 (pad cells included)
     double dx, gamma;
     int grav_kind, tab_n;
     double s0, ds, cx, cy, cz;
     const double* __restrict__ tab64;   // node k: g, rho0, p0 (3 doubles)
-    int layout, nbx, nby;               // 1 = 4x4x4 bricks (all extents multiples of 4)
+    int nbx, nby;                       // bricks along x, y
 };
 
-// storage offset of cell (i,j,k) inside one field
+// float offset of field 0 of cell (i,j,k): brick record [bz][by][bx][15][4z][4y][4x]; field f is 64*f further
 __device__ __forceinline__ long long cell_offset(const AuxParams& A, int i, int j, int k) {
-    if (A.layout == 0) return ((long long)k * A.ny + j) * A.nx + i;
-    return ((((long long)(k >> 2) * A.nby + (j >> 2)) * A.nbx + (i >> 2)) << 6) + ((k & 3) << 4 | (j & 3) << 2 | (i & 3));
+    return (((long long)(k >> 2) * A.nby + (j >> 2)) * A.nbx + (i >> 2)) * PPM_BRICK_FLOATS + ((k & 3) << 4 | (j & 3) << 2 | (i & 3));
 }
-// inverse: storage index t (0 .. ncell) -> (i,j,k); both layouts are dense (no padding)
-__device__ __forceinline__ void cell_of(const AuxParams& A, long long t, int& i, int& j, int& k) {
-    if (A.layout == 0) {
-        const long long plane = (long long)A.nx * A.ny;
-        k = (int)(t / plane);
-        const long long rem = t % plane;
-        j = (int)(rem / A.nx); i = (int)(rem % A.nx);
-    } else {
-        const int c = (int)(t & 63);
-        long long B = t >> 6;
-        const int bx = (int)(B % A.nbx); B /= A.nbx;
-        const int by = (int)(B % A.nby);
-        const int bz = (int)(B / A.nby);
-        i = bx * 4 + (c & 3); j = by * 4 + ((c >> 2) & 3); k = bz * 4 + (c >> 4);
-    }
+// storage slot t (brick * 64 + cell in brick) -> (i,j,k) and the offset of field 0; false for a pad cell
+__device__ __forceinline__ bool cell_of(const AuxParams& A, long long t, int& i, int& j, int& k, long long& off) {
+    const int c = (int)(t & 63);
+    long long B = t >> 6;
+    off = B * PPM_BRICK_FLOATS + c;
+    const int bx = (int)(B % A.nbx); B /= A.nbx;
+    const int by = (int)(B % A.nby);
+    const int bz = (int)(B / A.nby);
+    i = bx * 4 + (c & 3); j = by * 4 + ((c >> 2) & 3); k = bz * 4 + (c >> 4);
+    return i < A.nx && j < A.ny && k < A.nz;
 }
 
 // fp64 base state at a cell centre (same definition as the sweep's, evaluated in double: the
@@ -71,7 +65,7 @@ __global__ void __launch_bounds__(256) to_perturbation_kernel(AuxParams A, const
             float v = src[f * tot + t];
             if (f == 0) v = (float)((double)v - r0);
             if (f == 4) v = (float)((double)v - p0);
-            st[f * A.ncell + id] = v;
+            st[id + 64 * f] = v;
         }
     }
 }
@@ -88,7 +82,7 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
         base64(A, i, j, k, r0, p0);
 #pragma unroll
         for (int f = 0; f < PPM_NFIELDS; ++f) {
-            float v = st[f * A.ncell + id];
+            float v = st[id + 64 * f];
             if (f == 0) v = (float)((double)v + r0);
             if (f == 4) v = (float)((double)v + p0);
             dst[f * tot + t] = v;
@@ -102,14 +96,15 @@ __device__ __forceinline__ unsigned int enc(float x) { return __float_as_uint(fm
 __global__ void __launch_bounds__(256) cfl_kernel(AuxParams A, const float* __restrict__ st, unsigned int* __restrict__ out, int* flag) {
     float vmax = 0.f;
     const float gam = (float)A.gamma;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.ncell; t += (long long)gridDim.x * blockDim.x) {
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
         int i, j, k;
-        cell_of(A, t, i, j, k);
+        long long o;
+        if (!cell_of(A, t, i, j, k, o)) continue;
         double r0, p0;
         base64(A, i, j, k, r0, p0);
-        const float rho = (float)(r0 + (double)st[t]), p = (float)(p0 + (double)st[4 * A.ncell + t]);
+        const float rho = (float)(r0 + (double)st[o]), p = (float)(p0 + (double)st[o + 4 * 64]);
         const float c = sqrtf(gam * p / rho);
-        const float um = fmaxf(fabsf(st[A.ncell + t]), fmaxf(fabsf(st[2 * A.ncell + t]), fabsf(st[3 * A.ncell + t])));
+        const float um = fmaxf(fabsf(st[o + 64]), fmaxf(fabsf(st[o + 2 * 64]), fabsf(st[o + 3 * 64])));
         const float v = um + c;
         if (!(v == v) || !(rho > 0.f) || !(p > 0.f)) atomicOr(flag, 2);
         vmax = fmaxf(vmax, v);
@@ -130,16 +125,17 @@ __global__ void __launch_bounds__(256) cfl_kernel(AuxParams A, const float* __re
 // conserved sums: fp64 accumulation, fixed assignment of cells to threads, fixed reduction trees
 __global__ void __launch_bounds__(256) conserved_kernel(AuxParams A, const float* __restrict__ st, double* __restrict__ partial) {
     double acc[6] = {0, 0, 0, 0, 0, 0};
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.ncell; t += (long long)gridDim.x * blockDim.x) {
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
         int i, j, k;
-        cell_of(A, t, i, j, k);
+        long long o;
+        if (!cell_of(A, t, i, j, k, o)) continue;
         double r0, p0;
         base64(A, i, j, k, r0, p0);
-        const double rho = r0 + (double)st[t], p = p0 + (double)st[4 * A.ncell + t];
-        const double u = st[A.ncell + t], v = st[2 * A.ncell + t], w = st[3 * A.ncell + t];
+        const double rho = r0 + (double)st[o], p = p0 + (double)st[o + 4 * 64];
+        const double u = st[o + 64], v = st[o + 2 * 64], w = st[o + 3 * 64];
         acc[0] += rho; acc[1] += rho * u; acc[2] += rho * v; acc[3] += rho * w;
         acc[4] += p / (A.gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w);
-        acc[5] += rho * (double)st[5 * A.ncell + t];
+        acc[5] += rho * (double)st[o + 5 * 64];
     }
     __shared__ double sm[6][256];
 #pragma unroll
@@ -168,13 +164,13 @@ AuxParams make_aux(const ppm_ctx* c) {
     AuxParams A;
     const ppm_params& p = c->prm;
     A.nx = p.nx; A.ny = p.ny; A.nz = p.nz;
-    A.ncell = (long long)p.nx * p.ny * p.nz;
+    A.nslots = (long long)c->nbx * c->nby * c->nbz * 64;
     A.dx = p.dx; A.gamma = p.gamma;
     A.grav_kind = p.grav.kind; A.tab_n = p.grav.n;
     A.s0 = p.grav.s0; A.ds = p.grav.ds;
     A.cx = p.grav.center[0]; A.cy = p.grav.center[1]; A.cz = p.grav.center[2];
     A.tab64 = c->tab64;
-    A.layout = c->layout; A.nbx = (p.nx + 3) / 4; A.nby = (p.ny + 3) / 4;
+    A.nbx = c->nbx; A.nby = c->nby;
     return A;
 }
 
@@ -204,16 +200,14 @@ cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z
 cudaError_t ppm_launch_cfl(ppm_ctx* c) {
     cudaError_t e = cudaMemsetAsync(c->cflmax, 0, sizeof(unsigned int), c->stream);
     if (e != cudaSuccess) return e;
-    const long long n = (long long)c->prm.nx * c->prm.ny * c->prm.nz;
+    const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
     cfl_kernel<<<grid_for(n, 148 * 8), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->cflmax, c->flag);
     c->launches += 1;
     return cudaGetLastError();
 }
 
 cudaError_t ppm_launch_conserved(ppm_ctx* c) {
-    const long long n = (long long)c->prm.nx * c->prm.ny * c->prm.nz;
     const int nb = c->nblocks_red;
-    (void)n;
     conserved_kernel<<<nb, 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->partial);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

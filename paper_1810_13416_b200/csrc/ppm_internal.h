@@ -8,21 +8,24 @@
 
 #define PPM_TINY 1e-30f
 
+// State layout inside each borrowed buffer ("brick records"): the grid is cut into bricks of 4x4x4 cells
+// (extents rounded up to multiples of 4; pad cells are never read or written by the sweeps) and a brick
+// holds all 15 fields of its 64 cells, field-major:   [bz][by][bx][field 15][4z][4y][4x]   (3840 B per brick).
+// A cell's 15 values are 256 B apart, so one 64-bit pointer plus compile-time offsets addresses all of them,
+// and every sweep direction reads and writes whole 64-byte brick layers.
+#define PPM_BRICK_FLOATS (PPM_NFIELDS * 64)
+
 // Per-launch parameters of one directional sweep (passed by value as a kernel argument).
 struct SweepParams {
-    const float* inf[PPM_NFIELDS];  // 15 field planes, SoA, perturbation form
-    float* outf[PPM_NFIELDS];
-    long long ncell;                // nx*ny*nz (field stride)
+    const float* in;                // state, perturbation form
+    float* out;
     int n;                          // cells along the sweep axis
-    int na, nb;                     // transverse extents: a is mapped to threads, b to blockIdx.y
-    // element offset of cell (j along the sweep axis, a, b) inside a field plane set:
-    //   (j>>2)*SBd + (j&3)*SId + (a>>2)*SBa + (a&3)*SIa + (b>>2)*SBb + (b&3)*SIb
-    // brick layout: SB = stride between 4x4x4 bricks (256 B each), SI = stride inside a brick;
-    // plane layout: SB = 4*stride, SI = stride.
+    int na, nb;                     // transverse extents: a and b index the 4x4 pencils of a brick column
+    // float offset of cell (j along the sweep axis, a, b), field f:
+    //   (j>>2)*SBd + ((j&3) << 2*axis_d) + (a>>2)*SBa + ((a&3) << 2*axis_a) + (b>>2)*SBb + ((b&3) << 2*axis_b) + 64*f
+    // SB = stride between bricks along that axis (960, 960*nbx, 960*nbx*nby floats)
     long long SBd, SBa, SBb;
-    int SId, SIa, SIb;
-    int brick;                      // 1: threads map to in-brick coordinates (4 a x 4 b per 16 lanes)
-    int nbrick_d;                   // bricks along the sweep axis (brick layout)
+    int nbrick_d;                   // bricks along the sweep axis
     int bc_lo, bc_hi;
     int chunk;                      // cells marched per thread (pencil split along the sweep axis)
     float dt, dx, dtdx, inv_dx;
@@ -48,13 +51,12 @@ struct ppm_ctx {
     double* result;                 // device: final 6 sums
     int nblocks_red;
     int chunk;
-    int layout;                     // 0 = SoA planes [f][z][y][x]; 1 = SoA bricks [f][bz][by][bx][4z][4y][4x]
-    int layout_locked;              // set once a state has been loaded
+    int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
     int tma_ok;                     // tensor maps for the x-sweep TMA path are valid
     int force_direct;               // option: take the direct-global x path even when TMA is available
     long long launches;
     char err[512];
-    alignas(64) unsigned char xmap[2][128];   // CUtensorMap of buf[0], buf[1]: 5-D {64, nbx, nby, nbz, 15}, box {64,1,2,1,5}
+    alignas(64) unsigned char xmap[2][128];   // CUtensorMap of buf[0], buf[1]: 5-D {64, 15, nbx, nby, nbz}, box {64,5,1,2,1}
 };
 
 // launchers (defined in the .cu files)

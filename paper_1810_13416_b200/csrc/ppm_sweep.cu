@@ -43,6 +43,15 @@
 #ifndef PPM_MARCH_UNROLL
 #define PPM_MARCH_UNROLL 1
 #endif
+// direct-path CTA shape (build knobs): threads per CTA (a multiple of 16 = one brick column; the kernel uses no
+// shared memory and no block-wide sync, so the CTA size only sets the granularity of occupancy) and the register
+// cap per thread (65536 / (cap rounded up to 8) / 32 = resident warps per SM)
+#ifndef PPM_CTA
+#define PPM_CTA 128
+#endif
+#ifndef PPM_MAXREG
+#define PPM_MAXREG 168
+#endif
 
 namespace {
 
@@ -102,21 +111,31 @@ template <class F> __device__ __forceinline__ V5 map3(const V5& a, const V5& b, 
     V5 r; r.A = mk(f(a.A.x, b.A.x, c.A.x), f(a.A.y, b.A.y, c.A.y)); r.B = mk(f(a.B.x, b.B.x, c.B.x), f(a.B.y, b.B.y, c.B.y)); r.u = f(a.u, b.u, c.u); return r;
 }
 
-// image of a cell / face index outside [0, n) under the boundary condition (C3)
+// image of a cell / face index outside [0, n) under the boundary condition (C3).  The index is the same for
+// every lane of a warp; all but the 8 ghost iterations of a pencil take the first return.
 __device__ __forceinline__ int image_cell(int i, int n, int bc_lo, int bc_hi, float& sgn) {
     sgn = 1.0f;
-    if (i >= 0 && i < n) return i;
+    if ((unsigned)i < (unsigned)n) return i;
     const int bcx = (i < 0) ? bc_lo : bc_hi;
-    if (bcx == PPM_BC_PERIODIC) return ((i % n) + n) % n;
+    if (bcx == PPM_BC_PERIODIC) {
+        i += (i < 0) ? n : -n;
+        if ((unsigned)i >= (unsigned)n) i = ((i % n) + n) % n;      // fewer cells than ghosts
+        return i;
+    }
     sgn = -1.0f;
-    int s = (i < 0) ? (-1 - i) : (2 * n - 1 - i);
+    const int s = (i < 0) ? (-1 - i) : (2 * n - 1 - i);
     return min(max(s, 0), n - 1);
 }
 __device__ __forceinline__ int image_face(int f, int n, int bc_lo, int bc_hi) {
-    if (f >= 0 && f <= n) return (f == n && bc_hi == PPM_BC_PERIODIC) ? 0 : f;
+    if ((unsigned)f < (unsigned)n) return f;
+    if (f == n) return (bc_hi == PPM_BC_PERIODIC) ? 0 : f;
     const int bcx = (f < 0) ? bc_lo : bc_hi;
-    if (bcx == PPM_BC_PERIODIC) return ((f % n) + n) % n;
-    int s = (f < 0) ? -f : 2 * n - f;
+    if (bcx == PPM_BC_PERIODIC) {
+        f += (f < 0) ? n : -n;
+        if ((unsigned)f >= (unsigned)n) f = ((f % n) + n) % n;
+        return f;
+    }
+    const int s = (f < 0) ? -f : 2 * n - f;
     return min(max(s, 0), n);
 }
 
@@ -436,10 +455,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             };
             // first iteration in straight-line code (the scheduler can overlap it with independent work); the
             // remaining ones only while some lane still moves (rare at low Mach: the acoustic guess is nearly exact)
-            if (!__all_sync(wmask, newton())) {
+            // (lanes on pad cells of a ragged grid carry garbage and do not vote)
+            if (!__all_sync(wmask, newton() || !valid)) {
 #pragma unroll 1
                 for (int it = 1; it < 5; ++it)
-                    if (__all_sync(wmask, newton())) break;
+                    if (__all_sync(wmask, newton() || !valid)) break;
             }
             const float ps = p0f + pps;
             const v2 w2 = fma2(gpr, bc(ps), gmr);
@@ -529,26 +549,31 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 }
 
 // =====================================================================================================
-// IoDirect: straight global loads / stores, lanes along a contiguous axis; next plane prefetched.
+// IoDirect: straight global loads / stores.  16 lanes = the 4x4 pencils of one brick column; a load of one
+// field is one 64-byte brick layer per half warp.  A cell's 15 fields sit 256 B apart in its brick record, so
+// each of the three access streams (hydro plane n+1, PPB cell n-2, finished cell n-4) needs one pointer per
+// iteration and the fields are compile-time offsets.  Next plane / next PPB cell prefetched into registers.
 // =====================================================================================================
-__device__ __forceinline__ unsigned axis_off(const SweepParams& P, int j) { return (unsigned)(j >> 2) * (unsigned)P.SBd + (unsigned)(j & 3) * (unsigned)P.SId; }
-
 template <int DIR>
 struct IoDirect {
+    static constexpr int SH = 2 * DIR;       // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
-    const unsigned pbase;    // element offsets inside one field fit 32 bits (ppm_create checks)
+    const float* __restrict__ const pin;     // the thread's pencil: cell 0 of the sweep axis, field 0
+    float* __restrict__ const pout;
     float nx5[5];            // plane n+1, already in flight
     float nm[10];            // PPB coefficients of the next cell, already in flight
     int jn; float sn, snm;
-    __device__ __forceinline__ IoDirect(const SweepParams& P_, unsigned pb, int n0, int c0) : P(P_), pbase(pb) { fetch(n0); fetch_ppb(c0 - 1); }
+    __device__ __forceinline__ IoDirect(const SweepParams& P_, long long tb, int n0, int c0) : P(P_), pin(P_.in + tb), pout(P_.out + tb) { fetch(n0); fetch_ppb(c0 - 1); }
+    // float offset of cell j along the pencil (same for every lane)
+    __device__ __forceinline__ long long off(int j) const { return (long long)(j >> 2) * P.SBd + ((j & 3) << SH); }
     __device__ __forceinline__ void fetch(int n) {
         jn = image_cell(n, P.n, P.bc_lo, P.bc_hi, sn);
-        const unsigned id = pbase + axis_off(P, jn);
-        nx5[0] = __ldg(P.inf[0] + id);
-        nx5[1] = __ldg(P.inf[Dir<DIR>::U] + id);
-        nx5[2] = __ldg(P.inf[Dir<DIR>::V] + id);
-        nx5[3] = __ldg(P.inf[Dir<DIR>::W] + id);
-        nx5[4] = __ldg(P.inf[4] + id);
+        const float* __restrict__ p = pin + off(jn);
+        nx5[0] = __ldg(p);
+        nx5[1] = __ldg(p + 64 * Dir<DIR>::U);
+        nx5[2] = __ldg(p + 64 * Dir<DIR>::V);
+        nx5[3] = __ldg(p + 64 * Dir<DIR>::W);
+        nx5[4] = __ldg(p + 64 * 4);
     }
     __device__ __forceinline__ void begin(int) {}
     __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
@@ -560,9 +585,9 @@ struct IoDirect {
     }
     __device__ __forceinline__ void fetch_ppb(int c) {
         const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, snm);
-        const unsigned id = pbase + axis_off(P, j);
+        const float* __restrict__ p = pin + off(j);
 #pragma unroll
-        for (int k = 0; k < 10; ++k) nm[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
+        for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
     }
     __device__ __forceinline__ void ppb(int, float (&m)[10]) {
 #pragma unroll
@@ -575,50 +600,47 @@ struct IoDirect {
     // and parks a register copy — which waits for DRAM — right behind the loads).
     __device__ __forceinline__ void ppb_prefetch(int c, const PpbCell& used) {
         const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, snm);
-        unsigned id = pbase + axis_off(P, j);
-        asm volatile("" : "+r"(id) : "f"(used.a0), "f"(used.a1), "f"(used.a2), "f"(used.f), "f"(used.bc0.x), "f"(used.bc0.y),
+        const float* p = pin + off(j);
+        asm volatile("" : "+l"(p) : "f"(used.a0), "f"(used.a1), "f"(used.a2), "f"(used.f), "f"(used.bc0.x), "f"(used.bc0.y),
                      "f"(used.bc1.x), "f"(used.bc1.y), "f"(used.de.x), "f"(used.de.y));
 #pragma unroll
-        for (int k = 0; k < 10; ++k) nm[k] = __ldg(P.inf[5 + PPB_PERM[DIR][k]] + id);
+        for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
     }
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
-        const unsigned id = pbase + axis_off(P, i);
-        P.outf[0][id] = h[0];
-        P.outf[Dir<DIR>::U][id] = h[1];
-        P.outf[Dir<DIR>::V][id] = h[2];
-        P.outf[Dir<DIR>::W][id] = h[3];
-        P.outf[4][id] = h[4];
+        float* __restrict__ p = pout + off(i);
+        p[0] = h[0];
+        p[64 * Dir<DIR>::U] = h[1];
+        p[64 * Dir<DIR>::V] = h[2];
+        p[64 * Dir<DIR>::W] = h[3];
+        p[64 * 4] = h[4];
 #pragma unroll
-        for (int k = 0; k < 10; ++k) P.outf[5 + PPB_PERM[DIR][k]][id] = m[k];
+        for (int k = 0; k < 10; ++k) p[64 * (5 + PPB_PERM[DIR][k])] = m[k];
     }
     __device__ __forceinline__ void end(int) {}
     __device__ __forceinline__ void finish() {}
 };
 
+// thread -> pencil: 16 lanes = the 4x4 transverse cells of one brick column; a CTA of 128 threads = 8 brick
+// columns adjacent along a.  (a, b) = the two transverse axes in increasing axis order.
 template <int DIR, int GRAV>
-__global__ void __launch_bounds__(128, 3) ppm_sweep_kernel(const SweepParams P) {
-    int a, b;
-    if (P.brick) {      // 16 lanes = the 4x4 transverse cells of one brick; 8 bricks along a per CTA
-        const int t = threadIdx.x;
-        a = blockIdx.x * 32 + (t >> 4) * 4 + (t & 3);
-        b = blockIdx.y * 4 + ((t >> 2) & 3);
-    } else {
-        a = blockIdx.x * blockDim.x + threadIdx.x;
-        b = blockIdx.y;
-    }
+__global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
+    constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
+    const int t = threadIdx.x;
+    const int ba = blockIdx.x * (PPM_CTA / 16) + (t >> 4), bb = blockIdx.y;
+    const int a = ba * 4 + (t & 3), b = bb * 4 + ((t >> 2) & 3);
     if (a >= P.na || b >= P.nb) return;
     const unsigned wmask = __activemask();
     const int c0 = blockIdx.z * P.chunk;
     const int c1 = min(c0 + P.chunk, P.n);
-    const unsigned tb = (unsigned)(a >> 2) * (unsigned)P.SBa + (unsigned)(a & 3) * (unsigned)P.SIa + (unsigned)(b >> 2) * (unsigned)P.SBb + (unsigned)(b & 3) * (unsigned)P.SIb;
+    const long long tb = (long long)ba * P.SBa + (long long)bb * P.SBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)));
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     march<DIR, GRAV>(P, io, a, b, c0, c1, true, wmask);
 }
 
 // =====================================================================================================
-// IoTmaX: x sweep on the brick layout.  Warp = 2 bricks adjacent in y (lane = bsel*16 + iz*4 + iy).  The TMA
-// box {64 floats of a brick, 1 bx, 2 by, 1 bz, 5 fields} lands as [field][lane][4 x-cells], so every lane owns
-// the 16 bytes at slot `lane` of every field: thread-private, conflict-free, whole 256-byte bricks on the wire.
+// IoTmaX: x sweep (nx a multiple of 4).  Warp = 2 brick columns adjacent in y (lane = bsel*16 + iz*4 + iy).  A TMA
+// box {64 floats, 5 fields, 1 bx, 2 by, 1 bz} lands as [bsel][field][iz][iy][4 x-cells]: every lane owns the 16
+// bytes at (bsel, iz, iy) of every field — thread-private, and whole 1280-byte runs of a brick record on the wire.
 // Rings: hydro fields 2 chunks (2 x 2560 B), PPB fields 2 chunks (2 x 5120 B, read three cells later),
 // results 1 chunk (7680 B) written back by TMA store.  23040 B per warp.
 // =====================================================================================================
@@ -647,16 +669,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-// coordinates: (element in brick = 0, bx, by, bz, field)
+// coordinates: (element in brick = 0, field, bx, by, bz)
 __device__ __forceinline__ void tma_load_brick(void* dst, const CUtensorMap* map, uint64_t* bar, int bx, int by, int bz, int f) {
     asm volatile(
         "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(0), "r"(bx), "r"(by), "r"(bz), "r"(f) : "memory");
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(0), "r"(f), "r"(bx), "r"(by), "r"(bz) : "memory");
 }
 __device__ __forceinline__ void tma_store_brick(const CUtensorMap* map, const void* src, int bx, int by, int bz, int f) {
     asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
-                 ::"l"(map), "r"(smem_u32(src)), "r"(0), "r"(bx), "r"(by), "r"(bz), "r"(f) : "memory");
+                 ::"l"(map), "r"(smem_u32(src)), "r"(0), "r"(f), "r"(bx), "r"(by), "r"(bz) : "memory");
 }
+// float index of field F (0..14) inside a staged group of boxes, each box = [2 bsel][5 fields][64]
+__device__ __forceinline__ constexpr int tx_slot(int F) { return (F / 5) * (2 * 5 * 64) + (F % 5) * 64; }
 __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
@@ -670,14 +694,14 @@ struct IoTmaX {
     float* ppbuf;        // warp's PPB ring   [2][10][32][4]
     float* outb;         // warp's result chunk [15][32][4]
     uint64_t* bar;       // [0..1] hydro ring, [2..3] PPB ring
-    const int lane, by0, bz;
+    const int lane, lbase, by0, bz;   // lbase: the lane's 16-byte slot inside a box = bsel*320 + (iz*4+iy)*4
     const int k0, kend;  // first / last chunk index (chunk k = brick bx = k = cells 4k .. 4k+3)
     bool store_pending;
 
     __device__ __forceinline__ IoTmaX(const SweepParams& P_, const CUtensorMap* ti, const CUtensorMap* to, float* wsm, uint64_t* wbar,
                                       int lane_, int by0_, int bz_, int c0, int c1)
         : P(P_), tin(ti), tout(to), hyd(wsm), ppbuf(wsm + 2 * TX_HYD), outb(wsm + 2 * TX_HYD + 2 * TX_PPB), bar(wbar),
-          lane(lane_), by0(by0_), bz(bz_), k0(c0 / TX_CH - 1), kend(c1 / TX_CH), store_pending(false) {
+          lane(lane_), lbase((lane_ >> 4) * 320 + (lane_ & 15) * 4), by0(by0_), bz(bz_), k0(c0 / TX_CH - 1), kend(c1 / TX_CH), store_pending(false) {
         if (lane == 0) {
             issue_hydro(k0); issue_ppb(k0);
             if (k0 + 1 <= kend) { issue_hydro(k0 + 1); issue_ppb(k0 + 1); }
@@ -722,12 +746,12 @@ struct IoTmaX {
         if (rev) s = 3 - s;
         sgn = rev ? -1.0f : 1.0f;
         j = bx * TX_CH + s;
-        const float* src = hyd + ((k - k0) & 1) * TX_HYD + lane * TX_CH + s;
+        const float* src = hyd + ((k - k0) & 1) * TX_HYD + lbase + s;
         v[0] = src[0];
-        v[1] = sgn * src[1 * TX_ROWS * TX_CH];                 // normal velocity ux is field 1 (odd under mirror)
-        v[2] = src[2 * TX_ROWS * TX_CH];
-        v[3] = src[3 * TX_ROWS * TX_CH];
-        v[4] = src[4 * TX_ROWS * TX_CH];
+        v[1] = sgn * src[1 * 64];                              // normal velocity ux is field 1 (odd under mirror)
+        v[2] = src[2 * 64];
+        v[3] = src[3 * 64];
+        v[4] = src[4 * 64];
     }
     __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
         const int k = c >> 2;
@@ -735,9 +759,9 @@ struct IoTmaX {
         int s = c & 3;
         if (rev) s = 3 - s;
         const float sgn = rev ? -1.0f : 1.0f;
-        const float* src = ppbuf + ((k - k0) & 1) * TX_PPB + lane * TX_CH + s;
+        const float* src = ppbuf + ((k - k0) & 1) * TX_PPB + lbase + s;
 #pragma unroll
-        for (int q = 0; q < 10; ++q) m[q] = src[PPB_PERM[0][q] * TX_ROWS * TX_CH];
+        for (int q = 0; q < 10; ++q) m[q] = src[tx_slot(PPB_PERM[0][q])];
         m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
     }
     __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
@@ -748,11 +772,11 @@ struct IoTmaX {
             __syncwarp();
             store_pending = false;
         }
-        float* dst = outb + lane * TX_CH + s;
+        float* dst = outb + lbase + s;
 #pragma unroll
-        for (int f = 0; f < 5; ++f) dst[f * TX_ROWS * TX_CH] = h[f];
+        for (int f = 0; f < 5; ++f) dst[f * 64] = h[f];
 #pragma unroll
-        for (int q = 0; q < 10; ++q) dst[(5 + PPB_PERM[0][q]) * TX_ROWS * TX_CH] = m[q];
+        for (int q = 0; q < 10; ++q) dst[tx_slot(5 + PPB_PERM[0][q])] = m[q];
         if (s == 3) {
             fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
             __syncwarp();
@@ -805,7 +829,7 @@ __global__ void __launch_bounds__(TX_WARPS * 32, 2) ppm_sweep_x_tma_kernel(const
     const int c0 = blockIdx.z * P.chunk;
     const int c1 = min(c0 + P.chunk, P.n);
     IoTmaX io(P, &tin, &tout, sm + warp * TX_WARP_FLOATS, bars + warp * 4, lane, by0, bz, c0, c1);
-    march<0, GRAV>(P, io, a, b, c0, c1, a < P.na, 0xffffffffu);
+    march<0, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);   // pad pencils of a ragged grid compute garbage that is never read
 }
 
 template <int DIR>
@@ -842,7 +866,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 bool ppm_make_xmaps(ppm_ctx* c) {
     c->tma_ok = 0;
     const ppm_params& p = c->prm;
-    if (c->layout != 1) return false;                           // the TMA path stages bricks
+    if (p.nx % 4 != 0) return false;                            // ghost chunks must be whole bricks (mirror / wrap by brick)
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
@@ -851,10 +875,11 @@ bool ppm_make_xmaps(ppm_ctx* c) {
         return false;
     }
     EncodeTiledFn enc = (EncodeTiledFn)fn;
-    const cuuint64_t nbx = p.nx / 4, nby = p.ny / 4, nbz = p.nz / 4;
-    const cuuint64_t dims[5] = {64, nbx, nby, nbz, PPM_NFIELDS};
-    const cuuint64_t strides[4] = {256, 256 * nbx, 256 * nbx * nby, 256 * nbx * nby * nbz};
-    const cuuint32_t box[5] = {64, 1, 2, 1, 5};
+    const cuuint64_t nbx = c->nbx, nby = c->nby, nbz = c->nbz;
+    const cuuint64_t rec = PPM_BRICK_FLOATS * sizeof(float);
+    const cuuint64_t dims[5] = {64, PPM_NFIELDS, nbx, nby, nbz};
+    const cuuint64_t strides[4] = {256, rec, rec * nbx, rec * nbx * nby};
+    const cuuint32_t box[5] = {64, 5, 1, 2, 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     for (int b = 0; b < 2; ++b) {
         CUresult r = enc(reinterpret_cast<CUtensorMap*>(c->xmap[b]), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, c->buf[b], dims, strides, box, estr,
@@ -868,29 +893,16 @@ bool ppm_make_xmaps(ppm_ctx* c) {
 
 cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     const ppm_params& p = c->prm;
-    const long long nx = p.nx, ny = p.ny, nz = p.nz;
     SweepParams P;
-    const float* in = c->buf[c->cur];
-    float* out = c->buf[c->cur ^ 1];
-    P.ncell = nx * ny * nz;
-    for (int f = 0; f < PPM_NFIELDS; ++f) { P.inf[f] = in + f * P.ncell; P.outf[f] = out + f * P.ncell; }
+    P.in = c->buf[c->cur];
+    P.out = c->buf[c->cur ^ 1];
     const int ext[3] = {p.nx, p.ny, p.nz};
-    const int ia = (axis == 0) ? 1 : 0;       // thread-mapped transverse axis
+    const int ia = (axis == 0) ? 1 : 0;       // first transverse axis
     const int ib = (axis == 2) ? 1 : 2;       // second transverse axis
     P.n = ext[axis]; P.na = ext[ia]; P.nb = ext[ib];
-    long long SB[3]; int SI[3];
-    if (c->layout == 1) {
-        const long long nbx = nx / 4, nby = ny / 4;
-        SB[0] = 64; SB[1] = 64 * nbx; SB[2] = 64 * nbx * nby;
-        SI[0] = 1; SI[1] = 4; SI[2] = 16;
-    } else {
-        const long long str[3] = {1, nx, nx * ny};
-        for (int d = 0; d < 3; ++d) { SB[d] = 4 * str[d]; SI[d] = (int)str[d]; }
-    }
+    const long long SB[3] = {PPM_BRICK_FLOATS, (long long)PPM_BRICK_FLOATS * c->nbx, (long long)PPM_BRICK_FLOATS * c->nbx * c->nby};
     P.SBd = SB[axis]; P.SBa = SB[ia]; P.SBb = SB[ib];
-    P.SId = SI[axis]; P.SIa = SI[ia]; P.SIb = SI[ib];
-    P.brick = c->layout;
-    P.nbrick_d = P.n / 4;
+    P.nbrick_d = (P.n + 3) / 4;
     P.bc_lo = p.bc[2 * axis]; P.bc_hi = p.bc[2 * axis + 1];
     const bool use_tma = (axis == 0) && c->tma_ok && !c->force_direct;
     int chunk = c->chunk > 0 ? c->chunk : P.n;
@@ -904,17 +916,18 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     P.tab = c->tab;
     P.flag = c->flag;
     const int nchunks = (P.n + chunk - 1) / chunk;
+    const int nba = (P.na + 3) / 4, nbb = (P.nb + 3) / 4;
     cudaError_t e;
     if (use_tma) {
         const CUtensorMap& tin = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur]);
         const CUtensorMap& tout = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur ^ 1]);
-        dim3 grid((P.na + TX_WARPS * 8 - 1) / (TX_WARPS * 8), P.nb / 4, nchunks);   // CTA = 8 bricks along y, 1 along z
+        dim3 grid((nba + TX_WARPS * 2 - 1) / (TX_WARPS * 2), nbb, nchunks);   // CTA = 8 brick columns along y, 1 along z
         if (p.grav.kind == PPM_GRAV_NONE) e = launch_x_tma<PPM_GRAV_NONE>(P, tin, tout, grid, c->stream);
         else if (p.grav.kind == PPM_GRAV_CONST_Z) e = launch_x_tma<PPM_GRAV_CONST_Z>(P, tin, tout, grid, c->stream);
         else e = launch_x_tma<PPM_GRAV_RADIAL>(P, tin, tout, grid, c->stream);
     } else {
-        dim3 block(128, 1, 1);
-        dim3 grid = c->layout == 1 ? dim3((P.na + 31) / 32, (P.nb + 3) / 4, nchunks) : dim3((P.na + 127) / 128, P.nb, nchunks);
+        dim3 block(PPM_CTA, 1, 1);
+        dim3 grid((nba + PPM_CTA / 16 - 1) / (PPM_CTA / 16), nbb, nchunks);
         if (axis == 0) e = launch_dir<0>(P, p.grav.kind, grid, block, c->stream);
         else if (axis == 1) e = launch_dir<1>(P, p.grav.kind, grid, block, c->stream);
         else e = launch_dir<2>(P, p.grav.kind, grid, block, c->stream);

@@ -60,12 +60,21 @@ def test_create_rejects_bad_arguments_before_touching_cuda(lib):
     assert _create(lib, bc=(0, 0, 0, 0, 7, 7))[0] == E
     assert _create(lib, nz=3, bc=(0, 0, 0, 0, 1, 1))[0] == E       # reflecting axis needs >= 4 cells
     assert _create(lib, struct_size=8)[0] == E
-    assert _create(lib, a=0)[0] == E and _create(lib, a=0x1004)[0] == E and _create(lib, a=0x2000)[0] == E
+    assert _create(lib, a=0)[0] == E and _create(lib, a=0x1040)[0] == E and _create(lib, a=0x2000)[0] == E   # NULL, not 128-byte aligned, aliased
     tab = np.ones(5, dtype=np.float32)
     bad = dict(kind=1, s0=0.0, ds=0.1, g=tab, rho0=tab, p0=tab)    # CONST_Z table must sit on centres and faces
     rc, _, msg = _create(lib, grav=bad)
     assert rc == E and "CONST_Z" in msg
     assert _create(lib, grav=dict(kind=9, s0=0.0, ds=0.1, g=tab, rho0=tab, p0=tab))[0] == E
+
+
+def test_state_floats_is_whole_brick_records(lib):
+    L = lib.lib()
+    assert L.ppm_state_floats(8, 8, 8) == 15 * 512
+    assert L.ppm_state_floats(512, 512, 512) == 15 * 512 ** 3
+    assert L.ppm_state_floats(37, 29, 23) == 15 * 64 * 10 * 8 * 6      # extents rounded up to 4-cell bricks
+    assert L.ppm_state_floats(1, 1, 1) == 15 * 64
+    assert L.ppm_state_floats(0, 8, 8) == 0 and L.ppm_state_floats(8, -1, 8) == 0
 
 
 def test_null_context_calls_return_einval(lib):
