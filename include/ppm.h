@@ -114,7 +114,7 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
 /* Options (results do not depend on them).
  *  PPM_OPT_X_PATH : 0 = automatic (nx a multiple of 4: the x sweep stages whole bricks through shared
  *                   memory with TMA), 1 = force the direct global-memory path. */
-enum { PPM_OPT_X_PATH = 1 };
+enum { PPM_OPT_X_PATH = 1, PPM_OPT_IO_PATH = 2 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* 1 if the next x sweep will take the TMA-staged path, 0 if the direct path. */
 int ppm_x_path(const ppm_ctx *ctx);

@@ -212,6 +212,7 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
     if (option == PPM_OPT_X_PATH && (value == 0 || value == 1)) { c->force_direct = value; return PPM_OK; }
+    if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1 || value == 3)) { c->io_path = value; return PPM_OK; }
     set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
     return PPM_EINVAL;
 }

@@ -53,6 +53,7 @@ struct ppm_ctx {
     int chunk;
     int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
     int tma_ok;                     // tensor maps for the x-sweep TMA path are valid
+    int io_path;                    // PPM_OPT_IO_PATH: 0 auto, 1 direct (+ TMA x), 3 bulk-staged wherever possible
     int force_direct;               // option: take the direct-global x path even when TMA is available
     long long launches;
     char err[512];

@@ -52,6 +52,11 @@
 #ifndef PPM_MAXREG
 #define PPM_MAXREG 168
 #endif
+// direct path: whole brick records this many bricks ahead along the pencil are pulled into L2 with one bulk
+// prefetch per half warp (0 = off)
+#ifndef PPM_PREFETCH_BRICKS
+#define PPM_PREFETCH_BRICKS 1
+#endif
 
 namespace {
 
@@ -569,6 +574,12 @@ struct IoDirect {
     __device__ __forceinline__ void fetch(int n) {
         jn = image_cell(n, P.n, P.bc_lo, P.bc_hi, sn);
         const float* __restrict__ p = pin + off(jn);
+        if (PPM_PREFETCH_BRICKS > 0 && (n & 3) == 0 && (unsigned)(n + 4 * PPM_PREFETCH_BRICKS) < (unsigned)P.n) {
+            // first plane of a brick: ask L2 for the record PPM_PREFETCH_BRICKS further along (3840 contiguous bytes,
+            // one request per brick column = per half warp); also walks the TLB ahead of the loads
+            if ((threadIdx.x & 15) == 0)
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pin + off(n + 4 * PPM_PREFETCH_BRICKS)), "n"(PPM_BRICK_FLOATS * 4) : "memory");
+        }
         nx5[0] = __ldg(p);
         nx5[1] = __ldg(p + 64 * Dir<DIR>::U);
         nx5[2] = __ldg(p + 64 * Dir<DIR>::V);
@@ -832,6 +843,227 @@ __global__ void __launch_bounds__(TX_WARPS * 32, 2) ppm_sweep_x_tma_kernel(const
     march<0, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);   // pad pencils of a ragged grid compute garbage that is never read
 }
 
+// =====================================================================================================
+// IoBulk: every sweep direction (sweep-axis extent a multiple of 4).  Warp = 2 brick columns adjacent along a.
+// A brick record keeps its 15 fields contiguous, so the hydro part (5 fields, 1280 B) and the PPB part (10
+// fields, 2560 B) of a brick are plain 1-D bulk copies (cp.async.bulk, no tensor map): global -> shared when the
+// brick comes up, shared -> global when its four cells are finished.  Nothing else touches global memory, so
+// DRAM sees whole 1280/2560-byte runs in all three directions, no load sits in a register waiting, and the
+// marching body needs no prefetch registers.
+//
+// Results are written IN PLACE over the brick's own input in shared memory: cell i's hydro input is read at
+// iteration n = i and its PPB input at n = i + 3, its results are written at n = i + 4.  So a hydro slot lives
+// for 3 bricks of marching (input, output, in flight to global) and a PPB slot for 2: rings of 3 and 2 slots,
+// 17.8 KB per warp, 12 warps per SM.
+// =====================================================================================================
+template <int DIR> struct BulkGeom {
+    static constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
+    // the second brick of a slot is shifted so that the two half warps fall on different banks where the
+    // direction allows it (z: 16 lanes contiguous; y: 4-float runs 16 apart; x: every 4th bank, 4-way inherent)
+    static constexpr int PAD = (DIR == 2) ? 16 : ((DIR == 1) ? 8 : 4);
+    static constexpr int HB = 5 * 64, PB = 10 * 64;             // floats per brick: hydro part, PPB part
+    static constexpr int HSLOT = 2 * HB + PAD, PSLOT = 2 * PB + PAD;
+    static constexpr int NH = 3, NP = 2;                        // ring depths
+    static constexpr int WARP_FLOATS = NH * HSLOT + NP * PSLOT;
+    static constexpr int WARPS = 4;
+    static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * 4 + WARPS * (NH + NP) * sizeof(uint64_t);
+};
+
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
+}
+
+template <int DIR>
+struct IoBulk {
+    using G = BulkGeom<DIR>;
+    const SweepParams& P;
+    float* const hyd;            // warp's hydro ring [NH][HSLOT]
+    float* const ppr;            // warp's PPB ring   [NP][PSLOT]
+    uint64_t* const bar;         // [0..NH) hydro slots, [NH..NH+NP) PPB slots
+    const int lane;
+    const int loff;              // the lane's float offset inside a slot, sweep-axis layer 0, field 0
+    const long long gcol;        // float offset of the warp's first brick column (brick 0 along the sweep axis)
+    const int ncol;              // brick columns of this warp that exist (1 or 2)
+    const int k0, kend;          // first / last brick index along the sweep axis this pencil segment touches (ghosts included)
+
+    __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, int lane_, long long gcol_, int ncol_, int c0, int c1)
+        : P(P_), hyd(wsm), ppr(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_),
+          loff(((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
+          gcol(gcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4) {
+        if (lane == 0) {
+#pragma unroll
+            for (int j = 0; j < G::NH; ++j) if (k0 + j <= kend) issue_hydro(k0 + j);
+#pragma unroll
+            for (int j = 0; j < G::NP; ++j) if (k0 + j <= kend) issue_ppb(k0 + j);
+        }
+    }
+    // brick holding chunk k (ghost chunks map onto their periodic / mirror image; mirrored ones are read reversed)
+    __device__ __forceinline__ int chunk_brick(int k, bool& rev) const {
+        rev = false;
+        const int nk = P.nbrick_d;
+        if (k < 0) { if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = true; return 0; }
+        if (k >= nk) { if (P.bc_hi == PPM_BC_PERIODIC) return 0; rev = true; return nk - 1; }
+        return k;
+    }
+    __device__ __forceinline__ int hslot(int k) const { return (k - k0) % G::NH; }
+    __device__ __forceinline__ int pslot(int k) const { return (k - k0) % G::NP; }
+    __device__ __forceinline__ int hoff(int k) const { return hslot(k) * G::HSLOT; }
+    __device__ __forceinline__ int poff(int k) const { return pslot(k) * G::PSLOT; }
+    // second brick column of the warp: lanes 16..31
+    __device__ __forceinline__ int hlane() const { return (lane >> 4) * (G::HB + G::PAD) + loff; }
+    __device__ __forceinline__ int plane_() const { return (lane >> 4) * (G::PB + G::PAD) + loff; }
+
+    __device__ __forceinline__ void issue_hydro(int k) {       // lane 0 only
+        bool rev; const int bd = chunk_brick(k, rev);
+        const int s = hslot(k);
+        const float* src = P.in + gcol + (long long)bd * P.SBd;
+        mbar_expect_tx(bar + s, ncol * G::HB * 4);
+        bulk_g2s(hyd + s * G::HSLOT, src, G::HB * 4, bar + s);
+        if (ncol > 1) bulk_g2s(hyd + s * G::HSLOT + G::HB + G::PAD, src + P.SBa, G::HB * 4, bar + s);
+    }
+    __device__ __forceinline__ void issue_ppb(int k) {         // lane 0 only
+        bool rev; const int bd = chunk_brick(k, rev);
+        const int s = pslot(k);
+        const float* src = P.in + gcol + (long long)bd * P.SBd + G::HB;
+        mbar_expect_tx(bar + G::NH + s, ncol * G::PB * 4);
+        bulk_g2s(ppr + s * G::PSLOT, src, G::PB * 4, bar + G::NH + s);
+        if (ncol > 1) bulk_g2s(ppr + s * G::PSLOT + G::PB + G::PAD, src + P.SBa, G::PB * 4, bar + G::NH + s);
+    }
+    __device__ __forceinline__ void begin(int n) {
+        if ((n & 3) == 0) {                                    // first cell of hydro chunk k
+            const int k = n >> 2;
+            mbar_wait(bar + hslot(k), ((k - k0) / G::NH) & 1);
+        }
+        const int c = n - 3;                                   // PPB cell of this iteration
+        if ((c & 3) == 0 || c == 4 * k0 + 3) {                 // first PPB cell read from its chunk
+            const int k = c >> 2;
+            if (k >= k0) mbar_wait(bar + G::NH + pslot(k), ((k - k0) / G::NP) & 1);
+        }
+    }
+    __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
+        const int k = n >> 2;
+        bool rev; const int bd = chunk_brick(k, rev);
+        int s = n & 3;
+        if (rev) s = 3 - s;
+        sgn = rev ? -1.0f : 1.0f;
+        j = bd * 4 + s;
+        const float* src = hyd + hoff(k) + hlane() + (s << (2 * DIR));
+        v[0] = src[0];
+        v[1] = sgn * src[64 * Dir<DIR>::U];                    // normal velocity: odd under the mirror
+        v[2] = src[64 * Dir<DIR>::V];
+        v[3] = src[64 * Dir<DIR>::W];
+        v[4] = src[64 * 4];
+    }
+    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
+        const int k = c >> 2;
+        bool rev; chunk_brick(k, rev);
+        int s = c & 3;
+        if (rev) s = 3 - s;
+        const float sgn = rev ? -1.0f : 1.0f;
+        const float* src = ppr + poff(k) + plane_() + (s << (2 * DIR));
+#pragma unroll
+        for (int q = 0; q < 10; ++q) m[q] = src[64 * PPB_PERM[DIR][q]];
+        m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
+    }
+    __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
+    // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
+    __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
+        const int k = i >> 2, s = i & 3;
+        float* dh = hyd + hoff(k) + hlane() + (s << (2 * DIR));
+        dh[0] = h[0];
+        dh[64 * Dir<DIR>::U] = h[1];
+        dh[64 * Dir<DIR>::V] = h[2];
+        dh[64 * Dir<DIR>::W] = h[3];
+        dh[64 * 4] = h[4];
+        float* dp = ppr + poff(k) + plane_() + (s << (2 * DIR));
+#pragma unroll
+        for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
+        if (s == 3) {                                          // brick k is complete: ship it
+            fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
+            __syncwarp();
+            if (lane == 0) {
+                float* dst = P.out + gcol + (long long)k * P.SBd;
+                const float* sh = hyd + hoff(k);
+                const float* sp = ppr + poff(k);
+                bulk_s2g(dst, sh, G::HB * 4);
+                bulk_s2g(dst + G::HB, sp, G::PB * 4);
+                if (ncol > 1) {
+                    bulk_s2g(dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
+                    bulk_s2g(dst + P.SBa + G::HB, sp + G::PB + G::PAD, G::PB * 4);
+                }
+                tma_commit();
+            }
+        }
+    }
+    __device__ __forceinline__ void end(int n) {
+        // ring refill, once per brick: by the end of iteration n = 4m the slots of brick m - 2 are dead (its last
+        // cell was stored at n = 4m - 1; for a ghost brick the last read was earlier still)
+        if ((n & 3) == 0) {
+            const int m = n >> 2;
+            __syncwarp();
+            if (lane == 0) {
+                tma_wait_read0();                              // the bulk stores issued one iteration ago have read their slots
+                if (m + 1 >= k0 + G::NH && m + 1 <= kend) issue_hydro(m + 1);
+                if (m >= k0 + G::NP && m <= kend) issue_ppb(m);
+            }
+        }
+    }
+    __device__ __forceinline__ void finish() {
+        if (lane == 0) tma_wait_all0();                        // smem must outlive the last bulk store
+        __syncwarp();
+    }
+};
+
+template <int DIR, int GRAV>
+__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
+    using G = BulkGeom<DIR>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* sm = reinterpret_cast<float*>(smem_raw);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x < G::WARPS * (G::NH + G::NP)) mbar_init(bars + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_async_smem();
+    __syncthreads();
+    const int nba = (P.na + 3) >> 2;
+    const int ba0 = (blockIdx.x * G::WARPS + warp) * 2;        // the warp's brick columns: ba0, ba0 + 1 along a; bb along b
+    if (ba0 >= nba) return;                                    // whole warp out of range (no block-wide sync below)
+    const int bb = blockIdx.y;
+    const int a = (ba0 + (lane >> 4)) * 4 + (lane & 3);
+    const int b = bb * 4 + ((lane >> 2) & 3);
+    const int c0 = blockIdx.z * P.chunk;
+    const int c1 = min(c0 + P.chunk, P.n);
+    const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
+    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), lane, gcol, min(2, nba - ba0), c0, c1);
+    // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
+    march<DIR, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);
+}
+
+template <int DIR, int GRAV>
+cudaError_t launch_bulk(const SweepParams& P, dim3 grid, cudaStream_t st) {
+    using G = BulkGeom<DIR>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(ppm_sweep_bulk_kernel<DIR, GRAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    ppm_sweep_bulk_kernel<DIR, GRAV><<<grid, G::WARPS * 32, G::SMEM, st>>>(P);
+    return cudaGetLastError();
+}
+template <int DIR>
+cudaError_t launch_bulk_dir(const SweepParams& P, int grav, dim3 grid, cudaStream_t st) {
+    switch (grav) {
+        case PPM_GRAV_NONE: return launch_bulk<DIR, PPM_GRAV_NONE>(P, grid, st);
+        case PPM_GRAV_CONST_Z: return launch_bulk<DIR, PPM_GRAV_CONST_Z>(P, grid, st);
+        default: return launch_bulk<DIR, PPM_GRAV_RADIAL>(P, grid, st);
+    }
+}
+
 template <int DIR>
 cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cudaStream_t st) {
     switch (grav) {
@@ -904,9 +1136,11 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     P.SBd = SB[axis]; P.SBa = SB[ia]; P.SBb = SB[ib];
     P.nbrick_d = (P.n + 3) / 4;
     P.bc_lo = p.bc[2 * axis]; P.bc_hi = p.bc[2 * axis + 1];
-    const bool use_tma = (axis == 0) && c->tma_ok && !c->force_direct;
+    // data path: bulk-staged (any axis whose extent is a multiple of 4), else TMA-staged x, else direct
+    const bool use_bulk = ((c->io_path == 0 && axis == 0) || c->io_path == 3) && (P.n % 4 == 0) && !(axis == 0 && c->force_direct);
+    const bool use_tma = !use_bulk && (axis == 0) && c->tma_ok && !c->force_direct && c->io_path != 1;
     int chunk = c->chunk > 0 ? c->chunk : P.n;
-    if (use_tma) chunk = (chunk + 3) / 4 * 4;
+    if (use_tma || use_bulk) chunk = (chunk + 3) / 4 * 4;
     if (chunk > P.n) chunk = P.n;
     P.chunk = chunk;
     P.dt = (float)dt; P.dx = (float)p.dx; P.dtdx = (float)(dt / p.dx); P.inv_dx = (float)(1.0 / p.dx);
@@ -918,7 +1152,12 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     const int nchunks = (P.n + chunk - 1) / chunk;
     const int nba = (P.na + 3) / 4, nbb = (P.nb + 3) / 4;
     cudaError_t e;
-    if (use_tma) {
+    if (use_bulk) {
+        dim3 grid((nba + 7) / 8, nbb, nchunks);                               // CTA = 4 warps x 2 brick columns along a
+        if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, grid, c->stream);
+        else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, grid, c->stream);
+        else e = launch_bulk_dir<2>(P, p.grav.kind, grid, c->stream);
+    } else if (use_tma) {
         const CUtensorMap& tin = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur]);
         const CUtensorMap& tout = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur ^ 1]);
         dim3 grid((nba + TX_WARPS * 2 - 1) / (TX_WARPS * 2), nbb, nchunks);   // CTA = 8 brick columns along y, 1 along z
