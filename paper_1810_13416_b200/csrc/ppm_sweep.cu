@@ -670,15 +670,15 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+    // Called by whole warps.  The loop exit is a warp vote, i.e. provably uniform: a per-lane spin loop (in C++ or
+    // hidden inside the asm) makes ptxas treat everything after it as divergent and give up the uniform datapath
+    // for the marching loop's index arithmetic.
+    const uint32_t addr = smem_u32(bar);
+    uint32_t done;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    } while (!__all_sync(0xffffffffu, done));   // warp-uniform exit: every lane polls, the vote decides
 }
 // coordinates: (element in brick = 0, field, bx, by, bz)
 __device__ __forceinline__ void tma_load_brick(void* dst, const CUtensorMap* map, uint64_t* bar, int bx, int by, int bz, int f) {
@@ -880,78 +880,93 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
 template <int DIR>
 struct IoBulk {
     using G = BulkGeom<DIR>;
+    static constexpr int SH = 2 * DIR;   // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
-    float* const hyd;            // warp's hydro ring [NH][HSLOT]
-    float* const ppr;            // warp's PPB ring   [NP][PSLOT]
+    float* const hyd;            // warp's hydro ring [NH][HSLOT], already offset to the lane's layer-0 element
+    float* const ppr;            // warp's PPB ring   [NP][PSLOT], same
+    float* const hyd0;           // ring bases as the bulk copies see them (lane 0 uses them)
+    float* const ppr0;
     uint64_t* const bar;         // [0..NH) hydro slots, [NH..NH+NP) PPB slots
     const int lane;
-    const int loff;              // the lane's float offset inside a slot, sweep-axis layer 0, field 0
     const long long gcol;        // float offset of the warp's first brick column (brick 0 along the sweep axis)
     const int ncol;              // brick columns of this warp that exist (1 or 2)
     const int k0, kend;          // first / last brick index along the sweep axis this pencil segment touches (ghosts included)
+    // per-brick state, refreshed when a new brick comes up (once per 4 iterations); everything is warp-uniform
+    int hs, ps;                  // ring slot of the hydro brick being read / of the PPB brick being read
+    int par;                     // bit 0: mbarrier phase of hydro slot hs; bit 1: of PPB slot ps
+    int hcur, hprv;              // float offset (from hyd) of the hydro slot being read / of the one receiving results
+    int pcur, pst;               // float offset (from ppr) of the PPB slot being read / of the one receiving results
+    int hrev, prev;              // 3 if the brick being read is a mirror image (cells taken in reverse, odd fields negated), else 0
+    int jb;                      // image index of the hydro brick's cell 0
 
     __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, int lane_, long long gcol_, int ncol_, int c0, int c1)
-        : P(P_), hyd(wsm), ppr(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_),
-          loff(((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
-          gcol(gcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4) {
+        : P(P_),
+          hyd(wsm + (lane_ >> 4) * (G::HB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
+          ppr(wsm + G::NH * G::HSLOT + (lane_ >> 4) * (G::PB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
+          hyd0(wsm), ppr0(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_), gcol(gcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4),
+          hs(0), ps(0), par(0), hcur(0), hprv(0), pcur(0), pst(0), hrev(0), prev(0), jb(0) {
         if (lane == 0) {
 #pragma unroll
-            for (int j = 0; j < G::NH; ++j) if (k0 + j <= kend) issue_hydro(k0 + j);
+            for (int j = 0; j < G::NH; ++j) if (k0 + j <= kend) issue_hydro(k0 + j, j);
 #pragma unroll
-            for (int j = 0; j < G::NP; ++j) if (k0 + j <= kend) issue_ppb(k0 + j);
+            for (int j = 0; j < G::NP; ++j) if (k0 + j <= kend) issue_ppb(k0 + j, j);
         }
     }
     // brick holding chunk k (ghost chunks map onto their periodic / mirror image; mirrored ones are read reversed)
-    __device__ __forceinline__ int chunk_brick(int k, bool& rev) const {
-        rev = false;
+    __device__ __forceinline__ int chunk_brick(int k, int& rev) const {
+        rev = 0;
         const int nk = P.nbrick_d;
-        if (k < 0) { if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = true; return 0; }
-        if (k >= nk) { if (P.bc_hi == PPM_BC_PERIODIC) return 0; rev = true; return nk - 1; }
-        return k;
+        if ((unsigned)k < (unsigned)nk) return k;
+        if (k < 0) { if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = 3; return 0; }
+        if (P.bc_hi == PPM_BC_PERIODIC) return 0;
+        rev = 3; return nk - 1;
     }
-    __device__ __forceinline__ int hslot(int k) const { return (k - k0) % G::NH; }
-    __device__ __forceinline__ int pslot(int k) const { return (k - k0) % G::NP; }
-    __device__ __forceinline__ int hoff(int k) const { return hslot(k) * G::HSLOT; }
-    __device__ __forceinline__ int poff(int k) const { return pslot(k) * G::PSLOT; }
-    // second brick column of the warp: lanes 16..31
-    __device__ __forceinline__ int hlane() const { return (lane >> 4) * (G::HB + G::PAD) + loff; }
-    __device__ __forceinline__ int plane_() const { return (lane >> 4) * (G::PB + G::PAD) + loff; }
-
-    __device__ __forceinline__ void issue_hydro(int k) {       // lane 0 only
-        bool rev; const int bd = chunk_brick(k, rev);
-        const int s = hslot(k);
+    __device__ __forceinline__ void issue_hydro(int k, int slot) {       // lane 0 only
+        int rev; const int bd = chunk_brick(k, rev);
         const float* src = P.in + gcol + (long long)bd * P.SBd;
-        mbar_expect_tx(bar + s, ncol * G::HB * 4);
-        bulk_g2s(hyd + s * G::HSLOT, src, G::HB * 4, bar + s);
-        if (ncol > 1) bulk_g2s(hyd + s * G::HSLOT + G::HB + G::PAD, src + P.SBa, G::HB * 4, bar + s);
+        mbar_expect_tx(bar + slot, ncol * G::HB * 4);
+        bulk_g2s(hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
+        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + P.SBa, G::HB * 4, bar + slot);
     }
-    __device__ __forceinline__ void issue_ppb(int k) {         // lane 0 only
-        bool rev; const int bd = chunk_brick(k, rev);
-        const int s = pslot(k);
+    __device__ __forceinline__ void issue_ppb(int k, int slot) {         // lane 0 only
+        int rev; const int bd = chunk_brick(k, rev);
         const float* src = P.in + gcol + (long long)bd * P.SBd + G::HB;
-        mbar_expect_tx(bar + G::NH + s, ncol * G::PB * 4);
-        bulk_g2s(ppr + s * G::PSLOT, src, G::PB * 4, bar + G::NH + s);
-        if (ncol > 1) bulk_g2s(ppr + s * G::PSLOT + G::PB + G::PAD, src + P.SBa, G::PB * 4, bar + G::NH + s);
+        mbar_expect_tx(bar + G::NH + slot, ncol * G::PB * 4);
+        bulk_g2s(ppr0 + slot * G::PSLOT, src, G::PB * 4, bar + G::NH + slot);
+        if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + P.SBa, G::PB * 4, bar + G::NH + slot);
     }
     __device__ __forceinline__ void begin(int n) {
-        if ((n & 3) == 0) {                                    // first cell of hydro chunk k
+        const int s = n & 3;
+        if (s == 0) {                                          // a new hydro brick k comes up; results of brick k - 1 start
             const int k = n >> 2;
-            mbar_wait(bar + hslot(k), ((k - k0) / G::NH) & 1);
-        }
-        const int c = n - 3;                                   // PPB cell of this iteration
-        if ((c & 3) == 0 || c == 4 * k0 + 3) {                 // first PPB cell read from its chunk
-            const int k = c >> 2;
-            if (k >= k0) mbar_wait(bar + G::NH + pslot(k), ((k - k0) / G::NP) & 1);
+            pst = pcur;                                        // PPB brick k - 1 is the one being read since n - 1
+            hprv = hcur;
+            if (k != k0) {
+                hs = (hs == G::NH - 1) ? 0 : hs + 1;
+                if (hs == 0) par ^= 1;
+                hcur = hs * G::HSLOT;
+            }
+            jb = chunk_brick(k, hrev) * 4;
+            mbar_wait(bar + hs, par & 1);
+        } else if (s == 3) {                                   // PPB cell c = n - 3 is the first of brick c >> 2
+            const int c = n - 3, k = c >> 2;
+            if (k > k0) {
+                ps ^= 1;
+                if (ps == 0) par ^= 2;
+                pcur = ps * G::PSLOT;
+                chunk_brick(k, prev);
+                mbar_wait(bar + G::NH + ps, (par >> 1) & 1);
+            }
+        } else if (n == 4 * k0 + 6) {                          // the very first PPB cell (c0 - 1) is the last cell of brick k0
+            chunk_brick(k0, prev);
+            mbar_wait(bar + G::NH, 0);
         }
     }
     __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
-        const int k = n >> 2;
-        bool rev; const int bd = chunk_brick(k, rev);
-        int s = n & 3;
-        if (rev) s = 3 - s;
-        sgn = rev ? -1.0f : 1.0f;
-        j = bd * 4 + s;
-        const float* src = hyd + hoff(k) + hlane() + (s << (2 * DIR));
+        const int s = (n & 3) ^ hrev;
+        sgn = hrev ? -1.0f : 1.0f;
+        j = jb + s;
+        const float* src = hyd + hcur + (s << SH);
         v[0] = src[0];
         v[1] = sgn * src[64 * Dir<DIR>::U];                    // normal velocity: odd under the mirror
         v[2] = src[64 * Dir<DIR>::V];
@@ -959,12 +974,9 @@ struct IoBulk {
         v[4] = src[64 * 4];
     }
     __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
-        const int k = c >> 2;
-        bool rev; chunk_brick(k, rev);
-        int s = c & 3;
-        if (rev) s = 3 - s;
-        const float sgn = rev ? -1.0f : 1.0f;
-        const float* src = ppr + poff(k) + plane_() + (s << (2 * DIR));
+        const int s = (c & 3) ^ prev;
+        const float sgn = prev ? -1.0f : 1.0f;
+        const float* src = ppr + pcur + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) m[q] = src[64 * PPB_PERM[DIR][q]];
         m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
@@ -972,23 +984,23 @@ struct IoBulk {
     __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
     // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
-        const int k = i >> 2, s = i & 3;
-        float* dh = hyd + hoff(k) + hlane() + (s << (2 * DIR));
+        const int s = i & 3;
+        float* dh = hyd + hprv + (s << SH);
         dh[0] = h[0];
         dh[64 * Dir<DIR>::U] = h[1];
         dh[64 * Dir<DIR>::V] = h[2];
         dh[64 * Dir<DIR>::W] = h[3];
         dh[64 * 4] = h[4];
-        float* dp = ppr + poff(k) + plane_() + (s << (2 * DIR));
+        float* dp = ppr + pst + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
-        if (s == 3) {                                          // brick k is complete: ship it
+        if (s == 3) {                                          // brick i >> 2 is complete: ship it
             fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
             __syncwarp();
             if (lane == 0) {
-                float* dst = P.out + gcol + (long long)k * P.SBd;
-                const float* sh = hyd + hoff(k);
-                const float* sp = ppr + poff(k);
+                float* dst = P.out + gcol + (long long)(i >> 2) * P.SBd;
+                const float* sh = hyd0 + hprv;
+                const float* sp = ppr0 + pst;
                 bulk_s2g(dst, sh, G::HB * 4);
                 bulk_s2g(dst + G::HB, sp, G::PB * 4);
                 if (ncol > 1) {
@@ -1001,14 +1013,16 @@ struct IoBulk {
     }
     __device__ __forceinline__ void end(int n) {
         // ring refill, once per brick: by the end of iteration n = 4m the slots of brick m - 2 are dead (its last
-        // cell was stored at n = 4m - 1; for a ghost brick the last read was earlier still)
+        // cell was stored at n = 4m - 1; for a ghost brick the last read was earlier still).  Hydro brick m sits in
+        // slot hs and brick m - 1 (receiving results) in hs - 1, so the dead slot is hs - 2 = hs + 1 (mod 3);
+        // the PPB brick being read is m - 1 in slot ps, the dead one is ps ^ 1.
         if ((n & 3) == 0) {
             const int m = n >> 2;
             __syncwarp();
             if (lane == 0) {
                 tma_wait_read0();                              // the bulk stores issued one iteration ago have read their slots
-                if (m + 1 >= k0 + G::NH && m + 1 <= kend) issue_hydro(m + 1);
-                if (m >= k0 + G::NP && m <= kend) issue_ppb(m);
+                if (m + 1 >= k0 + G::NH && m + 1 <= kend) issue_hydro(m + 1, hs == G::NH - 1 ? 0 : hs + 1);
+                if (m >= k0 + G::NP && m <= kend) issue_ppb(m, ps ^ 1);
             }
         }
     }
@@ -1137,7 +1151,7 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     P.nbrick_d = (P.n + 3) / 4;
     P.bc_lo = p.bc[2 * axis]; P.bc_hi = p.bc[2 * axis + 1];
     // data path: bulk-staged (any axis whose extent is a multiple of 4), else TMA-staged x, else direct
-    const bool use_bulk = ((c->io_path == 0 && axis == 0) || c->io_path == 3) && (P.n % 4 == 0) && !(axis == 0 && c->force_direct);
+    const bool use_bulk = (c->io_path == 0 || c->io_path == 3) && (P.n % 4 == 0) && !(axis == 0 && c->force_direct);
     const bool use_tma = !use_bulk && (axis == 0) && c->tma_ok && !c->force_direct && c->io_path != 1;
     int chunk = c->chunk > 0 ? c->chunk : P.n;
     if (use_tma || use_bulk) chunk = (chunk + 3) / 4 * 4;
