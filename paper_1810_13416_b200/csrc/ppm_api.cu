@@ -80,6 +80,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0;
     c->stream = (cudaStream_t)prm->stream;
     c->nblocks_red = 148 * 4;
+    { int dev = 0; cudaGetDevice(&dev); if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->sms < 1) c->sms = 148; }
     c->chunk = 0;
     c->err[0] = 0;
     // brick records of 4x4x4 cells x 15 fields; extents are rounded up to whole bricks (ppm_state_floats)

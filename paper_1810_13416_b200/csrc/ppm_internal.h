@@ -26,6 +26,8 @@ struct SweepParams {
     // SB = stride between bricks along that axis (960, 960*nbx, 960*nbx*nby floats)
     long long SBd, SBa, SBb;
     int nbrick_d;                   // bricks along the sweep axis
+    int ntiles;                     // bulk path: CTA tiles (8 x 1 brick columns) in the transverse plane
+    int tiles_a, chunk_b;           // bulk path: tiles [0, tiles_a) march segments of `chunk` cells, the rest of `chunk_b` cells
     int bc_lo, bc_hi;
     int chunk;                      // cells marched per thread (pencil split along the sweep axis)
     float dt, dx, dtdx, inv_dx;
@@ -53,6 +55,7 @@ struct ppm_ctx {
     int chunk;
     int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
     int tma_ok;                     // tensor maps for the x-sweep TMA path are valid
+    int sms;                        // multiprocessors of the device
     int io_path;                    // PPM_OPT_IO_PATH: 0 auto, 1 direct (+ TMA x), 3 bulk-staged wherever possible
     int force_direct;               // option: take the direct-global x path even when TMA is available
     long long launches;

@@ -893,18 +893,18 @@ struct IoBulk {
     const int k0, kend;          // first / last brick index along the sweep axis this pencil segment touches (ghosts included)
     // per-brick state, refreshed when a new brick comes up (once per 4 iterations); everything is warp-uniform
     int hs, ps;                  // ring slot of the hydro brick being read / of the PPB brick being read
-    int par;                     // bit 0: mbarrier phase of hydro slot hs; bit 1: of PPB slot ps
+    unsigned ph;                 // bit j: phase the next wait on mbarrier j (0..NH-1 hydro slots, NH.. PPB slots) must see; lives across pencil segments
     int hcur, hprv;              // float offset (from hyd) of the hydro slot being read / of the one receiving results
     int pcur, pst;               // float offset (from ppr) of the PPB slot being read / of the one receiving results
     int hrev, prev;              // 3 if the brick being read is a mirror image (cells taken in reverse, odd fields negated), else 0
     int jb;                      // image index of the hydro brick's cell 0
 
-    __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, int lane_, long long gcol_, int ncol_, int c0, int c1)
+    __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, unsigned ph_, int lane_, long long gcol_, int ncol_, int c0, int c1)
         : P(P_),
           hyd(wsm + (lane_ >> 4) * (G::HB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
           ppr(wsm + G::NH * G::HSLOT + (lane_ >> 4) * (G::PB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
           hyd0(wsm), ppr0(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_), gcol(gcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4),
-          hs(0), ps(0), par(0), hcur(0), hprv(0), pcur(0), pst(0), hrev(0), prev(0), jb(0) {
+          ph(ph_), hs(0), ps(0), hcur(0), hprv(0), pcur(0), pst(0), hrev(0), prev(0), jb(0) {
         if (lane == 0) {
 #pragma unroll
             for (int j = 0; j < G::NH; ++j) if (k0 + j <= kend) issue_hydro(k0 + j, j);
@@ -935,6 +935,10 @@ struct IoBulk {
         bulk_g2s(ppr0 + slot * G::PSLOT, src, G::PB * 4, bar + G::NH + slot);
         if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + P.SBa, G::PB * 4, bar + G::NH + slot);
     }
+    __device__ __forceinline__ void wait_slot(int j) {        // whole warp
+        mbar_wait(bar + j, (ph >> j) & 1);
+        ph ^= 1u << j;
+    }
     __device__ __forceinline__ void begin(int n) {
         const int s = n & 3;
         if (s == 0) {                                          // a new hydro brick k comes up; results of brick k - 1 start
@@ -943,23 +947,35 @@ struct IoBulk {
             hprv = hcur;
             if (k != k0) {
                 hs = (hs == G::NH - 1) ? 0 : hs + 1;
-                if (hs == 0) par ^= 1;
                 hcur = hs * G::HSLOT;
+            } else {
+                chunk_brick(k0, prev);                         // the very first PPB cell (c0 - 1) is the last cell of brick k0
+                wait_slot(G::NH);
             }
             jb = chunk_brick(k, hrev) * 4;
-            mbar_wait(bar + hs, par & 1);
+            wait_slot(hs);
+        } else if (s == 1) {
+            // ring refill, once per brick, one full iteration after brick k - 2 was shipped (so its bulk stores have
+            // long read their slots and lane 0 does not wait here).  Hydro brick k sits in slot hs and brick k - 1
+            // (receiving results) in hs - 1, so the dead hydro slot is hs + 1 (mod 3); the PPB brick being read is
+            // k - 1 in slot ps, the dead one is ps ^ 1.
+            const int k = n >> 2;
+            if (k != k0) {
+                __syncwarp();
+                if (lane == 0) {
+                    tma_wait_read0();
+                    if (k + 1 >= k0 + G::NH && k + 1 <= kend) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
+                    if (k >= k0 + G::NP && k <= kend) issue_ppb(k, ps ^ 1);
+                }
+            }
         } else if (s == 3) {                                   // PPB cell c = n - 3 is the first of brick c >> 2
-            const int c = n - 3, k = c >> 2;
+            const int k = (n - 3) >> 2;
             if (k > k0) {
                 ps ^= 1;
-                if (ps == 0) par ^= 2;
                 pcur = ps * G::PSLOT;
                 chunk_brick(k, prev);
-                mbar_wait(bar + G::NH + ps, (par >> 1) & 1);
+                wait_slot(G::NH + ps);
             }
-        } else if (n == 4 * k0 + 6) {                          // the very first PPB cell (c0 - 1) is the last cell of brick k0
-            chunk_brick(k0, prev);
-            mbar_wait(bar + G::NH, 0);
         }
     }
     __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
@@ -1011,27 +1027,18 @@ struct IoBulk {
             }
         }
     }
-    __device__ __forceinline__ void end(int n) {
-        // ring refill, once per brick: by the end of iteration n = 4m the slots of brick m - 2 are dead (its last
-        // cell was stored at n = 4m - 1; for a ghost brick the last read was earlier still).  Hydro brick m sits in
-        // slot hs and brick m - 1 (receiving results) in hs - 1, so the dead slot is hs - 2 = hs + 1 (mod 3);
-        // the PPB brick being read is m - 1 in slot ps, the dead one is ps ^ 1.
-        if ((n & 3) == 0) {
-            const int m = n >> 2;
-            __syncwarp();
-            if (lane == 0) {
-                tma_wait_read0();                              // the bulk stores issued one iteration ago have read their slots
-                if (m + 1 >= k0 + G::NH && m + 1 <= kend) issue_hydro(m + 1, hs == G::NH - 1 ? 0 : hs + 1);
-                if (m >= k0 + G::NP && m <= kend) issue_ppb(m, ps ^ 1);
-            }
-        }
-    }
+    __device__ __forceinline__ void end(int) {}
     __device__ __forceinline__ void finish() {
         if (lane == 0) tma_wait_all0();                        // smem must outlive the last bulk store
         __syncwarp();
     }
 };
 
+// One CTA = one segment of one pencil tile (8 x 1 brick columns).  Tiles [0, P.tiles_a) are cut into segments of
+// P.chunk cells, the remaining tiles into segments of P.chunk_b cells (both multiples of 4): the launcher marches
+// whole pencils while they fill complete waves of resident CTAs and cuts the pencils of the ragged last wave into
+// shorter segments, so that the SMs run dry together.  A cut costs 8 redundant warm-up cells; results do not
+// depend on where the cuts are.
 template <int DIR, int GRAV>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
@@ -1044,37 +1051,75 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     fence_async_smem();
     __syncthreads();
     const int nba = (P.na + 3) >> 2;
-    const int ba0 = (blockIdx.x * G::WARPS + warp) * 2;        // the warp's brick columns: ba0, ba0 + 1 along a; bb along b
-    if (ba0 >= nba) return;                                    // whole warp out of range (no block-wide sync below)
-    const int bb = blockIdx.y;
+    const int ntx = (nba + 2 * G::WARPS - 1) / (2 * G::WARPS);    // tiles along a
+    int tile, c0, c1;
+    {
+        const int ncha = (P.n + P.chunk - 1) / P.chunk;
+        const int na_ctas = P.tiles_a * ncha;
+        int u = blockIdx.x, ch = P.chunk, nch = ncha, t0 = 0;
+        if (u >= na_ctas) { u -= na_ctas; ch = P.chunk_b; nch = (P.n + ch - 1) / ch; t0 = P.tiles_a; }
+        const int t = u / nch;
+        tile = t0 + t;
+        c0 = (u - t * nch) * ch;
+        c1 = min(c0 + ch, P.n);
+    }
+    const int bb = tile / ntx, tx = tile - bb * ntx;
+    const int ba0 = (tx * G::WARPS + warp) * 2;                    // the warp's brick columns: ba0, ba0 + 1 along a; bb along b
+    if (ba0 >= nba) return;                                        // whole warp out of range (no block-wide sync below)
     const int a = (ba0 + (lane >> 4)) * 4 + (lane & 3);
     const int b = bb * 4 + ((lane >> 2) & 3);
-    const int c0 = blockIdx.z * P.chunk;
-    const int c1 = min(c0 + P.chunk, P.n);
     const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
-    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), lane, gcol, min(2, nba - ba0), c0, c1);
+    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
     march<DIR, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);
 }
 
+// cells per segment for the tiles of the ragged last wave: the cut that minimises (waves of segments) x (segment
+// length + 8 warm-up cells); ntail tiles, slots resident CTAs, n cells per pencil
+static int tail_chunk(int ntail, int slots, int n) {
+    int best = n;
+    double best_t = 1e300;
+    for (int np = 1; np <= 8; ++np) {
+        const int ch = ((n + np - 1) / np + 3) / 4 * 4;
+        if (ch < 32 && np > 1) break;
+        const int nch = (n + ch - 1) / ch;
+        const long long waves = ((long long)ntail * nch + slots - 1) / slots;
+        const double t = (double)waves * (ch + (nch > 1 ? 8 : 0));
+        if (t < best_t * 0.97) { best_t = t; best = ch; }          // prefer fewer cuts unless the gain is clear
+    }
+    return best;
+}
+
 template <int DIR, int GRAV>
-cudaError_t launch_bulk(const SweepParams& P, dim3 grid, cudaStream_t st) {
+cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
     using G = BulkGeom<DIR>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static int occ = 0;
+    if (!occ) {
         cudaError_t e = cudaFuncSetAttribute(ppm_sweep_bulk_kernel<DIR, GRAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ppm_sweep_bulk_kernel<DIR, GRAV>, G::WARPS * 32, G::SMEM);
+        if (e != cudaSuccess) return e;
+        if (occ < 1) occ = 1;
     }
-    ppm_sweep_bulk_kernel<DIR, GRAV><<<grid, G::WARPS * 32, G::SMEM, st>>>(P);
+    const int ntiles = P.ntiles, slots = sms * occ;
+    if (user_chunk > 0) {                                          // explicit: every pencil in segments of user_chunk cells
+        P.chunk = P.chunk_b = user_chunk;
+        P.tiles_a = ntiles;
+    } else {
+        P.chunk = P.n;
+        P.tiles_a = ntiles / slots * slots;                        // whole pencils while they fill complete waves
+        P.chunk_b = (P.tiles_a < ntiles) ? tail_chunk(ntiles - P.tiles_a, slots, P.n) : P.n;
+    }
+    const long long grid = (long long)P.tiles_a * ((P.n + P.chunk - 1) / P.chunk) + (long long)(ntiles - P.tiles_a) * ((P.n + P.chunk_b - 1) / P.chunk_b);
+    ppm_sweep_bulk_kernel<DIR, GRAV><<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
     return cudaGetLastError();
 }
 template <int DIR>
-cudaError_t launch_bulk_dir(const SweepParams& P, int grav, dim3 grid, cudaStream_t st) {
+cudaError_t launch_bulk_dir(SweepParams& P, int grav, int sms, int user_chunk, cudaStream_t st) {
     switch (grav) {
-        case PPM_GRAV_NONE: return launch_bulk<DIR, PPM_GRAV_NONE>(P, grid, st);
-        case PPM_GRAV_CONST_Z: return launch_bulk<DIR, PPM_GRAV_CONST_Z>(P, grid, st);
-        default: return launch_bulk<DIR, PPM_GRAV_RADIAL>(P, grid, st);
+        case PPM_GRAV_NONE: return launch_bulk<DIR, PPM_GRAV_NONE>(P, sms, user_chunk, st);
+        case PPM_GRAV_CONST_Z: return launch_bulk<DIR, PPM_GRAV_CONST_Z>(P, sms, user_chunk, st);
+        default: return launch_bulk<DIR, PPM_GRAV_RADIAL>(P, sms, user_chunk, st);
     }
 }
 
@@ -1167,10 +1212,11 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     const int nba = (P.na + 3) / 4, nbb = (P.nb + 3) / 4;
     cudaError_t e;
     if (use_bulk) {
-        dim3 grid((nba + 7) / 8, nbb, nchunks);                               // CTA = 4 warps x 2 brick columns along a
-        if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, grid, c->stream);
-        else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, grid, c->stream);
-        else e = launch_bulk_dir<2>(P, p.grav.kind, grid, c->stream);
+        P.ntiles = ((nba + 7) / 8) * nbb;                                     // CTA tile = 4 warps x 2 brick columns along a
+        const int uc = c->chunk > 0 ? chunk : 0;                              // 0: whole pencils, the last wave cut to finish together
+        if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
+        else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, c->sms, uc, c->stream);
+        else e = launch_bulk_dir<2>(P, p.grav.kind, c->sms, uc, c->stream);
     } else if (use_tma) {
         const CUtensorMap& tin = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur]);
         const CUtensorMap& tout = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur ^ 1]);
