@@ -183,9 +183,9 @@ def run_gpu(args):
     g = PPM.from_workload(w, device=dev)
     if args.chunk:
         g.set_chunk(args.chunk)
-    if args.x_direct:
-        from paper_1810_13416_b200.binding import OPT_X_PATH
-        g.set_option(OPT_X_PATH, 1)
+    if args.direct:
+        from paper_1810_13416_b200.binding import OPT_IO_PATH
+        g.set_option(OPT_IO_PATH, 1)
     _load_state(g, w, 8 if n >= 1024 else 32)
     dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
 
@@ -288,7 +288,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number (4 = 512^3, 5 = 1024^3)")
     ap.add_argument("--chunk", type=int, default=0)
-    ap.add_argument("--x-direct", action="store_true", help="x sweep through the direct global-memory path instead of TMA staging")
+    ap.add_argument("--direct", action="store_true", help="direct global-memory sweep path instead of the bulk-staged one")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window")
     ap.add_argument("--no-e2e", action="store_true")

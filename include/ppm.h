@@ -112,12 +112,13 @@ int ppm_sync(ppm_ctx *ctx);
 int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
 
 /* Options (results do not depend on them).
- *  PPM_OPT_X_PATH : 0 = automatic (nx a multiple of 4: the x sweep stages whole bricks through shared
- *                   memory with TMA), 1 = force the direct global-memory path. */
-enum { PPM_OPT_X_PATH = 1, PPM_OPT_IO_PATH = 2 };
+ *  PPM_OPT_IO_PATH : 0 = automatic: a sweep along an axis whose extent is a multiple of 4 stages whole brick
+ *                    records through shared memory with bulk copies (cp.async.bulk), any other axis uses the
+ *                    direct global-memory path; 1 = direct path for every axis. */
+enum { PPM_OPT_IO_PATH = 2 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
-/* 1 if the next x sweep will take the TMA-staged path, 0 if the direct path. */
-int ppm_x_path(const ppm_ctx *ctx);
+/* 1 if the next sweep along axis (0,1,2) will take the bulk-staged path, 0 if the direct path. */
+int ppm_axis_path(const ppm_ctx *ctx, int axis);
 
 /* Number of kernel launches the context has enqueued so far (bench.py reports it). */
 long long ppm_launch_count(const ppm_ctx *ctx);

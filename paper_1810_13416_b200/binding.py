@@ -21,9 +21,9 @@ BC_PERIODIC, BC_REFLECT = 0, 1
 GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_cfl_dt",
-           "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_x_path", "ppm_launch_count",
+           "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
            "ppm_state_floats", "ppm_destroy", "ppm_last_error")
-OPT_X_PATH, OPT_IO_PATH = 1, 2
+OPT_IO_PATH = 2
 
 
 class ppm_gravity(C.Structure):
@@ -62,7 +62,7 @@ def lib():
         L.ppm_sync.argtypes = [C.c_void_p]
         L.ppm_set_chunk.argtypes = [C.c_void_p, C.c_int]
         L.ppm_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
-        L.ppm_x_path.argtypes = [C.c_void_p]
+        L.ppm_axis_path.argtypes = [C.c_void_p, C.c_int]
         L.ppm_launch_count.argtypes = [C.c_void_p]
         L.ppm_launch_count.restype = C.c_longlong
         L.ppm_destroy.argtypes = [C.c_void_p]
@@ -197,8 +197,8 @@ class PPM:
     def set_option(self, option, value):
         self._check(lib().ppm_set_option(self._h, int(option), int(value)))
 
-    def x_path(self):
-        return int(lib().ppm_x_path(self._h))
+    def axis_path(self, axis):
+        return int(lib().ppm_axis_path(self._h, int(axis)))
 
     def launch_count(self):
         return int(lib().ppm_launch_count(self._h))

@@ -105,7 +105,6 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
         CUC(cudaMemcpy(c->tab64, t64.data(), sizeof(double) * 3 * g.n, cudaMemcpyHostToDevice));
     }
 #undef CUC
-    ppm_make_xmaps(c);      // x-sweep TMA path when nx % 4 == 0; otherwise the direct path serves all three axes
     *out = c;
     return PPM_OK;
 }
@@ -212,12 +211,11 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
-    if (option == PPM_OPT_X_PATH && (value == 0 || value == 1)) { c->force_direct = value; return PPM_OK; }
-    if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1 || value == 3)) { c->io_path = value; return PPM_OK; }
+    if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
     set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
     return PPM_EINVAL;
 }
 
-extern "C" int ppm_x_path(const ppm_ctx* c) { return (c && c->tma_ok && !c->force_direct) ? 1 : 0; }
+extern "C" int ppm_axis_path(const ppm_ctx* c, int axis) { return (c && axis >= 0 && axis <= 2 && ppm_axis_is_bulk(c, axis)) ? 1 : 0; }
 
 extern "C" long long ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }

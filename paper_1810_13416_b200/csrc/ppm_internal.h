@@ -54,18 +54,15 @@ struct ppm_ctx {
     int nblocks_red;
     int chunk;
     int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
-    int tma_ok;                     // tensor maps for the x-sweep TMA path are valid
     int sms;                        // multiprocessors of the device
-    int io_path;                    // PPM_OPT_IO_PATH: 0 auto, 1 direct (+ TMA x), 3 bulk-staged wherever possible
-    int force_direct;               // option: take the direct-global x path even when TMA is available
+    int io_path;                    // PPM_OPT_IO_PATH: 0 = bulk-staged where the sweep-axis extent is whole bricks, 1 = direct everywhere
     long long launches;
     char err[512];
-    alignas(64) unsigned char xmap[2][128];   // CUtensorMap of buf[0], buf[1]: 5-D {64, 15, nbx, nby, nbz}, box {64,5,1,2,1}
 };
 
 // launchers (defined in the .cu files)
 cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt);
-bool ppm_make_xmaps(ppm_ctx* c);
+bool ppm_axis_is_bulk(const ppm_ctx* c, int axis);
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs);
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs);
 cudaError_t ppm_launch_cfl(ppm_ctx* c);

@@ -17,25 +17,24 @@
 //   J  conservative update of cell n-4 in increment form (H9)
 //   K  PPB remap of cell n-4 from cells n-5, n-4, n-3    (P1-P4)
 //
-// State layout in HBM: SoA bricks — per field, bricks of 4x4x4 cells (256 B, x fastest inside), bricks
-// ordered x-fastest.  Every sweep direction then reads and writes whole 256-byte bricks (measured on SoA
-// planes: the x sweep re-read DRAM 6.5x because 16-byte row pieces thrash L2; profiles/).  The paper's
-// briquettes answer the same problem; here they are per-field (SoA), so a warp's 32
-// pencils = 2 bricks x (4x4 transverse cells) and no on-chip transposition is ever needed.
+// State layout in HBM: brick records — the grid is cut into bricks of 4x4x4 cells and a brick holds all 15
+// fields of its 64 cells, field-major: [bz][by][bx][15][4z][4y][4x], 3840 B per brick (ppm_internal.h).  The
+// paper's briquettes answer the same problem; here the fields stay separate inside the record
+// (SoA), so a warp's 32 pencils = 2 brick columns x (4x4 transverse cells) and no on-chip transposition or
+// 16||16 splice (L118, L124) is ever needed.
 //
 // Two data paths feed the same marching body:
-//   IoDirect  y/z sweeps (and grids whose extents are not multiples of 4, kept as SoA planes): loads and
-//             stores straight from/to HBM, 16 lanes per brick layer, L1 keeps a brick for the 2-4 iterations
-//             that consume it; next plane software-prefetched into registers.
-//   IoTmaX    x sweep: each warp stages one brick column step (2 bricks x 5 fields = 2560 B per TMA box,
-//             cp.async.bulk.tensor 5-D) into THREAD-PRIVATE 16-byte slots, double buffered behind the
-//             arithmetic, and writes results back with TMA stores; no transposes, no bank conflicts.
+//   IoBulk    (default; extent along the sweep axis a multiple of 4) every direction: the hydro part (1280 B) and
+//             the PPB part (2560 B) of a brick are 1-D bulk copies (cp.async.bulk + mbarrier) into per-warp rings
+//             in shared memory; results are written in place over the brick's own input and shipped back with a
+//             bulk store.  DRAM only ever sees whole 1280/2560-byte runs; no load waits in a register.
+//   IoDirect  (any extent) straight global loads / stores, 16 lanes per 64-byte brick layer, next plane
+//             software-prefetched into registers.
 //
 // fp32 arithmetic.  rho and p are carried as perturbations to the base state; every
 // difference of nearly equal numbers is taken between perturbation-sized quantities only ("explicitly
 // cancel out all large contributions", L35): the Newton iteration runs on p*' = p* - p0f, the update
 // adds increments to rho', p' instead of rebuilding them from E.
-#include <cuda.h>
 #include <stdlib.h>
 
 #include "ppm_internal.h"
@@ -648,20 +647,7 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     march<DIR, GRAV>(P, io, a, b, c0, c1, true, wmask);
 }
 
-// =====================================================================================================
-// IoTmaX: x sweep (nx a multiple of 4).  Warp = 2 brick columns adjacent in y (lane = bsel*16 + iz*4 + iy).  A TMA
-// box {64 floats, 5 fields, 1 bx, 2 by, 1 bz} lands as [bsel][field][iz][iy][4 x-cells]: every lane owns the 16
-// bytes at (bsel, iz, iy) of every field — thread-private, and whole 1280-byte runs of a brick record on the wire.
-// Rings: hydro fields 2 chunks (2 x 2560 B), PPB fields 2 chunks (2 x 5120 B, read three cells later),
-// results 1 chunk (7680 B) written back by TMA store.  23040 B per warp.
-// =====================================================================================================
-constexpr int TX_ROWS = 32, TX_CH = 4;
-constexpr int TX_HYD = 5 * TX_ROWS * TX_CH;           // floats per hydro chunk buffer
-constexpr int TX_PPB = 10 * TX_ROWS * TX_CH;
-constexpr int TX_OUT = 15 * TX_ROWS * TX_CH;
-constexpr int TX_WARP_FLOATS = 2 * TX_HYD + 2 * TX_PPB + TX_OUT;   // 5760 floats = 23040 B
-constexpr int TX_WARPS = 4;
-
+// ---- shared-memory / mbarrier / bulk-copy primitives ----------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -680,168 +666,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
                      : "=r"(done) : "r"(addr), "r"(parity) : "memory");
     } while (!__all_sync(0xffffffffu, done));   // warp-uniform exit: every lane polls, the vote decides
 }
-// coordinates: (element in brick = 0, field, bx, by, bz)
-__device__ __forceinline__ void tma_load_brick(void* dst, const CUtensorMap* map, uint64_t* bar, int bx, int by, int bz, int f) {
-    asm volatile(
-        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(0), "r"(f), "r"(bx), "r"(by), "r"(bz) : "memory");
-}
-__device__ __forceinline__ void tma_store_brick(const CUtensorMap* map, const void* src, int bx, int by, int bz, int f) {
-    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
-                 ::"l"(map), "r"(smem_u32(src)), "r"(0), "r"(f), "r"(bx), "r"(by), "r"(bz) : "memory");
-}
-// float index of field F (0..14) inside a staged group of boxes, each box = [2 bsel][5 fields][64]
-__device__ __forceinline__ constexpr int tx_slot(int F) { return (F / 5) * (2 * 5 * 64) + (F % 5) * 64; }
 __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_all0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
-struct IoTmaX {
-    const SweepParams& P;
-    const CUtensorMap* tin;
-    const CUtensorMap* tout;
-    float* hyd;          // warp's hydro ring [2][5][32][4]
-    float* ppbuf;        // warp's PPB ring   [2][10][32][4]
-    float* outb;         // warp's result chunk [15][32][4]
-    uint64_t* bar;       // [0..1] hydro ring, [2..3] PPB ring
-    const int lane, lbase, by0, bz;   // lbase: the lane's 16-byte slot inside a box = bsel*320 + (iz*4+iy)*4
-    const int k0, kend;  // first / last chunk index (chunk k = brick bx = k = cells 4k .. 4k+3)
-    bool store_pending;
-
-    __device__ __forceinline__ IoTmaX(const SweepParams& P_, const CUtensorMap* ti, const CUtensorMap* to, float* wsm, uint64_t* wbar,
-                                      int lane_, int by0_, int bz_, int c0, int c1)
-        : P(P_), tin(ti), tout(to), hyd(wsm), ppbuf(wsm + 2 * TX_HYD), outb(wsm + 2 * TX_HYD + 2 * TX_PPB), bar(wbar),
-          lane(lane_), lbase((lane_ >> 4) * 320 + (lane_ & 15) * 4), by0(by0_), bz(bz_), k0(c0 / TX_CH - 1), kend(c1 / TX_CH), store_pending(false) {
-        if (lane == 0) {
-            issue_hydro(k0); issue_ppb(k0);
-            if (k0 + 1 <= kend) { issue_hydro(k0 + 1); issue_ppb(k0 + 1); }
-        }
-    }
-    // brick index bx holding chunk k (ghost chunks map onto their periodic / mirror image; mirrored ones are read reversed)
-    __device__ __forceinline__ int chunk_bx(int k, bool& rev) const {
-        rev = false;
-        const int nk = P.nbrick_d;
-        if (k < 0) { if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = true; return 0; }
-        if (k >= nk) { if (P.bc_hi == PPM_BC_PERIODIC) return 0; rev = true; return nk - 1; }
-        return k;
-    }
-    __device__ __forceinline__ void issue_hydro(int k) {
-        bool rev; const int bx = chunk_bx(k, rev);
-        const int bsel = (k - k0) & 1;
-        mbar_expect_tx(bar + bsel, TX_HYD * 4);
-        tma_load_brick(hyd + bsel * TX_HYD, tin, bar + bsel, bx, by0, bz, 0);
-    }
-    __device__ __forceinline__ void issue_ppb(int k) {
-        bool rev; const int bx = chunk_bx(k, rev);
-        const int bsel = (k - k0) & 1;
-        mbar_expect_tx(bar + 2 + bsel, TX_PPB * 4);
-        tma_load_brick(ppbuf + bsel * TX_PPB, tin, bar + 2 + bsel, bx, by0, bz, 5);
-        tma_load_brick(ppbuf + bsel * TX_PPB + TX_HYD, tin, bar + 2 + bsel, bx, by0, bz, 10);
-    }
-    __device__ __forceinline__ void begin(int n) {
-        if ((n & 3) == 0) {                                   // first cell of hydro chunk k
-            const int k = n >> 2;
-            mbar_wait(bar + ((k - k0) & 1), ((k - k0) >> 1) & 1);
-        }
-        const int c = n - 3;                                   // PPB cell of this iteration
-        if ((c & 3) == 0 || c == 4 * k0 + 3) {                 // first PPB cell read from its chunk
-            const int k = c >> 2;
-            if (k >= k0) mbar_wait(bar + 2 + ((k - k0) & 1), ((k - k0) >> 1) & 1);
-        }
-    }
-    __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
-        const int k = n >> 2;
-        bool rev; const int bx = chunk_bx(k, rev);
-        int s = n & 3;
-        if (rev) s = 3 - s;
-        sgn = rev ? -1.0f : 1.0f;
-        j = bx * TX_CH + s;
-        const float* src = hyd + ((k - k0) & 1) * TX_HYD + lbase + s;
-        v[0] = src[0];
-        v[1] = sgn * src[1 * 64];                              // normal velocity ux is field 1 (odd under mirror)
-        v[2] = src[2 * 64];
-        v[3] = src[3 * 64];
-        v[4] = src[4 * 64];
-    }
-    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
-        const int k = c >> 2;
-        bool rev; chunk_bx(k, rev);
-        int s = c & 3;
-        if (rev) s = 3 - s;
-        const float sgn = rev ? -1.0f : 1.0f;
-        const float* src = ppbuf + ((k - k0) & 1) * TX_PPB + lbase + s;
-#pragma unroll
-        for (int q = 0; q < 10; ++q) m[q] = src[tx_slot(PPB_PERM[0][q])];
-        m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
-    }
-    __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
-    __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
-        const int s = i & 3;
-        if (s == 0 && store_pending) {                         // the previous chunk's TMA store must have read outb
-            if (lane == 0) tma_wait_read0();
-            __syncwarp();
-            store_pending = false;
-        }
-        float* dst = outb + lbase + s;
-#pragma unroll
-        for (int f = 0; f < 5; ++f) dst[f * 64] = h[f];
-#pragma unroll
-        for (int q = 0; q < 10; ++q) dst[tx_slot(5 + PPB_PERM[0][q])] = m[q];
-        if (s == 3) {
-            fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
-            __syncwarp();
-            if (lane == 0) {
-                const int bx = i >> 2;
-                tma_store_brick(tout, outb, bx, by0, bz, 0);
-                tma_store_brick(tout, outb + TX_HYD, bx, by0, bz, 5);
-                tma_store_brick(tout, outb + 2 * TX_HYD, bx, by0, bz, 10);
-                tma_commit();
-            }
-            store_pending = true;
-        }
-    }
-    __device__ __forceinline__ void end(int n) {
-        // ring refills: a buffer is free once every lane has taken its last value from it
-        if ((n & 3) == 3) {                                    // hydro chunk k = n>>2 fully consumed
-            const int k = n >> 2;
-            __syncwarp();
-            if (lane == 0 && k + 2 <= kend) issue_hydro(k + 2);
-        }
-        const int c = n - 3;
-        if ((c & 3) == 3) {                                    // PPB chunk k = c>>2 fully consumed
-            const int k = c >> 2;
-            __syncwarp();
-            if (lane == 0 && k >= k0 && k + 2 <= kend) issue_ppb(k + 2);
-        }
-    }
-    __device__ __forceinline__ void finish() {
-        if (lane == 0) tma_wait_all0();                        // smem must outlive the last bulk store
-        __syncwarp();
-    }
-};
-
-template <int GRAV>
-__global__ void __launch_bounds__(TX_WARPS * 32, 2) ppm_sweep_x_tma_kernel(const SweepParams P, const __grid_constant__ CUtensorMap tin,
-                                                                        const __grid_constant__ CUtensorMap tout) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* sm = reinterpret_cast<float*>(smem_raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)TX_WARPS * TX_WARP_FLOATS * 4);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x < TX_WARPS * 4) mbar_init(bars + threadIdx.x, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    fence_async_smem();
-    __syncthreads();
-    const int by0 = (blockIdx.x * TX_WARPS + warp) * 2;        // the warp's two bricks: by0, by0+1 at bz
-    if (by0 * 4 >= P.na) return;                               // whole warp out of range (no block-wide sync below)
-    const int bz = blockIdx.y;
-    const int a = (by0 + (lane >> 4)) * 4 + (lane & 3);        // y
-    const int b = bz * 4 + ((lane >> 2) & 3);                  // z
-    const int c0 = blockIdx.z * P.chunk;
-    const int c1 = min(c0 + P.chunk, P.n);
-    IoTmaX io(P, &tin, &tout, sm + warp * TX_WARP_FLOATS, bars + warp * 4, lane, by0, bz, c0, c1);
-    march<0, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);   // pad pencils of a ragged grid compute garbage that is never read
-}
 
 // =====================================================================================================
 // IoBulk: every sweep direction (sweep-axis extent a multiple of 4).  Warp = 2 brick columns adjacent along a.
@@ -1133,53 +961,11 @@ cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cu
     return cudaGetLastError();
 }
 
-constexpr size_t TX_SMEM = (size_t)TX_WARPS * TX_WARP_FLOATS * 4 + TX_WARPS * 4 * sizeof(uint64_t);
-
-template <int GRAV>
-cudaError_t launch_x_tma(const SweepParams& P, const CUtensorMap& tin, const CUtensorMap& tout, dim3 grid, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(ppm_sweep_x_tma_kernel<GRAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TX_SMEM);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    ppm_sweep_x_tma_kernel<GRAV><<<grid, TX_WARPS * 32, TX_SMEM, st>>>(P, tin, tout);
-    return cudaGetLastError();
-}
-
 }  // namespace
 
-// ---- host: tensor maps for the x-sweep TMA path -------------------------------------------------------
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-bool ppm_make_xmaps(ppm_ctx* c) {
-    c->tma_ok = 0;
-    const ppm_params& p = c->prm;
-    if (p.nx % 4 != 0) return false;                            // ghost chunks must be whole bricks (mirror / wrap by brick)
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
-        qres != cudaDriverEntryPointSuccess) {
-        cudaGetLastError();
-        return false;
-    }
-    EncodeTiledFn enc = (EncodeTiledFn)fn;
-    const cuuint64_t nbx = c->nbx, nby = c->nby, nbz = c->nbz;
-    const cuuint64_t rec = PPM_BRICK_FLOATS * sizeof(float);
-    const cuuint64_t dims[5] = {64, PPM_NFIELDS, nbx, nby, nbz};
-    const cuuint64_t strides[4] = {256, rec, rec * nbx, rec * nbx * nby};
-    const cuuint32_t box[5] = {64, 5, 1, 2, 1};
-    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    for (int b = 0; b < 2; ++b) {
-        CUresult r = enc(reinterpret_cast<CUtensorMap*>(c->xmap[b]), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, c->buf[b], dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) return false;
-    }
-    c->tma_ok = 1;
-    return true;
+bool ppm_axis_is_bulk(const ppm_ctx* c, int axis) {
+    const int ext[3] = {c->prm.nx, c->prm.ny, c->prm.nz};
+    return c->io_path == 0 && ext[axis] % 4 == 0;
 }
 
 cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
@@ -1195,11 +981,10 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     P.SBd = SB[axis]; P.SBa = SB[ia]; P.SBb = SB[ib];
     P.nbrick_d = (P.n + 3) / 4;
     P.bc_lo = p.bc[2 * axis]; P.bc_hi = p.bc[2 * axis + 1];
-    // data path: bulk-staged (any axis whose extent is a multiple of 4), else TMA-staged x, else direct
-    const bool use_bulk = (c->io_path == 0 || c->io_path == 3) && (P.n % 4 == 0) && !(axis == 0 && c->force_direct);
-    const bool use_tma = !use_bulk && (axis == 0) && c->tma_ok && !c->force_direct && c->io_path != 1;
+    // data path: bulk-staged when the extent along the sweep axis is whole bricks, else direct
+    const bool use_bulk = ppm_axis_is_bulk(c, axis);
     int chunk = c->chunk > 0 ? c->chunk : P.n;
-    if (use_tma || use_bulk) chunk = (chunk + 3) / 4 * 4;
+    if (use_bulk) chunk = (chunk + 3) / 4 * 4;
     if (chunk > P.n) chunk = P.n;
     P.chunk = chunk;
     P.dt = (float)dt; P.dx = (float)p.dx; P.dtdx = (float)(dt / p.dx); P.inv_dx = (float)(1.0 / p.dx);
@@ -1217,13 +1002,6 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
         if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
         else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, c->sms, uc, c->stream);
         else e = launch_bulk_dir<2>(P, p.grav.kind, c->sms, uc, c->stream);
-    } else if (use_tma) {
-        const CUtensorMap& tin = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur]);
-        const CUtensorMap& tout = *reinterpret_cast<const CUtensorMap*>(c->xmap[c->cur ^ 1]);
-        dim3 grid((nba + TX_WARPS * 2 - 1) / (TX_WARPS * 2), nbb, nchunks);   // CTA = 8 brick columns along y, 1 along z
-        if (p.grav.kind == PPM_GRAV_NONE) e = launch_x_tma<PPM_GRAV_NONE>(P, tin, tout, grid, c->stream);
-        else if (p.grav.kind == PPM_GRAV_CONST_Z) e = launch_x_tma<PPM_GRAV_CONST_Z>(P, tin, tout, grid, c->stream);
-        else e = launch_x_tma<PPM_GRAV_RADIAL>(P, tin, tout, grid, c->stream);
     } else {
         dim3 block(PPM_CTA, 1, 1);
         dim3 grid((nba + PPM_CTA / 16 - 1) / (PPM_CTA / 16), nbb, nchunks);

@@ -86,19 +86,19 @@ def test_cfg1_full_32cubed_20_steps():
 
 
 def test_data_paths_agree():
-    """the TMA-staged x sweep (default when nx % 4 == 0) and the direct global-memory x sweep run the same marching
-    body on the same brick records: bit-identical results."""
+    """the bulk-staged sweeps (default when the extent along the sweep axis is whole bricks) and the direct
+    global-memory sweeps run the same marching body on the same brick records: bit-identical results."""
     PPM = _gpu()
-    from paper_1810_13416_b200.binding import OPT_X_PATH
-    for cfg, n in ((1, 32), (4, 32), (3, 32), (1, 40)):     # 40: ny = 10 bricks, the last TMA warp of a CTA row is half empty
+    from paper_1810_13416_b200.binding import OPT_IO_PATH
+    for cfg, n in ((1, 32), (4, 32), (3, 32), (2, 32), (1, 40)):     # 40: 10 brick columns, the last warp of a CTA row is half empty
         w = W.make(cfg, n=n)
         f = w.fields().cuda()
         res = []
-        for mode in ("tma", "direct"):
+        for mode in ("bulk", "direct"):
             g = PPM.from_workload(w)
             if mode == "direct":
-                g.set_option(OPT_X_PATH, 1)
-            assert g.x_path() == (1 if mode == "tma" else 0)
+                g.set_option(OPT_IO_PATH, 1)
+            assert [g.axis_path(d) for d in range(3)] == [1 if mode == "bulk" else 0] * 3
             g.set_state(f)
             for s in range(3):
                 g.step(g.cfl_dt(0.8), s * 2)
@@ -170,7 +170,7 @@ def test_ragged_grid_all_boundaries_and_orders(dims):
     for bc in ((P_, P_, R_, R_, P_, P_), (R_, R_, P_, P_, R_, R_)):
         o = ob.Oracle(nx, ny, nz, 0.03, 1.4, bc, None)
         g = PPM(nx, ny, nz, 0.03, 1.4, bc)
-        assert g.x_path() == (1 if nx % 4 == 0 else 0)
+        assert [g.axis_path(d) for d in range(3)] == [int(e % 4 == 0) for e in (nx, ny, nz)]
         o.set_state(f)
         g.set_state(f)
         for order in range(6):
