@@ -34,7 +34,7 @@ FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, 
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` capture
 # (profiles/), keyed by cells per side; None where no capture exists.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {512: 16.097e9}      # profiles/r1f_sweeps_ncu_full.md: 8.088 GB read + 8.009 GB written per launch
 
 
 def _peaks():
@@ -260,7 +260,7 @@ def run_gpu(args):
                    "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(n), "peak_kind": "of " + peak_kind,
-                     "kernel": "ppm_sweep_kernel (3 launches per step; every launch moves 120 B/cell)",
+                     "kernel": "ppm_sweep_bulk_kernel (3 launches per step; every launch moves 120 B/cell)",
                      "alu": {"achieved": alu, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu / FP32_PEAK_TFLOPS,
                              "flops_per_cell_sweep": FLOPS_PER_CELL_SWEEP}},
         "clocks": clocks, "gpu_launches": int(launches),
