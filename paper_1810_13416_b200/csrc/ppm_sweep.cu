@@ -350,17 +350,6 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             pf[4] = full.y;
             gw[4] = bs.g;
         }
-        // ---- A, B, C, D: interpolation of cell n-2 ----------------------------------------------------
-        const V5 d2n = fma5(q[3], -2.0f, q[4]) + q[2];                                           // d2_{n-1}
-        const V5 Fn = fma5(q[1] + q[4], -1.0f / 12.0f, (q[2] + q[3]) * (7.0f / 12.0f));          // face (n-2)+1/2 (H1)
-        const V5 Fnl = map3(q[2], Fn, q[3], [](float x, float y, float z) { return med3(x, y, z); });   // H2: clamp
-        V5 pLn, pRn;
-        {
-            const V5 num = d2n - d2a;
-            const V5 den = fma5(abs5(d2b), 2.0f, abs5(d2a)) + (abs5(d2n) + bc5(PPM_TINY));
-            const V5 om = map3(num, den, den, [](float x, float y, float) { return sat(fmaf(fabsf(x) * rcp(y), 5.0f, -0.5f)); });   // H3
-            parabola(q[2], Fcl, Fnl, Fc, Fn, om, pLn, pRn);
-        }
         // ---- E, F: flattening ---------------------------------------------------------------------------
         const float cn2 = fsqrt(gam * pf[2] * rcp(rf[3]));          // c_{n-2}
         float ftn;
@@ -427,6 +416,18 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 const float su = hdt * gw[1] * fdiv(qc.A.x, rho);
                 Wr = Wr + bc(k * db.x); Wp = Wp + bc(k * db.y); Wu = Wu + bc(su);
             }
+        }
+        // ---- A, B, C, D: interpolation of cell n-2 (placed after the tracing of cell n-3, the last reader of the carried
+        //      parabola: the new one can then take its registers and the rotation at the loop end costs no move) ----
+        const V5 d2n = fma5(q[3], -2.0f, q[4]) + q[2];                                           // d2_{n-1}
+        const V5 Fn = fma5(q[1] + q[4], -1.0f / 12.0f, (q[2] + q[3]) * (7.0f / 12.0f));          // face (n-2)+1/2 (H1)
+        const V5 Fnl = map3(q[2], Fn, q[3], [](float x, float y, float z) { return med3(x, y, z); });   // H2: clamp
+        V5 pLn, pRn;
+        {
+            const V5 num = d2n - d2a;
+            const V5 den = fma5(abs5(d2b), 2.0f, abs5(d2a)) + (abs5(d2n) + bc5(PPM_TINY));
+            const V5 om = map3(num, den, den, [](float x, float y, float) { return sat(fmaf(fabsf(x) * rcp(y), 5.0f, -0.5f)); });   // H3
+            parabola(q[2], Fcl, Fnl, Fc, Fn, om, pLn, pRn);
         }
         // ---- I: Riemann problem at face (n-4)+1/2 : L = left state carried from cell n-4, R = right state of cell n-3
         float Frm, Frn, FrE;
