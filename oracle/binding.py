@@ -37,6 +37,10 @@ def lib():
         L.oracle_raw_field.argtypes = [C.c_void_p, C.c_int]
         L.oracle_sweep.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.oracle_set_flatten3d.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_flatten3d_update.argtypes = [C.c_void_p]
+        L.oracle_flatten3d_field.argtypes = [C.c_void_p]
+        L.oracle_flatten3d_field.restype = C.POINTER(C.c_double)
         L.oracle_cfl_dt.argtypes = [C.c_void_p, C.c_double, dp]
         L.oracle_reduce_conserved.argtypes = [C.c_void_p, dp]
         L.oracle_h1_face.restype = C.c_double
@@ -59,7 +63,7 @@ def lib():
         L.oracle_p4_remap.argtypes = [C.c_int, dp, dp, C.c_double, C.c_double, dp]
         L.oracle_sweep_pencil.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double,
                                           C.c_double, C.POINTER(dp), C.POINTER(dp), dp, dp, dp, dp, dp,
-                                          C.POINTER(dp), C.POINTER(dp)]
+                                          C.POINTER(dp), C.POINTER(dp), dp]
         L.oracle_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -136,8 +140,9 @@ def p4_remap(deg, a3x3, M3, dMl, dMr):
 
 
 def sweep_pencil(d, dx, dt, gamma, q5, m10, rho0c=None, p0c=None, gd=None, rho0f=None, p0f=None,
-                 rho_floor=1e-30, p_floor=1e-30):
-    """q5: (5, n+8) = rho', u_normal, v, w, p' with ghosts; m10: (10, n+8).  Returns (5,n), (10,n)."""
+                 rho_floor=1e-30, p_floor=1e-30, ft_ext=None):
+    """q5: (5, n+8) = rho', u_normal, v, w, p' with ghosts; m10: (10, n+8).  Returns (5,n), (10,n).
+    ft_ext: (n+8,) un-spread flattening coefficients that replace the 1-D detector (3-D flattening mode)."""
     q5, m10 = _arr(q5), _arr(m10)
     nt = q5.shape[1]
     n = nt - 8
@@ -154,7 +159,7 @@ def sweep_pencil(d, dx, dt, gamma, q5, m10, rho0c=None, p0c=None, gd=None, rho0f
     qop = (dp * 5)(*[_d(qo[k]) for k in range(5)])
     mop = (dp * 10)(*[_d(mo[k]) for k in range(10)])
     lib().oracle_sweep_pencil(n, d, dx, dt, gamma, rho_floor, p_floor, qi, mi, _d(rho0c), _d(p0c), _d(gd),
-                              _d(rho0f), _d(p0f), qop, mop)
+                              _d(rho0f), _d(p0f), qop, mop, _d(_arr(ft_ext)) if ft_ext is not None else None)
     return qo, mo
 
 
@@ -220,6 +225,19 @@ class Oracle:
     def raw_field(self, f):
         p = lib().oracle_raw_field(self._h, f)
         return np.ctypeslib.as_array(p, shape=self.shape)
+
+    def set_flatten3d(self, on=True):
+        """NEXT-1: fully 3-D shock detector instead of the per-sweep 1-D one"""
+        rc = lib().oracle_set_flatten3d(self._h, int(bool(on)))
+        if rc:
+            raise ValueError("oracle_set_flatten3d rc=%d" % rc)
+
+    def flatten3d_field(self, update=True):
+        """F~ [nz][ny][nx] evaluated on the current state"""
+        if update:
+            lib().oracle_flatten3d_update(self._h)
+        ptr = lib().oracle_flatten3d_field(self._h)
+        return np.ctypeslib.as_array(ptr, shape=self.shape).copy()
 
     def sweep(self, d, dt):
         rc = lib().oracle_sweep(self._h, d, dt)

@@ -51,6 +51,8 @@ typedef struct oracle_ctx {
     int bc[6];           /* xlo xhi ylo yhi zlo zhi */
     double *q[NF];       /* state: perturbation form, no ghosts */
     double *qn[NF];      /* sweep output */
+    int flat3d;          /* NEXT-1: fully 3-D shock detector instead of the per-sweep 1-D one */
+    double *F3;          /* F~ of every cell (flat3d only), evaluated on the state at the start of the call */
 } oracle_ctx;
 
 static double clamp01(double x) { return fmin(1.0, fmax(0.0, x)); }
@@ -327,7 +329,7 @@ void oracle_sweep_pencil(int n, int d, double dx, double dt, double gamma, doubl
                          const double *const q[5], const double *const m[10],
                          const double *rho0c, const double *p0c, const double *gd,
                          const double *rho0f, const double *p0f,
-                         double *const qn[5], double *const mn[10]) {
+                         double *const qn[5], double *const mn[10], const double *ft_ext) {
     const int nt = n + 2 * NG;
     const double dtdx = dt / dx;
     double *buf = (double *)calloc((size_t)nt * 40 + 64, sizeof(double));
@@ -356,6 +358,8 @@ void oracle_sweep_pencil(int n, int d, double dx, double dt, double gamma, doubl
     for (int j = 2; j <= nt - 3; ++j) {
         double p5[5] = {p[j - 2], p[j - 1], p[j], p[j + 1], p[j + 2]};
         ft[j] = oracle_h4_ftilde(p5, q[1][j - 1], q[1][j + 1], c[j]);
+        /* NEXT-1 ("fully 3-D"): the un-spread coefficient comes from the 3-D detector field instead */
+        if (ft_ext) ft[j] = ft_ext[j];
     }
     for (int j = 3; j <= nt - 4; ++j) fl[j] = fmax(ft[j - 1], fmax(ft[j], ft[j + 1]));
     /* H2, H3, H4 applied: parabolas of cells 3 .. nt-4 */
@@ -479,6 +483,7 @@ oracle_ctx *oracle_create(int nx, int ny, int nz, const int org[3], double dx, d
 void oracle_destroy(oracle_ctx *c) {
     if (!c) return;
     for (int f = 0; f < NF; ++f) { free(c->q[f]); free(c->qn[f]); }
+    free(c->F3);
     free(c->g); free(c->rho0); free(c->p0);
     free(c);
 }
@@ -521,7 +526,7 @@ int oracle_get_state(const oracle_ctx *c, double *const fields[NF]) {
 double *oracle_raw_field(oracle_ctx *c, int f) { return c->q[f]; }
 
 /* C2/C3/C4/C5: one sweep along d over every pencil of the window. */
-int oracle_sweep(oracle_ctx *c, int d, double dt) {
+static int sweep_impl(oracle_ctx *c, int d, double dt) {
     const int n = c->n[d];
     const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;   /* transverse axes, ascending */
     const int n1 = c->n[d1], n2 = c->n[d2];
@@ -532,7 +537,7 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
 #pragma omp parallel for collapse(2) schedule(static)
     for (int b = 0; b < n2; ++b)
         for (int a = 0; a < n1; ++a) {
-            double *buf = (double *)malloc(sizeof(double) * ((size_t)nt * 20 + 2 + (size_t)n * 15));
+            double *buf = (double *)malloc(sizeof(double) * ((size_t)nt * 21 + 2 + (size_t)n * 15));
             if (!buf) { fail = 1; continue; }
             double *qa[5], *ma[10], *r0c, *p0c, *gd, *r0f, *p0f, *qo[5], *mo[10];
             double *cur = buf;
@@ -540,6 +545,7 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
             for (int k = 0; k < 10; ++k) { ma[k] = cur; cur += nt; }
             r0c = cur; cur += nt; p0c = cur; cur += nt; gd = cur; cur += nt;
             r0f = cur; cur += nt + 1; p0f = cur; cur += nt + 1;
+            double *f3 = cur; cur += nt;
             for (int k = 0; k < 5; ++k) { qo[k] = cur; cur += n; }
             for (int k = 0; k < 10; ++k) { mo[k] = cur; cur += n; }
             int ijk[3], gidx[3];
@@ -559,6 +565,7 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
                 double gv[3];
                 cell_base(c, gidx[0], gidx[1], gidx[2], &r0c[j], &p0c[j], gv);
                 gd[j] = sgn * gv[d];
+                f3[j] = (c->flat3d && c->F3) ? c->F3[id] : 0.0;    /* a ghost cell carries its image's F~ (the detector is mirror-invariant) */
             }
             for (int f = 0; f <= nt; ++f) {
                 int gf = image_face(c, d, f - NG);
@@ -567,7 +574,8 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
                 base_at(c, X, &r0f[f], &p0f[f], gv);
             }
             oracle_sweep_pencil(n, d, c->dx, dt, c->gamma, c->rho_floor, c->p_floor,
-                                (const double *const *)qa, (const double *const *)ma, r0c, p0c, gd, r0f, p0f, qo, mo);
+                                (const double *const *)qa, (const double *const *)ma, r0c, p0c, gd, r0f, p0f, qo, mo,
+                                (c->flat3d && c->F3) ? f3 : NULL);
             for (int i = 0; i < n; ++i) {
                 ijk[d] = i;
                 size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
@@ -585,12 +593,64 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
     return 0;
 }
 
+/* NEXT-1 ("a fully 3-D treatment of the shock dissipation ... we evaluate in 3-D the
+ * strength and orientation of shocks").  [reading R5b, DESIGN.md]  F~_i = max over the three directions d of the
+ * H4 coefficient f~^d_i, each evaluated along d (full p at i-2..i+2, velocity component u_d at i-1, i+1, c_i) on
+ * the state the call starts from; ghost cells by the boundary images of C3.  A sweep then spreads it as H4 does:
+ * f_i = max(F~_{i-1}, F~_i, F~_{i+1}) along the sweep direction.  So a shock seen in ANY direction flattens the
+ * parabolas of EVERY sweep through its cells, which removes the imprint of the grid directions. */
+int oracle_set_flatten3d(oracle_ctx *c, int on) {
+    if (!c) return 1;
+    c->flat3d = on ? 1 : 0;
+    if (on && !c->F3) c->F3 = (double *)calloc(ncell(c), sizeof(double));
+    return (on && !c->F3) ? 2 : 0;
+}
+
+int oracle_flatten3d_update(oracle_ctx *c) {
+    if (!c || !c->F3) return 1;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < c->n[2]; ++k)
+        for (int j = 0; j < c->n[1]; ++j)
+            for (int i = 0; i < c->n[0]; ++i) {
+                const int ijk0[3] = {i, j, k};
+                double F = 0.0;
+                for (int d = 0; d < 3; ++d) {
+                    double p5[5], u3[3], ci = 0.0;
+                    for (int o = -2; o <= 2; ++o) {
+                        int ijk[3] = {ijk0[0], ijk0[1], ijk0[2]}, g[3], sgn, gpos;
+                        ijk[d] = image_cell(c, d, ijk0[d] + o, &sgn, &gpos);
+                        for (int e = 0; e < 3; ++e) g[e] = c->org[e] + ijk[e];
+                        g[d] = gpos;
+                        size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                        double r0, p0, gv[3];
+                        cell_base(c, g[0], g[1], g[2], &r0, &p0, gv);
+                        p5[o + 2] = p0 + c->q[4][id];
+                        if (o >= -1 && o <= 1) u3[o + 1] = sgn * c->q[1 + d][id];
+                        if (o == 0) ci = sqrt(c->gamma * p5[2] / (r0 + c->q[0][id]));
+                    }
+                    F = fmax(F, oracle_h4_ftilde(p5, u3[0], u3[2], ci));
+                }
+                c->F3[cidx(c, i, j, k)] = F;
+            }
+    return 0;
+}
+
+const double *oracle_flatten3d_field(const oracle_ctx *c) { return c ? c->F3 : NULL; }
+
+/* one sweep on its own; in 3-D flattening mode F~ is evaluated on the state this sweep starts from */
+int oracle_sweep(oracle_ctx *c, int d, double dt) {
+    if (!c || d < 0 || d > 2 || !(dt > 0.0)) return 1;
+    if (c->flat3d) oracle_flatten3d_update(c);
+    return sweep_impl(c, d, dt);
+}
+
 /* C2: sweep_order 0..5 = xyz, xzy, yxz, yzx, zxy, zyx; one dt for the three sweeps. */
 static const int ORDERS[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
 int oracle_step(oracle_ctx *c, double dt, int sweep_order) {
     if (!c || !(dt > 0.0) || sweep_order < 0 || sweep_order > 5) return 1;
+    if (c->flat3d) oracle_flatten3d_update(c);      /* once per step, on the step's starting state */
     for (int s = 0; s < 3; ++s) {
-        int rc = oracle_sweep(c, ORDERS[sweep_order][s], dt);
+        int rc = sweep_impl(c, ORDERS[sweep_order][s], dt);
         if (rc) return rc;
     }
     return 0;
