@@ -111,11 +111,20 @@ int ppm_sync(ppm_ctx *ctx);
  * split into another chunk (0 = library default).  Results do not depend on it. */
 int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
 
-/* Options (results do not depend on them).
+/* Options.  Tuning option (results do not depend on it):
  *  PPM_OPT_IO_PATH : 0 = automatic: a sweep along an axis whose extent is a multiple of 4 stages whole brick
  *                    records through shared memory with bulk copies (cp.async.bulk), any other axis uses the
- *                    direct global-memory path; 1 = direct path for every axis. */
-enum { PPM_OPT_IO_PATH = 2 };
+ *                    direct global-memory path; 1 = direct path for every axis.
+ *
+ * Option that changes the numerical scheme ("a fully 3-D treatment of the
+ * shock dissipation"; reading R5b in DESIGN.md):
+ *  PPM_OPT_FLATTEN3D : 0 (default) = the flattening coefficient of a sweep comes from the 1-D shock detector
+ *                    along that sweep (H4); 1 = it comes from a 3-D detector field F~ = max over the three
+ *                    directions of the H4 coefficient, evaluated once per ppm_step on the step's starting state
+ *                    (ppm_sweep: on the state that sweep starts from) and spread over i-1..i+1 along the sweep.
+ *                    Setting it allocates one library-owned device array of ppm_state_floats()/15 floats
+ *                    (PPM_ENOMEM if that fails) and adds one light kernel launch per step. */
+enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* 1 if the next sweep along axis (0,1,2) will take the bulk-staged path, 0 if the direct path. */
 int ppm_axis_path(const ppm_ctx *ctx, int axis);

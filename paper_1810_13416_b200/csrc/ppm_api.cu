@@ -112,7 +112,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
 extern "C" void ppm_destroy(ppm_ctx* c) {
     if (!c) return;
     cudaFree(c->flag); cudaFree(c->cflmax); cudaFree(c->partial); cudaFree(c->result);
-    cudaFree(c->tab); cudaFree(c->tab64);
+    cudaFree(c->tab); cudaFree(c->tab64); cudaFree(c->F3);
     free(c);
 }
 
@@ -163,6 +163,7 @@ extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z
 extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
     if (!c) { set_err(nullptr, "ppm_sweep: ctx is NULL"); return PPM_EINVAL; }
     if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "ppm_sweep: need finite dt > 0 and axis in 0..2"); return PPM_EINVAL; }
+    if (c->flat3d) CU(ppm_launch_flatten3d(c));     // the detector field of the state this sweep starts from
     CU(ppm_launch_sweep(c, axis, dt));
     return PPM_OK;
 }
@@ -170,6 +171,7 @@ extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
 extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
     if (!c) { set_err(nullptr, "ppm_step: ctx is NULL"); return PPM_EINVAL; }
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_step: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
+    if (c->flat3d) CU(ppm_launch_flatten3d(c));     // once per step, on the step's starting state
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt));
     return PPM_OK;
 }
@@ -212,6 +214,15 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
+    if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
+        if (value && !c->F3) {
+            const size_t n = (size_t)c->nbx * c->nby * c->nbz * 64;
+            cudaError_t e = cudaMalloc(&c->F3, n * sizeof(float));
+            if (e != cudaSuccess) { c->F3 = nullptr; cudaGetLastError(); set_err(c, "ppm_set_option: cannot allocate the %zu-byte detector field", n * sizeof(float)); return PPM_ENOMEM; }
+        }
+        c->flat3d = value;
+        return PPM_OK;
+    }
     set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
     return PPM_EINVAL;
 }

@@ -12,11 +12,14 @@ struct AuxParams {
     double s0, ds, cx, cy, cz;
     const double* __restrict__ tab64;   // node k: g, rho0, p0 (3 doubles)
     int nbx, nby;                       // bricks along x, y
+    int bc[6];
+    const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
+    float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
 };
 
 // float offset of field 0 of cell (i,j,k): brick record [bz][by][bx][15][4z][4y][4x]; field f is 64*f further
 __device__ __forceinline__ long long cell_offset(const AuxParams& A, int i, int j, int k) {
-    return (((long long)(k >> 2) * A.nby + (j >> 2)) * A.nbx + (i >> 2)) * PPM_BRICK_FLOATS + ((k & 3) << 4 | (j & 3) << 2 | (i & 3));
+    return (long long)(((k >> 2) * A.nby + (j >> 2)) * A.nbx + (i >> 2)) * PPM_BRICK_FLOATS + ((k & 3) << 4 | (j & 3) << 2 | (i & 3));   // (brick index < 2^25: ppm_create caps the cells at 2^31)
 }
 // storage slot t (brick * 64 + cell in brick) -> (i,j,k) and the offset of field 0; false for a pad cell
 __device__ __forceinline__ bool cell_of(const AuxParams& A, long long t, int& i, int& j, int& k, long long& off) {
@@ -160,6 +163,118 @@ __global__ void conserved_final_kernel(const double* __restrict__ partial, int n
     }
 }
 
+
+// ---- NEXT-1 ("a fully 3-D treatment of the shock dissipation"): the 3-D shock detector
+// F~_i = max over the three directions d of the H4 coefficient f~^d_i = steep * jump * conv, each evaluated along d
+// (full p at i-2..i+2, u_d at i-1, i+1, c_i) on the state the step starts from; ghost cells by the boundary images
+// (periodic wrap / mirror with the normal velocity negated).  One value per cell, [brick][4z][4y][4x].
+// fp32 base state (rho0, p0) at a cell centre, as the sweeps evaluate it
+__device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k) {
+    if (A.grav_kind == PPM_GRAV_CONST_Z) {
+        const float4 v = __ldg(A.tab32 + 2 * k + 2 * PPM_NGHOST + 1);
+        return make_float2(v.x, v.y);
+    }
+    if (A.grav_kind == PPM_GRAV_RADIAL) {
+        const float dx = A.dxf;
+        const float x = ((float)i + 0.5f) * dx - A.cxf, y = ((float)j + 0.5f) * dx - A.cyf, z = ((float)k + 0.5f) * dx - A.czf;
+        const float r2 = fmaf(x, x, fmaf(y, y, z * z));
+        const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
+        const float t = (r - A.s0f) * A.inv_dsf;
+        int kk = (int)floorf(t);
+        kk = min(max(kk, 0), A.tab_n - 2);
+        const float w = t - (float)kk;
+        const float4 a = __ldg(A.tab32 + kk), b = __ldg(A.tab32 + kk + 1);
+        return make_float2(fmaf(w, b.x - a.x, a.x), fmaf(w, b.y - a.y, a.y));
+    }
+    return make_float2(0.f, 0.f);
+}
+
+__device__ __forceinline__ int aux_image(int i, int n, int bc_lo, int bc_hi, float& sgn) {
+    sgn = 1.0f;
+    if ((unsigned)i < (unsigned)n) return i;
+    const int bcx = (i < 0) ? bc_lo : bc_hi;
+    if (bcx == PPM_BC_PERIODIC) return ((i % n) + n) % n;
+    sgn = -1.0f;
+    const int s = (i < 0) ? (-1 - i) : (2 * n - 1 - i);
+    return min(max(s, 0), n - 1);
+}
+
+// CTA = a tile of 2x2x2 bricks (8x8x8 cells), one thread per cell.  Phase 1 puts the full pressure of the tile and of
+// its two-cell arms along the three axes (the detector needs no corners) and the velocity components into shared
+// memory: 2.5 base-state evaluations per cell instead of 13.  Phase 2 evaluates the three 1-D detectors from there.
+constexpr int F3_T = 8, F3_H = 2, F3_W = F3_T + 2 * F3_H, F3_N = F3_W * F3_W * F3_W;
+__device__ __forceinline__ int f3_idx(int lx, int ly, int lz) { return ((lz + F3_H) * F3_W + (ly + F3_H)) * F3_W + (lx + F3_H); }
+
+__global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const float* __restrict__ st, float* __restrict__ F3) {
+    __shared__ float sP[F3_N], sU[3][F3_N];
+    const int tid = threadIdx.x;
+    const int org[3] = {(int)blockIdx.x * F3_T, (int)blockIdx.y * F3_T, (int)blockIdx.z * F3_T};
+    const float gam = A.gamf;
+    float rc = 1.f;
+    for (int idx = tid; idx < 512 + 6 * 2 * 64; idx += 512) {
+        int lx, ly, lz, d = -1;                // (scalars and selects only: a dynamically indexed l[3] would live in local memory)
+        if (idx < 512) {                       // the tile itself: thread = (brick in tile, cell in brick) -> coalesced brick reads
+            const int b = idx >> 6, c = idx & 63;
+            lx = (b & 1) * 4 + (c & 3); ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3); lz = (b >> 2) * 4 + (c >> 4);
+        } else {                               // the arms: axis d, side, depth h, position (a, bb) on the face
+            const int r = idx - 512, f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
+            d = f >> 1;
+            const int along = (f & 1) ? F3_T + h : -1 - h;
+            lx = (d == 0) ? along : (d == 1 ? bb : a);
+            ly = (d == 1) ? along : (d == 2 ? bb : a);
+            lz = (d == 2) ? along : (d == 0 ? bb : a);
+        }
+        int gx = org[0] + lx, gy = org[1] + ly, gz = org[2] + lz;
+        // A point outside the grid along ONE axis is the boundary image of a cell along that axis (an arm point
+        // by construction, a tile point when the tile overhangs a ragged grid); outside along two axes it is
+        // never anybody's neighbour.
+        const bool ox = (unsigned)gx >= (unsigned)A.nx, oy = (unsigned)gy >= (unsigned)A.ny, oz = (unsigned)gz >= (unsigned)A.nz;
+        const int nout = (int)ox + (int)oy + (int)oz;
+        const int dout = ox ? 0 : (oy ? 1 : (oz ? 2 : d));
+        const int si = f3_idx(lx, ly, lz);
+        if (nout > 1 || (d >= 0 && nout == 1 && dout != d)) {
+            sP[si] = 1.f;
+            sU[0][si] = sU[1][si] = sU[2][si] = 0.f;
+            continue;
+        }
+        float sgn = 1.f;
+        if (ox) gx = aux_image(gx, A.nx, A.bc[0], A.bc[1], sgn);
+        if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
+        if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
+        const long long o = cell_offset(A, gx, gy, gz);
+        const float2 b0 = base32(A, gx, gy, gz);
+        sP[si] = b0.y + st[o + 4 * 64];
+        if (d < 0) {
+            rc = b0.x + st[o];
+            const float ux = st[o + 64], uy = st[o + 2 * 64], uz = st[o + 3 * 64];
+            sU[0][si] = ox ? sgn * ux : ux; sU[1][si] = oy ? sgn * uy : uy; sU[2][si] = oz ? sgn * uz : uz;
+        } else {
+            const float u = st[o + (1 + d) * 64];
+            if (d == 0) sU[0][si] = sgn * u; else if (d == 1) sU[1][si] = sgn * u; else sU[2][si] = sgn * u;
+        }
+    }
+    __syncthreads();
+    const int b = tid >> 6, c = tid & 63;
+    const int lx = (b & 1) * 4 + (c & 3), ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3), lz = (b >> 2) * 4 + (c >> 4);
+    const int g[3] = {org[0] + lx, org[1] + ly, org[2] + lz};
+    if (g[0] >= A.nx || g[1] >= A.ny || g[2] >= A.nz) return;
+    const int s0 = f3_idx(lx, ly, lz);
+    const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
+    float F = 0.f;
+    const int stride[3] = {1, F3_W, F3_W * F3_W};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int sd = stride[d];
+        const float d1 = sP[s0 + sd] - sP[s0 - sd], d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
+        const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
+        const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), fminf(sP[s0 + sd], sP[s0 - sd])) - 1.0f);
+        const float conv = __saturatef((sU[d][s0 - sd] - sU[d][s0 + sd]) * ics);
+        F = fmaxf(F, steep * jump * conv);
+    }
+    const long long brick = ((long long)(g[2] >> 2) * A.nby + (g[1] >> 2)) * A.nbx + (g[0] >> 2);
+    F3[brick * 64 + c] = F;
+}
+
 AuxParams make_aux(const ppm_ctx* c) {
     AuxParams A;
     const ppm_params& p = c->prm;
@@ -171,6 +286,10 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.cx = p.grav.center[0]; A.cy = p.grav.center[1]; A.cz = p.grav.center[2];
     A.tab64 = c->tab64;
     A.nbx = c->nbx; A.nby = c->nby;
+    for (int k = 0; k < 6; ++k) A.bc[k] = p.bc[k];
+    A.tab32 = c->tab;
+    A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
+    A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
     return A;
 }
 
@@ -193,6 +312,13 @@ cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, floa
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs) {
     const long long tot = (long long)c->prm.nx * c->prm.ny * nzs;
     to_full_kernel<<<grid_for(tot, 148 * 16), 256, 0, c->stream>>>(make_aux(c), state, dst, z0, nzs);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t ppm_launch_flatten3d(ppm_ctx* c) {
+    const dim3 grid((c->nbx + 1) / 2, (c->nby + 1) / 2, (c->nbz + 1) / 2);
+    flatten3d_kernel<<<grid, 512, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->F3);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -38,6 +38,9 @@ struct SweepParams {
     float cen_d, cen_a, cen_b;      // RADIAL centre along (sweep, a, b) axes
     const float4* __restrict__ tab; // node k: {rho0, p0, g, 0}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
+    // 3-D flattening mode: F~ of every cell, [brick][4z][4y][4x] (a brick is 64 floats: strides = SB / 15); else NULL
+    const float* flat;
+    long long FBd, FBa, FBb;
 };
 
 struct ppm_ctx {
@@ -54,6 +57,8 @@ struct ppm_ctx {
     int nblocks_red;
     int chunk;
     int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
+    int flat3d;                     // PPM_OPT_FLATTEN3D
+    float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
     int sms;                        // multiprocessors of the device
     int io_path;                    // PPM_OPT_IO_PATH: 0 = bulk-staged where the sweep-axis extent is whole bricks, 1 = direct everywhere
     long long launches;
@@ -66,4 +71,5 @@ bool ppm_axis_is_bulk(const ppm_ctx* c, int axis);
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs);
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs);
 cudaError_t ppm_launch_cfl(ppm_ctx* c);
+cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_conserved(ppm_ctx* c);

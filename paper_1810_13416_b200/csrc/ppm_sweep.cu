@@ -305,9 +305,11 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float rm, float
 // The marching body, shared by every data path.  IO supplies plane n (hydro), cell n-3 (PPB coefficients,
 // local family order, mirror signs applied) and takes the finished cell n-4.
 // =====================================================================================================
-template <int DIR, int GRAV, class IO>
+// FLAT: 3-D flattening mode — the un-spread coefficient of cell n-2 is read from the detector field
+// (pflat = the pencil's cell 0 in it) instead of being computed from the pencil's own pressures and velocities.
+template <int DIR, int GRAV, bool FLAT, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
-                                      const bool valid, const unsigned wmask) {
+                                      const bool valid, const unsigned wmask, const float* __restrict__ pflat) {
     const float gam = P.gamma, gp = 0.5f * (gam + 1.0f), gmg = 0.5f * (gam - 1.0f) * rcp(gam), g_gm1 = gam * rcp(gam - 1.0f);
     const float dtdx = P.dtdx, hdt = 0.5f * P.dt;
 
@@ -331,6 +333,12 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 #pragma unroll
     for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
 
+    float fpre = 0.f;
+    if (FLAT) {
+        float sg;
+        const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
+        fpre = __ldg(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+    }
 #pragma unroll MARCH_UNROLL
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
         io.begin(n);
@@ -353,7 +361,12 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         // ---- E, F: flattening ---------------------------------------------------------------------------
         const float cn2 = fsqrt(gam * pf[2] * rcp(rf[3]));          // c_{n-2}
         float ftn;
-        {
+        if (FLAT) {
+            ftn = fpre;                                              // F~_{n-2}, in flight since the last iteration
+            float sg;
+            const int jf = image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (the detector is mirror-invariant)
+            fpre = __ldg(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+        } else {
             const float d1 = pf[3] - pf[1], dd2 = pf[4] - pf[0];
             const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
             const float jump = sat(fdiv(3.0f * fabsf(d1), fminf(pf[3], pf[1])) - 1.0f);
@@ -633,7 +646,7 @@ struct IoDirect {
 
 // thread -> pencil: 16 lanes = the 4x4 transverse cells of one brick column; a CTA of 128 threads = 8 brick
 // columns adjacent along a.  (a, b) = the two transverse axes in increasing axis order.
-template <int DIR, int GRAV>
+template <int DIR, int GRAV, bool FLAT>
 __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
     const int t = threadIdx.x;
@@ -645,7 +658,8 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     const int c1 = min(c0 + P.chunk, P.n);
     const long long tb = (long long)ba * P.SBa + (long long)bb * P.SBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)));
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
-    march<DIR, GRAV>(P, io, a, b, c0, c1, true, wmask);
+    const float* pflat = FLAT ? P.flat + ((long long)ba * P.FBa + (long long)bb * P.FBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)))) : nullptr;
+    march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, true, wmask, pflat);
 }
 
 // ---- shared-memory / mbarrier / bulk-copy primitives ----------------------------------------------------
@@ -868,7 +882,7 @@ struct IoBulk {
 // whole pencils while they fill complete waves of resident CTAs and cuts the pencils of the ragged last wave into
 // shorter segments, so that the SMs run dry together.  A cut costs 8 redundant warm-up cells; results do not
 // depend on where the cuts are.
-template <int DIR, int GRAV>
+template <int DIR, int GRAV, bool FLAT>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -900,7 +914,9 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
     IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
-    march<DIR, GRAV>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu);
+    const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
+                                          (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
+    march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu, pflat);
 }
 
 // cells per segment for the tiles of the ragged last wave: the cut that minimises (waves of segments) x (segment
@@ -919,14 +935,14 @@ static int tail_chunk(int ntail, int slots, int n) {
     return best;
 }
 
-template <int DIR, int GRAV>
+template <int DIR, int GRAV, bool FLAT>
 cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
     using G = BulkGeom<DIR>;
     static int occ = 0;
     if (!occ) {
-        cudaError_t e = cudaFuncSetAttribute(ppm_sweep_bulk_kernel<DIR, GRAV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ppm_sweep_bulk_kernel<DIR, GRAV>, G::WARPS * 32, G::SMEM);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, G::WARPS * 32, G::SMEM);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
     }
@@ -940,24 +956,32 @@ cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st
         P.chunk_b = (P.tiles_a < ntiles) ? tail_chunk(ntiles - P.tiles_a, slots, P.n) : P.n;
     }
     const long long grid = (long long)P.tiles_a * ((P.n + P.chunk - 1) / P.chunk) + (long long)(ntiles - P.tiles_a) * ((P.n + P.chunk_b - 1) / P.chunk_b);
-    ppm_sweep_bulk_kernel<DIR, GRAV><<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
+    ppm_sweep_bulk_kernel<DIR, GRAV, FLAT><<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
     return cudaGetLastError();
 }
 template <int DIR>
 cudaError_t launch_bulk_dir(SweepParams& P, int grav, int sms, int user_chunk, cudaStream_t st) {
+    const bool fl = P.flat != nullptr;
     switch (grav) {
-        case PPM_GRAV_NONE: return launch_bulk<DIR, PPM_GRAV_NONE>(P, sms, user_chunk, st);
-        case PPM_GRAV_CONST_Z: return launch_bulk<DIR, PPM_GRAV_CONST_Z>(P, sms, user_chunk, st);
-        default: return launch_bulk<DIR, PPM_GRAV_RADIAL>(P, sms, user_chunk, st);
+        case PPM_GRAV_NONE: return fl ? launch_bulk<DIR, PPM_GRAV_NONE, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_NONE, false>(P, sms, user_chunk, st);
+        case PPM_GRAV_CONST_Z: return fl ? launch_bulk<DIR, PPM_GRAV_CONST_Z, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_CONST_Z, false>(P, sms, user_chunk, st);
+        default: return fl ? launch_bulk<DIR, PPM_GRAV_RADIAL, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_RADIAL, false>(P, sms, user_chunk, st);
     }
 }
 
 template <int DIR>
 cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cudaStream_t st) {
+    const bool fl = P.flat != nullptr;
     switch (grav) {
-        case PPM_GRAV_NONE: ppm_sweep_kernel<DIR, PPM_GRAV_NONE><<<grid, block, 0, st>>>(P); break;
-        case PPM_GRAV_CONST_Z: ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z><<<grid, block, 0, st>>>(P); break;
-        default: ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL><<<grid, block, 0, st>>>(P); break;
+        case PPM_GRAV_NONE:
+            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_NONE, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_NONE, false><<<grid, block, 0, st>>>(P);
+            break;
+        case PPM_GRAV_CONST_Z:
+            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, false><<<grid, block, 0, st>>>(P);
+            break;
+        default:
+            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, false><<<grid, block, 0, st>>>(P);
+            break;
     }
     return cudaGetLastError();
 }
@@ -994,6 +1018,8 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
     P.tab = c->tab;
     P.flag = c->flag;
+    P.flat = c->flat3d ? c->F3 : nullptr;
+    P.FBd = P.SBd / PPM_NFIELDS; P.FBa = P.SBa / PPM_NFIELDS; P.FBb = P.SBb / PPM_NFIELDS;
     const int nchunks = (P.n + chunk - 1) / chunk;
     const int nba = (P.na + 3) / 4, nbb = (P.nb + 3) / 4;
     cudaError_t e;

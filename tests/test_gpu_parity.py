@@ -39,15 +39,21 @@ def _load(g, w, device="cuda", nzs=32):
         g.set_state(w.fields((0, 0, z0), (n, n, z1), device=device), z0=z0)
 
 
-def _run_pair(w, steps, chunk=0, check_each=()):
+def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False):
     """steps on both sides with the GPU's dt; returns dict of results after step 1 and at the end."""
     PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_FLATTEN3D, OPT_IO_PATH
     f = w.fields()
     o = _oracle(w)
     o.set_state(f.numpy())
     g = PPM.from_workload(w)
     if chunk:
         g.set_chunk(chunk)
+    if flat3d:                      # SURVEY 8(f) NEXT-1 on both sides
+        g.set_option(OPT_FLATTEN3D, 1)
+        o.set_flatten3d(True)
+    if direct:
+        g.set_option(OPT_IO_PATH, 1)
     g.set_state(f.cuda())
     out = {}
     c0g, c0o = g.reduce_conserved(), o.reduce_conserved()
@@ -142,6 +148,77 @@ def test_cfg3_blast_reduced_64_50_steps_L1():
     gs, os_ = r["final"]
     assert np.abs(os_[1:4]).max() > 3.0           # the Mach ~3 blast really ran
     assert gs[5].min() >= 0.0 and gs[5].max() <= 1.0
+
+
+# ---------------------------------------------------------------- NEXT-1: fully 3-D shock flattening --
+@pytest.mark.parametrize("direct", [False, True])
+def test_flatten3d_blast_matches_oracle(direct):
+    """config 3 (Mach ~3 blast through a 1000:1 density jump) in the 3-D flattening mode, both data
+    paths: the detector kernel + the sweeps that read its field against the oracle's 3-D mode."""
+    w = W.make(3, n=48)
+    r = _run_pair(w, 40, flat3d=True, direct=direct)
+    assert max(r[1][1].values()) <= L1_SHOCK, r[1][1]
+    assert max(r[40][1].values()) <= L1_SHOCK, r[40][1]
+    assert r["cons1"].max() <= CONS
+    # the mode really differs from the 1-D one on this flow (else the test would prove nothing)
+    r1 = _run_pair(w, 40)
+    d = l1_rel(r["final"][0], r1["final"][0])
+    assert max(d.values()) > 20 * L1_SHOCK, d
+
+
+def test_flatten3d_smooth_flow_equals_1d_mode_bitwise():
+    """no shock anywhere (config 1): F~ = 0 and the 3-D mode must reproduce the 1-D mode bit for bit"""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_FLATTEN3D
+    w = W.make(1)
+    f = w.fields().cuda()
+    res = []
+    for mode in (0, 1):
+        g = PPM.from_workload(w)
+        g.set_option(OPT_FLATTEN3D, mode)
+        g.set_state(f)
+        for s in range(3):
+            g.step(g.cfl_dt(0.8), s * 2)
+        res.append(g.get_state().cpu().numpy())
+        assert g.launch_count() == (3 * (3 + mode) + 3 + 2)       # per step: 3 sweeps (+ 1 detector), 3 cfl, set + get
+        g.close()
+    assert np.array_equal(res[0], res[1])
+
+
+def test_flatten3d_ragged_grid_and_paths_agree():
+    PPM = _gpu()
+    from oracle import binding as ob
+    from paper_1810_13416_b200.binding import OPT_FLATTEN3D, OPT_IO_PATH
+    rng = np.random.default_rng(12)
+    nx, ny, nz = 36, 30, 22
+    f = np.zeros((15, nz, ny, nx), dtype=np.float32)
+    f[0] = 1.0 + rng.random((nz, ny, nx))
+    f[1:4] = 0.25 * rng.normal(size=(3, nz, ny, nx))
+    f[4] = np.exp(0.6 * rng.normal(size=(nz, ny, nx)))        # pressure jumps: the detector is on in many cells
+    f[5] = 0.2 + 0.6 * rng.random((nz, ny, nx))
+    bc = (1, 1, 0, 0, 1, 1)
+    o = ob.Oracle(nx, ny, nz, 0.03, 1.4, bc, None)
+    o.set_flatten3d(True)
+    o.set_state(f)
+    assert (o.flatten3d_field() > 0.5).mean() > 0.02
+    res = []
+    for io in (0, 1):
+        g = PPM(nx, ny, nz, 0.03, 1.4, bc)
+        g.set_option(OPT_FLATTEN3D, 1)
+        g.set_option(OPT_IO_PATH, io)
+        g.set_state(f)
+        dts = []
+        for order in (0, 3, 5):
+            dt = 0.4 * g.cfl_dt(0.8)
+            dts.append(dt)
+            g.step(dt, order)
+        res.append(g.get_state().cpu().numpy().astype(np.float64))
+        g.close()
+    assert np.array_equal(res[0], res[1])
+    for dt, order in zip(dts, (0, 3, 5)):
+        o.step(dt, order)
+    e = l1_rel(res[0], o.get_state())
+    assert max(e.values()) <= L1_SHOCK, e
 
 
 def test_cfg4_convection_reduced_64_20_steps():
