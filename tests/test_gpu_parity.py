@@ -259,6 +259,36 @@ def test_ragged_grid_all_boundaries_and_orders(dims):
         g.close()
 
 
+@pytest.mark.parametrize("dims", [(16, 8, 1), (12, 1, 1), (1, 1, 9), (5, 3, 2), (8, 4, 4)])
+def test_degenerate_grids_2d_1d_and_fewer_cells_than_ghosts(dims):
+    """quasi-2-D and 1-D grids (one brick thick, mostly pad cells) and periodic axes with fewer cells than the 4
+    ghost cells a sweep reaches (the images wrap around more than once)."""
+    PPM = _gpu()
+    from oracle import binding as ob
+    rng = np.random.default_rng(21)
+    nx, ny, nz = dims
+    f = np.zeros((15, nz, ny, nx), dtype=np.float32)
+    f[0] = 1.0 + 0.3 * rng.random((nz, ny, nx))
+    f[1:4] = 0.2 * rng.normal(size=(3, nz, ny, nx))
+    f[4] = 0.8 + 0.3 * rng.random((nz, ny, nx))
+    f[5] = 0.2 + 0.6 * rng.random((nz, ny, nx))
+    f[6:] = 0.02 * rng.normal(size=(9, nz, ny, nx))
+    bc = (0,) * 6
+    o = ob.Oracle(nx, ny, nz, 0.05, 1.4, bc, None)
+    g = PPM(nx, ny, nz, 0.05, 1.4, bc)
+    o.set_state(f)
+    g.set_state(f)
+    for order in (0, 5, 2):
+        dt = 0.5 * g.cfl_dt(0.8)
+        g.step(dt, order)
+        o.step(dt, order)
+    e = max_rel(g.get_state().cpu().numpy().astype(np.float64), o.get_state())
+    assert max(e.values()) <= MULTI_STEP, e
+    c = g.reduce_conserved()
+    assert np.all(np.isfinite(c))
+    g.close()
+
+
 def test_hydrostatic_state_is_preserved_exactly_on_gpu():
     PPM = _gpu()
     for cfg, n in ((2, 32), (4, 32)):
