@@ -37,6 +37,8 @@ def lib():
         L.oracle_raw_field.argtypes = [C.c_void_p, C.c_int]
         L.oracle_sweep.argtypes = [C.c_void_p, C.c_int, C.c_double]
         L.oracle_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.oracle_advect.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.oracle_advect_pencil.argtypes = [C.c_int, C.c_int, C.c_double, C.c_double, dp, C.POINTER(dp), C.POINTER(dp)]
         L.oracle_set_flatten3d.argtypes = [C.c_void_p, C.c_int]
         L.oracle_flatten3d_update.argtypes = [C.c_void_p]
         L.oracle_flatten3d_field.argtypes = [C.c_void_p]
@@ -163,6 +165,18 @@ def sweep_pencil(d, dx, dt, gamma, q5, m10, rho0c=None, p0c=None, gd=None, rho0f
     return qo, mo
 
 
+def advect_pencil(d, dx, dt, u, m10):
+    """u: (n+8,) normal velocity with ghosts; m10: (10, n+8).  Returns (10, n)."""
+    u, m10 = _arr(u), _arr(m10)
+    n = u.size - 8
+    mo = np.zeros((10, n))
+    dp = C.POINTER(C.c_double)
+    mi = (dp * 10)(*[_d(m10[k]) for k in range(10)])
+    mop = (dp * 10)(*[_d(mo[k]) for k in range(10)])
+    lib().oracle_advect_pencil(n, d, dx, dt, _d(u), mi, mop)
+    return mo
+
+
 def num_threads():
     return lib().oracle_num_threads()
 
@@ -242,6 +256,12 @@ class Oracle:
     def sweep(self, d, dt):
         rc = lib().oracle_sweep(self._h, d, dt)
         assert rc == 0
+
+    def advect(self, dt, order=0):
+        """NEXT-2: PPB-only step (FV advected by the stored velocity field, hydro state held fixed)"""
+        rc = lib().oracle_advect(self._h, dt, order)
+        if rc:
+            raise ValueError("oracle_advect rc=%d" % rc)
 
     def step(self, dt, order=0):
         rc = lib().oracle_step(self._h, dt, order)

@@ -447,6 +447,46 @@ void oracle_sweep_pencil(int n, int d, double dx, double dt, double gamma, doubl
     free(buf);
 }
 
+/* NEXT-2 (Fig. 3: "a velocity field is applied ... this is linear advection").
+ * PPB-only sweep of one pencil: the hydro state is held fixed and FV is advected by the stored velocity field.
+ * [reading R22, DESIGN.md]  The gas is taken as uniform (rho = 1: M_i = dx), the velocity at face i+1/2 is the mean
+ * of the two cell values, u_f = (u_i + u_{i+1})/2 (exact for the solid-body rotation of Fig. 3, where the
+ * component along a sweep does not vary along it), the mass through the face is dM = dt u_f, and P2-P4 are used
+ * unchanged.  u: normal velocity with ghosts (nt = n + 8, odd image sign applied); m: 10 coefficients with ghosts. */
+void oracle_advect_pencil(int n, int d, double dx, double dt, const double *u, const double *const m[10],
+                          double *const mn[10]) {
+    const int nt = n + 2 * NG;
+    double *dM = (double *)calloc((size_t)2 * nt + 2, sizeof(double));
+    double *theta = dM + nt + 1;
+    for (int f = NG; f <= nt - NG; ++f) dM[f] = dt * 0.5 * (u[f - 1] + u[f]);
+    for (int j = 3; j <= nt - 4; ++j) {
+        double mm[10];
+        for (int k = 0; k < 10; ++k) mm[k] = m[k][j];
+        theta[j] = oracle_p2_theta(mm);
+    }
+    for (int j = NG; j < nt - NG; ++j) {
+        const int i = j - NG;
+        double M[3] = {dx, dx, dx};
+        for (int f = 0; f < 6; ++f) {
+            const int deg = PPB_FAM[d][f][0];
+            double a[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, out[3];
+            for (int s = 0; s < 3; ++s)
+                for (int nn = 0; nn <= deg; ++nn) {
+                    int idx = PPB_FAM[d][f][1 + nn];
+                    double v = m[idx][j - 1 + s];
+                    if (idx != 0) v *= theta[j - 1 + s];
+                    a[s][nn] = v;
+                }
+            int ok = oracle_p4_remap(deg, a, M, dM[j], dM[j + 1], out);
+            for (int nn = 0; nn <= deg; ++nn) {
+                int idx = PPB_FAM[d][f][1 + nn];
+                mn[idx][i] = ok ? out[nn] : m[idx][j];
+            }
+        }
+    }
+    free(dM);
+}
+
 /* ------------------------------------------------------------------------------------------
  * 3-D driver
  * ---------------------------------------------------------------------------------------- */
@@ -651,6 +691,53 @@ int oracle_step(oracle_ctx *c, double dt, int sweep_order) {
     if (c->flat3d) oracle_flatten3d_update(c);      /* once per step, on the step's starting state */
     for (int s = 0; s < 3; ++s) {
         int rc = sweep_impl(c, ORDERS[sweep_order][s], dt);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+/* NEXT-2: PPB-only sweep along d over every pencil; the five hydro fields are not touched. */
+static int advect_sweep(oracle_ctx *c, int d, double dt) {
+    const int n = c->n[d];
+    const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;
+    const int n1 = c->n[d1], n2 = c->n[d2];
+    const int nt = n + 2 * NG;
+    int fail = 0;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int b = 0; b < n2; ++b)
+        for (int a = 0; a < n1; ++a) {
+            double *buf = (double *)malloc(sizeof(double) * ((size_t)nt * 11 + (size_t)n * 10));
+            if (!buf) { fail = 1; continue; }
+            double *ua = buf, *ma[10], *mo[10], *cur = buf + nt;
+            for (int k = 0; k < 10; ++k) { ma[k] = cur; cur += nt; }
+            for (int k = 0; k < 10; ++k) { mo[k] = cur; cur += n; }
+            int ijk[3];
+            ijk[d1] = a; ijk[d2] = b;
+            for (int j = 0; j < nt; ++j) {
+                int sgn, gpos;
+                ijk[d] = image_cell(c, d, j - NG, &sgn, &gpos);
+                size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                ua[j] = sgn * c->q[1 + d][id];
+                for (int k = 0; k < 10; ++k) ma[k][j] = (ppb_is_odd(d, k) ? sgn : 1) * c->q[5 + k][id];
+            }
+            oracle_advect_pencil(n, d, c->dx, dt, ua, (const double *const *)ma, mo);
+            for (int i = 0; i < n; ++i) {
+                ijk[d] = i;
+                size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                for (int k = 0; k < 10; ++k) c->qn[5 + k][id] = mo[k][i];
+            }
+            free(buf);
+        }
+    if (fail) return 2;
+    for (int f = 5; f < NF; ++f) { double *t = c->q[f]; c->q[f] = c->qn[f]; c->qn[f] = t; }
+    return 0;
+}
+
+/* NEXT-2: one PPB-only step = three PPB-only sweeps in the given order with one dt. */
+int oracle_advect(oracle_ctx *c, double dt, int sweep_order) {
+    if (!c || !(dt > 0.0) || sweep_order < 0 || sweep_order > 5) return 1;
+    for (int s = 0; s < 3; ++s) {
+        int rc = advect_sweep(c, ORDERS[sweep_order][s], dt);
         if (rc) return rc;
     }
     return 0;

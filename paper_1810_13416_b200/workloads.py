@@ -298,3 +298,49 @@ def make(cfg: int, n: int | None = None, steps: int | None = None) -> Workload:
         w._p["vel_modes"] = [_modes(rng, 32, 8) for _ in range(3)]
         return w
     raise ValueError("cfg must be 1..5")
+
+
+# ---- NEXT-2: the slotted-disc rotation problem of PAPER.md Fig. 3 / L43 -----------------------------
+def slotted_disc(n: int = 100, sub: int = 16, nz: int = 1, revolutions_per_unit_time: float = 1.0):
+    """Zalesak's slotted disc in solid-body rotation about the centre of the unit square, as PAPER.md L43 describes it:
+    2-D, n x n cells (the paper: 100 x 100), the fractional volume 1 inside the slotted circle and 0 outside, "the
+    fractional volumes and higher moments ... computed exactly for a shape with boundaries of zero thickness" — here
+    by sub x sub midpoint sub-sampling of the indicator function in every cell (an input recipe, not the method).
+    The disc (standard proportions): centre (0.5, 0.75), radius 0.15, slot of width 0.05 cut from below up to y = 0.85.
+    Returns fields [15, nz, n, n] float32: rho = 1, p = 1, (u, v) = Omega x (r - centre), w = 0, and the in-plane
+    Legendre coefficients of FV (m000, m100, m010, m200, m020, m110; the z ones are zero).  dx = 1/n."""
+    dx = 1.0 / n
+    om = 2.0 * math.pi * revolutions_per_unit_time
+    c = (np.arange(n) + 0.5) * dx
+    s = (np.arange(sub) + 0.5) / sub - 0.5                     # sub-cell midpoints in cell units
+    xs = (c[:, None] + s[None, :] * dx).reshape(-1)            # n*sub sample coordinates
+    X, Y = np.meshgrid(xs, xs, indexing="xy")                  # [y, x]
+    inside = ((X - 0.5) ** 2 + (Y - 0.75) ** 2 <= 0.15 ** 2) & ~((np.abs(X - 0.5) <= 0.025) & (Y <= 0.85))
+    ind = inside.astype(np.float64).reshape(n, sub, n, sub)    # [cell y, sub y, cell x, sub x]
+    P = [np.ones(sub), s, s * s - 1.0 / 12.0]
+    f = np.zeros((NF, nz, n, n), dtype=np.float32)
+    f[0] = 1.0
+    f[4] = 1.0
+    f[1] = (-om * (c - 0.5))[None, :, None]                    # u_x = -Omega (y - 1/2)
+    f[2] = (om * (c - 0.5))[None, None, :]                     # u_y = +Omega (x - 1/2)
+    for k, (a, b, cz) in enumerate(_ABC):
+        if cz != 0:
+            continue
+        mom = np.einsum("jqip,q,p->ji", ind, P[b], P[a]) / (sub * sub) / (_NORM[a] * _NORM[b])
+        f[5 + k] = mom[None, :, :]
+    return f
+
+
+def subcell_image(m6, sub: int = 4):
+    """The paper's display of Fig. 3: "each grid cell is represented by a 4 x 4 square of subcells in which the
+    fractional volume is computed using the 6 low-order moments".  m6: dict or array of the in-plane coefficients
+    (m000, m100, m010, m200, m020, m110), each [ny, nx]; returns [ny*sub, nx*sub] sub-cell AVERAGES of the polynomial."""
+    m000, m100, m010, m200, m020, m110 = m6
+    e = np.arange(sub + 1) / sub - 0.5
+    a1 = 0.5 * (e[1:] + e[:-1])                                            # average of P1 over a sub-interval
+    a2 = (e[1:] ** 3 - e[:-1] ** 3) / (3.0 * (e[1:] - e[:-1])) - 1.0 / 12.0  # average of P2
+    ny, nx = m000.shape
+    out = (m000[:, None, :, None] + m100[:, None, :, None] * a1[None, None, None, :] + m010[:, None, :, None] * a1[None, :, None, None]
+           + m200[:, None, :, None] * a2[None, None, None, :] + m020[:, None, :, None] * a2[None, :, None, None]
+           + m110[:, None, :, None] * a1[None, :, None, None] * a1[None, None, None, :])
+    return out.reshape(ny * sub, nx * sub)
