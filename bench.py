@@ -30,6 +30,7 @@ from paper_1810_13416_b200 import workloads as W  # noqa: E402
 METRIC = "cell-updates/s per 3-D PPM+PPB step (fp32); achieved HBM GB/s vs peak"
 UNIT = "cell-updates/s"
 BYTES_PER_CELL_SWEEP = 120.0      # 15 fp32 fields read + written by every sweep
+BYTES_PER_CELL_SWEEP_ADVECT = 84.0   # PPB-only sweep: 1 velocity + 10 coefficients read, 10 written (it moves 120: hydro copied through)
 FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, FMA = 2
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` capture
@@ -191,6 +192,7 @@ def run_gpu(args):
         g.set_option(OPT_FLATTEN3D, 1)
     _load_state(g, w, 8 if n >= 1024 else 32)
     dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
+    do_step = g.advect if args.advect else g.step
 
     def barrier():
         if ws > 1:
@@ -199,7 +201,7 @@ def run_gpu(args):
 
     K, Wm = args.steps, max(args.warmup, 3)
     for s in range(Wm):
-        g.step(dt, 0 if s % 2 == 0 else 5)
+        do_step(dt, 0 if s % 2 == 0 else 5)
     barrier()
     clk = _Clocks(lr)
     l0 = g.launch_count()
@@ -207,7 +209,7 @@ def run_gpu(args):
     barrier()
     e0.record(g.stream)
     for s in range(K):
-        g.step(dt, 0 if s % 2 == 0 else 5)
+        do_step(dt, 0 if s % 2 == 0 else 5)
     e1.record(g.stream)
     barrier()
     ms = e0.elapsed_time(e1)
@@ -223,12 +225,12 @@ def run_gpu(args):
             host_in = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
             host_out = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
             g.get_state(out=host_in)
-            g.set_state(host_in); g.step(dt, 0); g.get_state(out=host_out)      # warm-up
+            g.set_state(host_in); do_step(dt, 0); g.get_state(out=host_out)      # warm-up
             barrier()
             t0 = time.perf_counter()
             for s in range(Ke):
                 g.set_state(host_in)
-                g.step(dt, 0 if s % 2 == 0 else 5)
+                do_step(dt, 0 if s % 2 == 0 else 5)
                 g.get_state(out=host_out)       # synchronises
                 host_in, host_out = host_out, host_in
             torch.cuda.synchronize()
@@ -254,8 +256,9 @@ def run_gpu(args):
     # the dominant kernel = the 3 sweep launches of every step (in --flatten3d mode the light detector kernel's time
     # is charged to them: conservative)
     per_launch_s = ms * 1e-3 / (3 * K)
-    achieved = BYTES_PER_CELL_SWEEP * ncell / per_launch_s / 1e9
-    alu = FLOPS_PER_CELL_SWEEP * ncell / per_launch_s / 1e12
+    achieved = (BYTES_PER_CELL_SWEEP_ADVECT if args.advect else BYTES_PER_CELL_SWEEP) * ncell / per_launch_s / 1e9
+    flops_cs = 478.0 if args.advect else FLOPS_PER_CELL_SWEEP     # PPB-only: P2 13 + P1/P3/P4 460 + face masses 5
+    alu = flops_cs * ncell / per_launch_s / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": Wm,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -263,12 +266,13 @@ def run_gpu(args):
         "config": {"workload": "%s %d^3, %s, dt fixed at 0.7*CFL dt, sweep order xyz/zyx alternating" % (w.name, n, "reflecting walls + radial gravity" if w.grav else "periodic"),
                    "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (NF * ncell * 4 / 1e9),
                    "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk,
-                   "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)"},
+                   "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)",
+                   "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step)"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES.get(n), "peak_kind": "of " + peak_kind,
-                     "kernel": "ppm_sweep_bulk_kernel (3 launches per step; every launch moves 120 B/cell)",
+                     "kernel": ("ppm_advect_bulk_kernel" if args.advect else "ppm_sweep_bulk_kernel") + " (3 launches per step; every launch moves 120 B/cell)",
                      "alu": {"achieved": alu, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu / FP32_PEAK_TFLOPS,
-                             "flops_per_cell_sweep": FLOPS_PER_CELL_SWEEP}},
+                             "flops_per_cell_sweep": flops_cs}},
         "clocks": clocks, "gpu_launches": int(launches),
     }
     if e2e and "ms" in e2e:
@@ -294,6 +298,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number (4 = 512^3, 5 = 1024^3)")
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--advect", action="store_true", help="time PPB-only steps (ppm_advect, SURVEY 8(f) NEXT-2) instead of full PPM+PPB steps")
     ap.add_argument("--flatten3d", action="store_true", help="fully 3-D shock-flattening mode (SURVEY 8(f) NEXT-1): one more light kernel per step")
     ap.add_argument("--direct", action="store_true", help="direct global-memory sweep path instead of the bulk-staged one")
     ap.add_argument("--e2e-steps", type=int, default=2)

@@ -97,6 +97,14 @@ int ppm_step(ppm_ctx *ctx, double dt, int sweep_order);
 /* One sweep along axis d (0,1,2) — the unit ppm_step is made of; exposed for per-sweep parity tests. */
 int ppm_sweep(ppm_ctx *ctx, double dt, int axis);
 
+/* PPB-only step (Fig. 3: the slotted disc in solid-body rotation, "linear
+ * advection"): three PPB-only sweeps in the given order with one dt.  The hydro fields are held fixed; FV (its ten
+ * coefficients) is advected by the stored velocity field with the PPB remap P2-P4 of the full step.  Reading R22
+ * (DESIGN.md): the gas is taken as uniform and the velocity at a face is the mean of the two cell values, so the
+ * mode is meant for velocity fields whose component along an axis does not vary along that axis (rotation, shear,
+ * translation), for which every sweep is volume preserving.  Only enqueues work (3 kernel launches). */
+int ppm_advect(ppm_ctx *ctx, double dt, int sweep_order);
+
 /* dt = cfl*dx / max over cells of max_d(|u_d|) + c.  Synchronises the stream.  dt_out: [host]. */
 int ppm_cfl_dt(ppm_ctx *ctx, double cfl, double *dt_out);
 

@@ -20,7 +20,7 @@ PPM_OK, PPM_EINVAL, PPM_ENOMEM, PPM_ECUDA, PPM_ESTATE = 0, 1, 2, 3, 4
 BC_PERIODIC, BC_REFLECT = 0, 1
 GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
-EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_cfl_dt",
+EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
            "ppm_state_floats", "ppm_destroy", "ppm_last_error")
 OPT_IO_PATH, OPT_FLATTEN3D = 2, 3
@@ -57,6 +57,7 @@ def lib():
         L.ppm_get_state.argtypes = [C.c_void_p, fpp, C.c_int, C.c_int, C.c_int]
         L.ppm_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.ppm_sweep.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.ppm_advect.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.ppm_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.ppm_reduce_conserved.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.ppm_sync.argtypes = [C.c_void_p]
@@ -174,6 +175,10 @@ class PPM:
 
     def step(self, dt, order=0):
         self._check(lib().ppm_step(self._h, float(dt), int(order)))
+
+    def advect(self, dt, order=0):
+        """PPB-only step: FV advected by the stored velocity field, hydro state held fixed (NEXT-2)"""
+        self._check(lib().ppm_advect(self._h, float(dt), int(order)))
 
     def sweep(self, dt, axis):
         self._check(lib().ppm_sweep(self._h, float(dt), int(axis)))

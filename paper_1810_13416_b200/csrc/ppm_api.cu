@@ -176,6 +176,13 @@ extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
     return PPM_OK;
 }
 
+extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
+    if (!c) { set_err(nullptr, "ppm_advect: ctx is NULL"); return PPM_EINVAL; }
+    if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_advect: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
+    for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt, true));
+    return PPM_OK;
+}
+
 extern "C" int ppm_cfl_dt(ppm_ctx* c, double cfl, double* dt_out) {
     if (!c) { set_err(nullptr, "ppm_cfl_dt: ctx is NULL"); return PPM_EINVAL; }
     if (!dt_out || !(cfl > 0.0)) { set_err(c, "ppm_cfl_dt: need cfl > 0 and dt_out"); return PPM_EINVAL; }

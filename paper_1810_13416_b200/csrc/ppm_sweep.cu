@@ -567,6 +567,58 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 }
 
 // =====================================================================================================
+// NEXT-2 (Fig. 3): PPB-only sweep.  The hydro state is held fixed (its fields are
+// copied through) and FV is advected by the stored velocity field: uniform gas (rho = 1), face velocity = mean of
+// the two cell values, mass through the face = dt * u_f (reading R22); P2-P4 exactly as in march().
+// Same iteration timing as march(), so the IO classes serve both: iteration n takes the velocity of cell n and
+// the coefficients of cell n-3, and finishes cell n-4.
+// =====================================================================================================
+template <int DIR, class IO>
+__device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const int c0, const int c1) {
+    const float dtdx = P.dtdx;
+    float uw[5] = {0.f, 0.f, 0.f, 0.f, 0.f};                // normal velocity of cells n-4 .. n
+    float Flm = 0.f;                                        // u at the left face of cell n-4
+    PpbCell mw[3];
+#pragma unroll
+    for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
+#pragma unroll 1
+    for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
+        io.begin(n);
+#pragma unroll
+        for (int s = 0; s < 4; ++s) uw[s] = uw[s + 1];
+        {
+            float sgn, v[5];
+            int j;
+            io.hydro(n, j, sgn, v);
+            uw[4] = v[1];
+        }
+        const float Frm = 0.5f * (uw[0] + uw[1]);           // face (n-4)+1/2
+        mw[0] = mw[1]; mw[1] = mw[2];
+        if (n - 3 >= c0 - 1) {
+            float m[10];
+            io.ppb(n - 3, m);
+            const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
+            const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
+            const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
+            const float th = fminf(1.0f, fdiv(fmaxf(0.f, fminf(m[0], 1.0f - m[0])), fmaxf(B, PPM_TINY)));
+            asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
+            mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+            mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
+            io.ppb_prefetch(n - 2, mw[2]);
+        }
+        const int i = n - PPM_NGHOST;
+        if (i >= c0) {
+            float mo[10];
+            ppb_remap(mw, 1.0f, 1.0f, 1.0f, dtdx * Flm, dtdx * Frm, mo);
+            io.store_ppb(i, mo);
+        }
+        Flm = Frm;
+        io.end(n);
+    }
+    io.finish();
+}
+
+// =====================================================================================================
 // IoDirect: straight global loads / stores.  16 lanes = the 4x4 pencils of one brick column; a load of one
 // field is one 64-byte brick layer per half warp.  A cell's 15 fields sit 256 B apart in its brick record, so
 // each of the three access streams (hydro plane n+1, PPB cell n-2, finished cell n-4) needs one pointer per
@@ -640,6 +692,16 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) p[64 * (5 + PPB_PERM[DIR][k])] = m[k];
     }
+    // PPB-only sweep: the hydro fields of the cell are copied through unchanged
+    __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
+        const long long o = off(i);
+        float* __restrict__ p = pout + o;
+        const float* __restrict__ q = pin + o;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) p[64 * f] = __ldg(q + 64 * f);
+#pragma unroll
+        for (int k = 0; k < 10; ++k) p[64 * (5 + PPB_PERM[DIR][k])] = m[k];
+    }
     __device__ __forceinline__ void end(int) {}
     __device__ __forceinline__ void finish() {}
 };
@@ -660,6 +722,21 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     const float* pflat = FLAT ? P.flat + ((long long)ba * P.FBa + (long long)bb * P.FBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)))) : nullptr;
     march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, true, wmask, pflat);
+}
+
+// PPB-only sweep (NEXT-2), direct path
+template <int DIR>
+__global__ void __launch_bounds__(PPM_CTA) ppm_advect_kernel(const SweepParams P) {
+    constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
+    const int t = threadIdx.x;
+    const int ba = blockIdx.x * (PPM_CTA / 16) + (t >> 4), bb = blockIdx.y;
+    const int a = ba * 4 + (t & 3), b = bb * 4 + ((t >> 2) & 3);
+    if (a >= P.na || b >= P.nb) return;
+    const int c0 = blockIdx.z * P.chunk;
+    const int c1 = min(c0 + P.chunk, P.n);
+    const long long tb = (long long)ba * P.SBa + (long long)bb * P.SBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)));
+    IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
+    march_ppb<DIR>(P, io, c0, c1);
 }
 
 // ---- shared-memory / mbarrier / bulk-copy primitives ----------------------------------------------------
@@ -850,6 +927,11 @@ struct IoBulk {
         dh[64 * Dir<DIR>::V] = h[2];
         dh[64 * Dir<DIR>::W] = h[3];
         dh[64 * 4] = h[4];
+        store_ppb(i, m);
+    }
+    // PPB part of cell i only (PPB-only sweep: the hydro slot goes back to global memory as it came in)
+    __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
+        const int s = i & 3;
         float* dp = ppr + pst + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
@@ -882,6 +964,26 @@ struct IoBulk {
 // whole pencils while they fill complete waves of resident CTAs and cuts the pencils of the ragged last wave into
 // shorter segments, so that the SMs run dry together.  A cut costs 8 redundant warm-up cells; results do not
 // depend on where the cuts are.
+// this CTA's pencil segment: tile index and cell range [c0, c1)
+__device__ __forceinline__ void bulk_segment(const SweepParams& P, int& tile, int& c0, int& c1) {
+    const int ncha = (P.n + P.chunk - 1) / P.chunk;
+    const int na_ctas = P.tiles_a * ncha;
+    int u = blockIdx.x, ch = P.chunk, nch = ncha, t0 = 0;
+    if (u >= na_ctas) { u -= na_ctas; ch = P.chunk_b; nch = (P.n + ch - 1) / ch; t0 = P.tiles_a; }
+    const int t = u / nch;
+    tile = t0 + t;
+    c0 = (u - t * nch) * ch;
+    c1 = min(c0 + ch, P.n);
+}
+template <int DIR>
+__device__ __forceinline__ void bulk_init_barriers(uint64_t* bars) {
+    using G = BulkGeom<DIR>;
+    if (threadIdx.x < G::WARPS * (G::NH + G::NP)) mbar_init(bars + threadIdx.x, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_async_smem();
+    __syncthreads();
+}
+
 template <int DIR, int GRAV, bool FLAT>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
@@ -889,23 +991,11 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     float* sm = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (threadIdx.x < G::WARPS * (G::NH + G::NP)) mbar_init(bars + threadIdx.x, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    fence_async_smem();
-    __syncthreads();
+    bulk_init_barriers<DIR>(bars);
     const int nba = (P.na + 3) >> 2;
     const int ntx = (nba + 2 * G::WARPS - 1) / (2 * G::WARPS);    // tiles along a
     int tile, c0, c1;
-    {
-        const int ncha = (P.n + P.chunk - 1) / P.chunk;
-        const int na_ctas = P.tiles_a * ncha;
-        int u = blockIdx.x, ch = P.chunk, nch = ncha, t0 = 0;
-        if (u >= na_ctas) { u -= na_ctas; ch = P.chunk_b; nch = (P.n + ch - 1) / ch; t0 = P.tiles_a; }
-        const int t = u / nch;
-        tile = t0 + t;
-        c0 = (u - t * nch) * ch;
-        c1 = min(c0 + ch, P.n);
-    }
+    bulk_segment(P, tile, c0, c1);
     const int bb = tile / ntx, tx = tile - bb * ntx;
     const int ba0 = (tx * G::WARPS + warp) * 2;                    // the warp's brick columns: ba0, ba0 + 1 along a; bb along b
     if (ba0 >= nba) return;                                        // whole warp out of range (no block-wide sync below)
@@ -917,6 +1007,27 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
     march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu, pflat);
+}
+
+// PPB-only sweep (NEXT-2), bulk-staged path: same rings; the hydro slots travel through unchanged
+template <int DIR>
+__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_advect_bulk_kernel(const SweepParams P) {
+    using G = BulkGeom<DIR>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* sm = reinterpret_cast<float*>(smem_raw);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    bulk_init_barriers<DIR>(bars);
+    const int nba = (P.na + 3) >> 2;
+    const int ntx = (nba + 2 * G::WARPS - 1) / (2 * G::WARPS);
+    int tile, c0, c1;
+    bulk_segment(P, tile, c0, c1);
+    const int bb = tile / ntx, tx = tile - bb * ntx;
+    const int ba0 = (tx * G::WARPS + warp) * 2;
+    if (ba0 >= nba) return;
+    const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
+    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
+    march_ppb<DIR>(P, io, c0, c1);
 }
 
 // cells per segment for the tiles of the ragged last wave: the cut that minimises (waves of segments) x (segment
@@ -935,14 +1046,14 @@ static int tail_chunk(int ntail, int slots, int n) {
     return best;
 }
 
-template <int DIR, int GRAV, bool FLAT>
-cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
+// segment plan + launch of one bulk-path kernel; occ caches the kernel's resident CTAs per SM
+template <int DIR>
+cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int& occ, SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
     using G = BulkGeom<DIR>;
-    static int occ = 0;
     if (!occ) {
-        cudaError_t e = cudaFuncSetAttribute(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, G::WARPS * 32, G::SMEM);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, G::WARPS * 32, G::SMEM);
         if (e != cudaSuccess) return e;
         if (occ < 1) occ = 1;
     }
@@ -956,8 +1067,18 @@ cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st
         P.chunk_b = (P.tiles_a < ntiles) ? tail_chunk(ntiles - P.tiles_a, slots, P.n) : P.n;
     }
     const long long grid = (long long)P.tiles_a * ((P.n + P.chunk - 1) / P.chunk) + (long long)(ntiles - P.tiles_a) * ((P.n + P.chunk_b - 1) / P.chunk_b);
-    ppm_sweep_bulk_kernel<DIR, GRAV, FLAT><<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
+    kern<<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
     return cudaGetLastError();
+}
+template <int DIR, int GRAV, bool FLAT>
+cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
+    static int occ = 0;
+    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, occ, P, sms, user_chunk, st);
+}
+template <int DIR>
+cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
+    static int occ = 0;
+    return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR>, occ, P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_bulk_dir(SweepParams& P, int grav, int sms, int user_chunk, cudaStream_t st) {
@@ -993,7 +1114,7 @@ bool ppm_axis_is_bulk(const ppm_ctx* c, int axis) {
     return c->io_path == 0 && ext[axis] % 4 == 0;
 }
 
-cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
+cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect) {
     const ppm_params& p = c->prm;
     SweepParams P;
     P.in = c->buf[c->cur];
@@ -1026,13 +1147,22 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt) {
     if (use_bulk) {
         P.ntiles = ((nba + 7) / 8) * nbb;                                     // CTA tile = 4 warps x 2 brick columns along a
         const int uc = c->chunk > 0 ? chunk : 0;                              // 0: whole pencils, the last wave cut to finish together
-        if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
+        if (advect) {
+            if (axis == 0) e = launch_advect_bulk<0>(P, c->sms, uc, c->stream);
+            else if (axis == 1) e = launch_advect_bulk<1>(P, c->sms, uc, c->stream);
+            else e = launch_advect_bulk<2>(P, c->sms, uc, c->stream);
+        } else if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
         else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, c->sms, uc, c->stream);
         else e = launch_bulk_dir<2>(P, p.grav.kind, c->sms, uc, c->stream);
     } else {
         dim3 block(PPM_CTA, 1, 1);
         dim3 grid((nba + PPM_CTA / 16 - 1) / (PPM_CTA / 16), nbb, nchunks);
-        if (axis == 0) e = launch_dir<0>(P, p.grav.kind, grid, block, c->stream);
+        if (advect) {
+            if (axis == 0) ppm_advect_kernel<0><<<grid, block, 0, c->stream>>>(P);
+            else if (axis == 1) ppm_advect_kernel<1><<<grid, block, 0, c->stream>>>(P);
+            else ppm_advect_kernel<2><<<grid, block, 0, c->stream>>>(P);
+            e = cudaGetLastError();
+        } else if (axis == 0) e = launch_dir<0>(P, p.grav.kind, grid, block, c->stream);
         else if (axis == 1) e = launch_dir<1>(P, p.grav.kind, grid, block, c->stream);
         else e = launch_dir<2>(P, p.grav.kind, grid, block, c->stream);
     }

@@ -221,6 +221,79 @@ def test_flatten3d_ragged_grid_and_paths_agree():
     assert max(e.values()) <= L1_SHOCK, e
 
 
+# ---------------------------------------------------------------- NEXT-2: PPB-only advection ----------
+def test_advect_matches_oracle_and_paths_agree():
+    """PPB-only steps (ppm_advect) on config 1's fields (32^3 periodic) and on a ragged grid with mirror walls: FV
+    against the oracle's mode, the hydro fields bit for bit untouched, bulk-staged == direct bitwise."""
+    PPM = _gpu()
+    from oracle import binding as ob
+    from paper_1810_13416_b200.binding import OPT_IO_PATH
+    rng = np.random.default_rng(31)
+    cases = []
+    w = W.make(1)
+    f1 = w.fields().numpy()
+    f1[1:4] *= 8.0                                             # Courant numbers up to ~0.5 at dt below
+    cases.append((f1, (w.n,) * 3, w.dx, w.bc, 0.5 * w.dx / np.abs(f1[1:4]).max()))
+    nx, ny, nz = 36, 30, 22
+    f2 = np.zeros((15, nz, ny, nx), dtype=np.float32)
+    f2[0], f2[4] = 1.0, 1.0
+    f2[1:4] = 0.5 * rng.normal(size=(3, nz, ny, nx))
+    f2[5] = 0.2 + 0.6 * rng.random((nz, ny, nx))
+    f2[6:] = 0.02 * rng.normal(size=(9, nz, ny, nx))
+    cases.append((f2, (nx, ny, nz), 0.03, (1, 1, 0, 0, 1, 1), 0.4 * 0.03 / np.abs(f2[1:4]).max()))
+    for f, dims, dx, bc, dt in cases:
+        o = ob.Oracle(dims[0], dims[1], dims[2], dx, 1.4, bc, None)
+        o.set_state(f)
+        for order in range(6):
+            o.advect(dt, order)
+        os_ = o.get_state()
+        res = []
+        for io in (0, 1):
+            g = PPM(dims[0], dims[1], dims[2], dx, 1.4, bc)
+            g.set_option(OPT_IO_PATH, io)
+            g.set_state(f)
+            h0 = g.get_state().cpu().numpy()
+            n0 = g.launch_count()
+            for order in range(6):
+                g.advect(dt, order)
+            assert g.launch_count() - n0 == 18
+            res.append(g.get_state().cpu().numpy())
+            assert np.array_equal(res[-1][:5], h0[:5])          # the hydro state is held fixed
+            g.close()
+        assert np.array_equal(res[0], res[1])
+        e = max_rel(res[0].astype(np.float64), os_)
+        assert e["FV"] <= ONE_STEP, e
+        assert np.abs(os_[5] - f[5]).max() > 1e-3               # ... and FV really moved
+
+
+def test_advect_slotted_disc_one_revolution_fig3():
+    """PAPER.md Fig. 3 on the paper's grid: 100 x 100 cells (x 1: the 2-D case, six in-plane coefficients), one
+    revolution = 1256 PPB-only steps, against the oracle.  The field is a 0/1 indicator, so the bar is the L1 one."""
+    PPM = _gpu()
+    from oracle import binding as ob
+    n, steps = 100, 1256
+    f = W.slotted_disc(n)
+    dt = 1.0 / steps
+    o = ob.Oracle(n, n, 1, 1.0 / n, 1.4, (0,) * 6)
+    g = PPM(n, n, 1, 1.0 / n, 1.4, (0,) * 6)
+    o.set_state(f)
+    g.set_state(f)
+    for k in range(steps):
+        order = 0 if k % 2 == 0 else 2
+        o.advect(dt, order)
+        g.advect(dt, order)
+    gs = g.get_state().cpu().numpy().astype(np.float64)
+    os_ = o.get_state()
+    g.close()
+    e = l1_rel(gs, os_)
+    assert e["FV"] <= L1_SHOCK, e
+    assert gs[5].min() >= 0.0 and gs[5].max() <= 1.0
+    assert abs(gs[5].sum() - f[5].astype(np.float64).sum()) <= 1e-5 * f[5].sum()      # fp32 round-off of 2512 sweeps
+    # the disc is back: slot still open, bridge still full (the oracle pins carry the comparison with donor-cell)
+    assert gs[5, 0, 64:78, 49:51].max() < 0.12 and gs[5, 0, 64:78, 43:45].min() > 0.9
+    assert not gs[[8, 11, 13, 14]].any()                       # the out-of-plane coefficients stay zero: the 6-moment 2-D scheme
+
+
 def test_cfg4_convection_reduced_64_20_steps():
     w = W.make(4, n=64)
     r = _run_pair(w, 20)
