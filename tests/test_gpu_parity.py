@@ -362,6 +362,40 @@ def test_degenerate_grids_2d_1d_and_fewer_cells_than_ghosts(dims):
     g.close()
 
 
+def test_state_flag_reports_floor_hits_and_bad_states():
+    """error behaviour of the boundary (include/ppm.h): a step that drives the pressure to its floor, or a state with
+    non-positive density, is reported as PPM_ESTATE by the next synchronising call; a new ppm_set_state clears it."""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import PPMError, PPM_ESTATE
+    n = 16
+    f = np.zeros((15, n, n, n), dtype=np.float32)
+    f[0], f[4], f[5] = 1.0, 1.0, 0.5
+    g = PPM(n, n, n, 1.0 / n, 1.4, (0,) * 6, p_floor=1e-6, rho_floor=1e-6)
+    g.set_state(f)
+    g.step(0.5 * g.cfl_dt(0.8), 0)
+    g.sync()                                               # a healthy state: no flag
+    bad = f.copy()
+    bad[1, :, :, : n // 2] = 30.0                          # Mach 25 streams pulling apart: a near-vacuum opens between them
+    bad[1, :, :, n // 2:] = -30.0
+    bad[1] *= -1.0
+    g.set_state(bad)
+    dt = g.cfl_dt(0.8)
+    for s in range(6):
+        g.step(4.0 * dt, 0)                                # and a time step far beyond the CFL limit
+    with pytest.raises(PPMError) as ei:
+        g.sync()
+    assert ei.value.code == PPM_ESTATE
+    g.set_state(f)                                         # loading a state clears the sticky flag
+    g.sync()
+    neg = f.copy()
+    neg[0, 3, 4, 5] = -1.0
+    g.set_state(neg)
+    with pytest.raises(PPMError) as ei:
+        g.cfl_dt(0.8)
+    assert ei.value.code == PPM_ESTATE
+    g.close()
+
+
 def test_hydrostatic_state_is_preserved_exactly_on_gpu():
     PPM = _gpu()
     for cfg, n in ((2, 32), (4, 32)):
