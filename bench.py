@@ -217,6 +217,19 @@ def run_gpu(args):
     clocks = clk.stop()
     g.sync()                         # raises if the state flag (NaN / floor) was set
 
+    # ---- the same K steps with ppm_cfl_dt before each one (SURVEY 8(d) "also report with ppm_cfl_dt per step
+    # included"): one more reduction kernel and one host sync per step ----
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e2.record(g.stream)
+    for s in range(K):
+        do_step(0.7 * g.cfl_dt(w.cfl), 0 if s % 2 == 0 else 5)
+    e3.record(g.stream)
+    barrier()
+    ms_cfl = e2.elapsed_time(e3)
+    if ws > 1:
+        ms_cfl = max_over_ranks([ms_cfl], ws, dev)[0]
+
     # ---- e2e: host buffers through the C ABI, copies inside the timed region ----
     e2e = None
     if not args.no_e2e:
@@ -274,6 +287,8 @@ def run_gpu(args):
                      "alu": {"achieved": alu, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu / FP32_PEAK_TFLOPS,
                              "flops_per_cell_sweep": flops_cs}},
         "clocks": clocks, "gpu_launches": int(launches),
+        "with_cfl_dt": {"value": aggregate_value(ncell, K, ms_cfl, ws), "unit": UNIT, "ms_per_step": ms_cfl / K,
+                        "note": "ppm_cfl_dt (max-reduction kernel + host sync) before every step"},
     }
     if e2e and "ms" in e2e:
         line["e2e"] = {"value": ws * ncell / (e2e["ms"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["bytes"],

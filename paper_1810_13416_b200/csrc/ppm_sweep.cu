@@ -231,17 +231,16 @@ __device__ __forceinline__ void parabola(const V5& q0, const V5& Lc, const V5& R
 // pre-limited coefficients of one cell in local family order, stored as the pairs the remap uses
 struct PpbCell { float a0, a1, a2; v2 bc0, bc1, de; float f; };   // bc0 = (b0, c0), bc1 = (b1, c1), de = (d0, e0)
 
-// S[0..2]: cells i-1, i, i+1; rm,r0,rp their masses per dx; dl, dr = mass per dx through the left / right
+// S[0..2]: cells i-1, i, i+1 (masses per dx rm, r0, rp); dl, dr = mass per dx through the left / right
 // face (positive rightward).  The two donor pieces (from i-1 and from i+1) run as one packed computation for
 // the degree-2 family; the (b,c) and (d,e) families are packed inside every piece.
-__device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float rm, float r0, float rp, float dl, float dr, float (&out)[10]) {
-    const float rn = r0 - dr + dl;
+// irm, ir0, irp: reciprocals of the three masses; rn, irn: the cell's new mass per dx (= r0 - dr + dl; the caller has it
+// as the updated density) and its reciprocal.
+__device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, float ir0, float irp, float rn, float irn, float dl, float dr, float (&out)[10]) {
     const bool ok = rn > PPM_TINY;
-    const float irn = rcp(fmaxf(rn, PPM_TINY));
     const float dln = fmaxf(-dl, 0.f), drp = fmaxf(dr, 0.f);
     const v2 dD = mk(fmaxf(dl, 0.f), fmaxf(-dr, 0.f));      // donated mass: from the left cell, from the right cell
-    const v2 irD = mk(rcp(rm), rcp(rp));
-    const float ir0 = rcp(r0);
+    const v2 irD = mk(irm, irp);
     // piece geometry: new-coordinate midpoint x, half width h; old-coordinate midpoint s, slope beta
     const v2 hD = dD * bc(0.5f * irn);                       // half widths of the donor pieces in the new cell
     const v2 xD = fma2(hD, mk(1.f, -1.f), mk(-0.5f, 0.5f));
@@ -553,7 +552,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
-            ppb_remap(mw, rf[0], rf[1], rf[2], dtdx * Flm, dtdx * Frm, mo);
+            ppb_remap(mw, rcp(rf[0]), rcp(rf[1]), rcp(rf[2]), r_new, irn, dtdx * Flm, dtdx * Frm, mo);
             io.store(i, ho, mo);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
@@ -609,7 +608,8 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
         const int i = n - PPM_NGHOST;
         if (i >= c0) {
             float mo[10];
-            ppb_remap(mw, 1.0f, 1.0f, 1.0f, dtdx * Flm, dtdx * Frm, mo);
+            const float rn = 1.0f - dtdx * (Frm - Flm);
+            ppb_remap(mw, 1.0f, 1.0f, 1.0f, rn, rcp(fmaxf(rn, PPM_TINY)), dtdx * Flm, dtdx * Frm, mo);
             io.store_ppb(i, mo);
         }
         Flm = Frm;
@@ -904,18 +904,18 @@ struct IoBulk {
         j = jb + s;
         const float* src = hyd + hcur + (s << SH);
         v[0] = src[0];
-        v[1] = sgn * src[64 * Dir<DIR>::U];                    // normal velocity: odd under the mirror
+        const float un = src[64 * Dir<DIR>::U];
+        v[1] = hrev ? -un : un;                                // normal velocity: odd under the mirror
         v[2] = src[64 * Dir<DIR>::V];
         v[3] = src[64 * Dir<DIR>::W];
         v[4] = src[64 * 4];
     }
     __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
         const int s = (c & 3) ^ prev;
-        const float sgn = prev ? -1.0f : 1.0f;
         const float* src = ppr + pcur + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) m[q] = src[64 * PPB_PERM[DIR][q]];
-        m[1] *= sgn; m[4] *= sgn; m[6] *= sgn;
+        if (prev) { m[1] = -m[1]; m[4] = -m[4]; m[6] = -m[6]; }   // odd coefficients under the mirror (warp-uniform, rare)
     }
     __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
     // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
