@@ -2,7 +2,7 @@
 //
 // One thread owns one grid pencil (pencils are independent within a 1-D pass) and
 // marches along the sweep axis with a short sliding window held on chip — the paper's pipelined pencil
-// update with a barrel shift (Fig. 7), re-designed for SoA planes: lanes run along
+// update with a barrel shift (Fig. 7), re-designed for brick records with SoA fields: lanes run along
 // a transverse axis, so no briquette records, transposes or 16||16 vector splices are needed.
 //
 // Each iteration n takes plane n and finishes cell n-4 (stencil reach 4, L120).  Per iteration:

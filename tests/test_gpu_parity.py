@@ -305,7 +305,7 @@ def test_cfg4_convection_reduced_64_20_steps():
 @pytest.mark.parametrize("dims", [(37, 29, 23), (36, 30, 22)])
 def test_ragged_grid_all_boundaries_and_orders(dims):
     """extents that are not multiples of the 4-cell brick (pad cells in the last bricks, half-empty warps), mixed
-    boundaries, all six orders.  (36, 30, 22): nx % 4 == 0, so the x sweep takes the TMA path over ragged y, z."""
+    boundaries, all six orders.  (36, 30, 22): nx % 4 == 0, so the x sweep takes the bulk-staged path over ragged y, z."""
     PPM = _gpu()
     from oracle import binding as ob
     rng = np.random.default_rng(11)
