@@ -24,11 +24,12 @@ __device__ __forceinline__ long long cell_offset(const AuxParams& A, int i, int 
 // storage slot t (brick * 64 + cell in brick) -> (i,j,k) and the offset of field 0; false for a pad cell
 __device__ __forceinline__ bool cell_of(const AuxParams& A, long long t, int& i, int& j, int& k, long long& off) {
     const int c = (int)(t & 63);
-    long long B = t >> 6;
-    off = B * PPM_BRICK_FLOATS + c;
-    const int bx = (int)(B % A.nbx); B /= A.nbx;
-    const int by = (int)(B % A.nby);
-    const int bz = (int)(B / A.nby);
+    const unsigned B = (unsigned)(t >> 6);                 // brick index < 2^25 (ppm_create caps the cells at 2^31): 32-bit divisions
+    off = (long long)B * PPM_BRICK_FLOATS + c;
+    const unsigned q = B / (unsigned)A.nbx;
+    const int bx = (int)(B - q * (unsigned)A.nbx);
+    const int bz = (int)(q / (unsigned)A.nby);
+    const int by = (int)(q - (unsigned)bz * (unsigned)A.nby);
     i = bx * 4 + (c & 3); j = by * 4 + ((c >> 2) & 3); k = bz * 4 + (c >> 4);
     return i < A.nx && j < A.ny && k < A.nz;
 }
@@ -93,19 +94,39 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
     }
 }
 
+// fp32 base state (rho0, p0) at a cell centre, as the sweeps evaluate it
+__device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k) {
+    if (A.grav_kind == PPM_GRAV_CONST_Z) {
+        const float4 v = __ldg(A.tab32 + 2 * k + 2 * PPM_NGHOST + 1);
+        return make_float2(v.x, v.y);
+    }
+    if (A.grav_kind == PPM_GRAV_RADIAL) {
+        const float dx = A.dxf;
+        const float x = ((float)i + 0.5f) * dx - A.cxf, y = ((float)j + 0.5f) * dx - A.cyf, z = ((float)k + 0.5f) * dx - A.czf;
+        const float r2 = fmaf(x, x, fmaf(y, y, z * z));
+        const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
+        const float t = (r - A.s0f) * A.inv_dsf;
+        int kk = (int)floorf(t);
+        kk = min(max(kk, 0), A.tab_n - 2);
+        const float w = t - (float)kk;
+        const float4 a = __ldg(A.tab32 + kk), b = __ldg(A.tab32 + kk + 1);
+        return make_float2(fmaf(w, b.x - a.x, a.x), fmaf(w, b.y - a.y, a.y));
+    }
+    return make_float2(0.f, 0.f);
+}
+
 // order-preserving float -> uint encoding for atomicMax (all values here are >= 0)
 __device__ __forceinline__ unsigned int enc(float x) { return __float_as_uint(fmaxf(x, 0.f)); }
 
-__global__ void __launch_bounds__(256) cfl_kernel(AuxParams A, const float* __restrict__ st, unsigned int* __restrict__ out, int* flag) {
+__global__ void __launch_bounds__(256) cfl_kernel(const AuxParams A, const float* __restrict__ st, unsigned int* __restrict__ out, int* flag) {
     float vmax = 0.f;
-    const float gam = (float)A.gamma;
+    const float gam = A.gamf;
     for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
         int i, j, k;
         long long o;
         if (!cell_of(A, t, i, j, k, o)) continue;
-        double r0, p0;
-        base64(A, i, j, k, r0, p0);
-        const float rho = (float)(r0 + (double)st[o]), p = (float)(p0 + (double)st[o + 4 * 64]);
+        const float2 b0 = base32(A, i, j, k);              // fp32 base state, as the sweeps evaluate it
+        const float rho = b0.x + st[o], p = b0.y + st[o + 4 * 64];
         const float c = sqrtf(gam * p / rho);
         const float um = fmaxf(fabsf(st[o + 64]), fmaxf(fabsf(st[o + 2 * 64]), fabsf(st[o + 3 * 64])));
         const float v = um + c;
@@ -168,27 +189,6 @@ __global__ void conserved_final_kernel(const double* __restrict__ partial, int n
 // F~_i = max over the three directions d of the H4 coefficient f~^d_i = steep * jump * conv, each evaluated along d
 // (full p at i-2..i+2, u_d at i-1, i+1, c_i) on the state the step starts from; ghost cells by the boundary images
 // (periodic wrap / mirror with the normal velocity negated).  One value per cell, [brick][4z][4y][4x].
-// fp32 base state (rho0, p0) at a cell centre, as the sweeps evaluate it
-__device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k) {
-    if (A.grav_kind == PPM_GRAV_CONST_Z) {
-        const float4 v = __ldg(A.tab32 + 2 * k + 2 * PPM_NGHOST + 1);
-        return make_float2(v.x, v.y);
-    }
-    if (A.grav_kind == PPM_GRAV_RADIAL) {
-        const float dx = A.dxf;
-        const float x = ((float)i + 0.5f) * dx - A.cxf, y = ((float)j + 0.5f) * dx - A.cyf, z = ((float)k + 0.5f) * dx - A.czf;
-        const float r2 = fmaf(x, x, fmaf(y, y, z * z));
-        const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
-        const float t = (r - A.s0f) * A.inv_dsf;
-        int kk = (int)floorf(t);
-        kk = min(max(kk, 0), A.tab_n - 2);
-        const float w = t - (float)kk;
-        const float4 a = __ldg(A.tab32 + kk), b = __ldg(A.tab32 + kk + 1);
-        return make_float2(fmaf(w, b.x - a.x, a.x), fmaf(w, b.y - a.y, a.y));
-    }
-    return make_float2(0.f, 0.f);
-}
-
 __device__ __forceinline__ int aux_image(int i, int n, int bc_lo, int bc_hi, float& sgn) {
     sgn = 1.0f;
     if ((unsigned)i < (unsigned)n) return i;
