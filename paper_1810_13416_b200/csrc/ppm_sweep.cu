@@ -527,8 +527,16 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         // ---- J, K, L: finish cell n-4 ---------------------------------------------------------------------
         const int i = n - PPM_NGHOST;
         if (i >= c0) {
-            const float r_old = rf[1], rp_old = q[0].A.x, pp_old = q[0].A.y, u0 = q[0].u, g = gw[0];
-            const v2 vw0 = q[0].B;
+            // the cell's old values: the bulk path still has them in shared memory (its results overwrite them below),
+            // so the register window need not carry them for four iterations
+            V5 qo = q[0];
+            if (IO::HAS_OLD) {
+                float v[5];
+                io.old_hydro(i, v);
+                qo.A = mk(v[0], v[4]); qo.B = mk(v[2], v[3]); qo.u = v[1];
+            }
+            const float r_old = rf[1], rp_old = qo.A.x, pp_old = qo.A.y, u0 = qo.u, g = gw[0];
+            const v2 vw0 = qo.B;
             float drho = -dtdx * (Frm - Flm);
             int bad = 0;
             if (!(r_old + drho > P.rho_floor)) { drho = P.rho_floor - r_old; bad = 1; }
@@ -626,6 +634,8 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
 // =====================================================================================================
 template <int DIR>
 struct IoDirect {
+    static constexpr bool HAS_OLD = false;   // no staged copy of a cell's old values: march() carries them in registers
+    __device__ __forceinline__ void old_hydro(int, float (&)[5]) {}
     static constexpr int SH = 2 * DIR;       // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
     const float* __restrict__ const pin;     // the thread's pencil: cell 0 of the sweep axis, field 0
@@ -918,6 +928,16 @@ struct IoBulk {
         if (prev) { m[1] = -m[1]; m[4] = -m[4]; m[6] = -m[6]; }   // odd coefficients under the mirror (warp-uniform, rare)
     }
     __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
+    static constexpr bool HAS_OLD = true;
+    // the hydro input of interior cell i, still in its slot when the cell is finished (n = i + 4)
+    __device__ __forceinline__ void old_hydro(int i, float (&v)[5]) {
+        const float* src = hyd + hprv + ((i & 3) << SH);
+        v[0] = src[0];
+        v[1] = src[64 * Dir<DIR>::U];
+        v[2] = src[64 * Dir<DIR>::V];
+        v[3] = src[64 * Dir<DIR>::W];
+        v[4] = src[64 * 4];
+    }
     // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
     __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
         const int s = i & 3;
