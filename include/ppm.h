@@ -77,7 +77,8 @@ size_t ppm_state_floats(int nx, int ny, int nz);
 /* Creates a context.  dev_buf_a, dev_buf_b: [device] two caller-owned buffers of
  * ppm_state_floats(nx,ny,nz) floats each, 128-byte aligned (e.g. torch tensors).  The library BORROWS them for the
  * life of the context: the state lives in one, the other is sweep scratch, and they ping-pong.  It
- * never frees them.  Contents are undefined until ppm_set_state has covered every z-slab. */
+ * never frees them.  Contents are undefined until ppm_set_state has covered every z-slab.  Every later call runs on
+ * the device that owns these buffers, whatever device is current in the calling thread (and restores the caller's). */
 int ppm_create(ppm_ctx **out, const ppm_params *prm, float *dev_buf_a, float *dev_buf_b);
 
 /* Loads the full state (rho, ux, uy, uz, p, m000..m011) for z-planes [z0, z0+nz_slab).

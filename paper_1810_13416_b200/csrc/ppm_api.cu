@@ -27,6 +27,15 @@ static void set_err(ppm_ctx* c, const char* fmt, ...) {
         }                                                                                   \
     } while (0)
 
+// Every entry point runs on the device that owns the state buffers, whatever device is current in the caller.
+struct DevGuard {
+    int old = -1, dev;
+    explicit DevGuard(const ppm_ctx* c) : dev(c ? c->device : -1) {
+        if (dev >= 0 && cudaGetDevice(&old) == cudaSuccess && old != dev) cudaSetDevice(dev); else old = -1;
+    }
+    ~DevGuard() { if (old >= 0) cudaSetDevice(old); }
+};
+
 static const int ORDERS[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
 
 extern "C" const char* ppm_last_error(const ppm_ctx* c) { return c ? c->err : g_err; }
@@ -78,9 +87,17 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c->prm = *prm;
     c->prm.grav.g = c->prm.grav.rho0 = c->prm.grav.p0 = nullptr;   // host arrays are not kept
     c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0;
+    {   // the device that owns the buffers (falls back to the current one for memory the runtime does not know)
+        cudaPointerAttributes pa;
+        int cur = 0;
+        cudaGetDevice(&cur);
+        c->device = (cudaPointerGetAttributes(&pa, dev_buf_a) == cudaSuccess && pa.type == cudaMemoryTypeDevice) ? pa.device : cur;
+        cudaGetLastError();
+    }
+    DevGuard guard(c);
     c->stream = (cudaStream_t)prm->stream;
     c->nblocks_red = 148 * 4;
-    { int dev = 0; cudaGetDevice(&dev); if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->sms < 1) c->sms = 148; }
+    if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sms < 1) c->sms = 148;
     c->chunk = 0;
     c->err[0] = 0;
     // brick records of 4x4x4 cells x 15 fields; extents are rounded up to whole bricks (ppm_state_floats)
@@ -111,6 +128,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
 
 extern "C" void ppm_destroy(ppm_ctx* c) {
     if (!c) return;
+    DevGuard guard(c);
     cudaFree(c->flag); cudaFree(c->cflmax); cudaFree(c->partial); cudaFree(c->result);
     cudaFree(c->tab); cudaFree(c->tab64); cudaFree(c->F3);
     free(c);
@@ -134,6 +152,7 @@ static int read_flag(ppm_ctx* c) {
 extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS], int z0, int nzs, int src_is_device) {
     int rc = check_slab(c, fields, z0, nzs, "ppm_set_state");
     if (rc) return rc;
+    DevGuard guard(c);
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_set_state: fields[%d] is NULL", f); return PPM_EINVAL; }
     const long long plane = (long long)c->prm.nx * c->prm.ny;
     float* st = c->buf[c->cur];
@@ -150,6 +169,7 @@ extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS],
 extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z0, int nzs, int dst_is_device) {
     int rc = check_slab(c, fields, z0, nzs, "ppm_get_state");
     if (rc) return rc;
+    DevGuard guard(c);
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_get_state: fields[%d] is NULL", f); return PPM_EINVAL; }
     const long long plane = (long long)c->prm.nx * c->prm.ny, tot = plane * nzs;
     float* scratch = c->buf[c->cur ^ 1];    // free between steps
@@ -162,6 +182,7 @@ extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z
 
 extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
     if (!c) { set_err(nullptr, "ppm_sweep: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "ppm_sweep: need finite dt > 0 and axis in 0..2"); return PPM_EINVAL; }
     if (c->flat3d) CU(ppm_launch_flatten3d(c));     // the detector field of the state this sweep starts from
     CU(ppm_launch_sweep(c, axis, dt));
@@ -170,6 +191,7 @@ extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
 
 extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
     if (!c) { set_err(nullptr, "ppm_step: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_step: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
     if (c->flat3d) CU(ppm_launch_flatten3d(c));     // once per step, on the step's starting state
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt));
@@ -178,6 +200,7 @@ extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
 
 extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
     if (!c) { set_err(nullptr, "ppm_advect: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_advect: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt, true));
     return PPM_OK;
@@ -185,6 +208,7 @@ extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
 
 extern "C" int ppm_cfl_dt(ppm_ctx* c, double cfl, double* dt_out) {
     if (!c) { set_err(nullptr, "ppm_cfl_dt: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (!dt_out || !(cfl > 0.0)) { set_err(c, "ppm_cfl_dt: need cfl > 0 and dt_out"); return PPM_EINVAL; }
     CU(ppm_launch_cfl(c));
     unsigned int enc = 0;
@@ -200,6 +224,7 @@ extern "C" int ppm_cfl_dt(ppm_ctx* c, double cfl, double* dt_out) {
 
 extern "C" int ppm_reduce_conserved(ppm_ctx* c, double out[6]) {
     if (!c) { set_err(nullptr, "ppm_reduce_conserved: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (!out) { set_err(c, "ppm_reduce_conserved: out is NULL"); return PPM_EINVAL; }
     CU(ppm_launch_conserved(c));
     CU(cudaMemcpyAsync(out, c->result, sizeof(double) * 6, cudaMemcpyDeviceToHost, c->stream));
@@ -208,6 +233,7 @@ extern "C" int ppm_reduce_conserved(ppm_ctx* c, double out[6]) {
 
 extern "C" int ppm_sync(ppm_ctx* c) {
     if (!c) { set_err(nullptr, "ppm_sync: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     return read_flag(c);
 }
 
@@ -220,6 +246,7 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
     if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
         if (value && !c->F3) {

@@ -48,6 +48,7 @@ struct ppm_ctx {
     float* buf[2];
     int cur;                        // buf[cur] holds the state
     cudaStream_t stream;
+    int device;                     // the device that owns buf[0], buf[1]; every entry point switches to it
     float4* tab;                    // device gravity table (fp32 nodes)
     double* tab64;                  // device gravity table as doubles {g, rho0, p0} x n (set/get/reductions)
     int* flag;                      // device sticky flag

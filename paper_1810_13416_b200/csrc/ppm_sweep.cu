@@ -1066,10 +1066,15 @@ static int tail_chunk(int ntail, int slots, int n) {
     return best;
 }
 
-// segment plan + launch of one bulk-path kernel; occ caches the kernel's resident CTAs per SM
+// segment plan + launch of one bulk-path kernel; occs caches the kernel's resident CTAs per SM, per device (the
+// shared-memory opt-in is a per-device function attribute)
+constexpr int MAX_DEV = 64;
 template <int DIR>
-cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int& occ, SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
+cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_DEV], SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
     using G = BulkGeom<DIR>;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int& occ = occs[dev & (MAX_DEV - 1)];
     if (!occ) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM);
         if (e != cudaSuccess) return e;
@@ -1092,12 +1097,12 @@ cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int& occ, SweepP
 }
 template <int DIR, int GRAV, bool FLAT>
 cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ = 0;
+    static int occ[MAX_DEV] = {};
     return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, occ, P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ = 0;
+    static int occ[MAX_DEV] = {};
     return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR>, occ, P, sms, user_chunk, st);
 }
 template <int DIR>
