@@ -35,7 +35,7 @@ FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, 
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` capture
 # (profiles/), keyed by cells per side; None where no capture exists.
-NCU_TRAFFIC_BYTES = {512: 16.099e9}      # profiles/r1g_sweeps_ncu_full.md: 8.089 GB read + 8.010 GB written per launch
+NCU_TRAFFIC_BYTES = {512: 16.099e9}      # profiles/r1h_sweeps_ncu_full.md: 8.089 GB read + 8.010 GB written per launch
 
 
 def _peaks():
