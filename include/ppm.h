@@ -74,7 +74,8 @@ typedef struct {
  * Returns 0 for a non-positive extent.  Pure host arithmetic; needs no device. */
 size_t ppm_state_floats(int nx, int ny, int nz);
 
-/* Creates a context.  dev_buf_a, dev_buf_b: [device] two caller-owned buffers of
+/* Creates a context for one uniform Cartesian grid with its boundary types (L69: walls; periodic for
+ * the test problems), equation of state and gravity profile (L35).  dev_buf_a, dev_buf_b: [device] two caller-owned buffers of
  * ppm_state_floats(nx,ny,nz) floats each, 128-byte aligned (e.g. torch tensors).  The library BORROWS them for the
  * life of the context: the state lives in one, the other is sweep scratch, and they ping-pong.  It
  * never frees them.  Contents are undefined until ppm_set_state has covered every z-slab.  Every later call runs on
@@ -88,10 +89,12 @@ int ppm_create(ppm_ctx **out, const ppm_params *prm, float *dev_buf_a, float *de
  * SURVEY 8(c) C1).  Asynchronous w.r.t. the host only if the sources are device or pinned memory. */
 int ppm_set_state(ppm_ctx *ctx, const float *const fields[PPM_NFIELDS], int z0, int nz_slab, int src_is_device);
 
-/* Inverse of ppm_set_state; synchronises the stream before returning. */
+/* Inverse of ppm_set_state (full rho = rho0 + rho', p = p0 + p'); synchronises the stream before
+ * returning and reports the sticky state flag. */
 int ppm_get_state(ppm_ctx *ctx, float *const fields[PPM_NFIELDS], int z0, int nz_slab, int dst_is_device);
 
-/* One timestep = three 1-D sweeps (ghost fill, PPM hydro, PPB remap fused) with the same dt.
+/* One timestep = three 1-D sweeps (ghost fill, PPM hydro, PPB remap fused) with the same dt (PAPER.md L87
+ * "directionally split"; L27, L33, L35, L37, L51, L120).
  * sweep_order 0..5 = xyz, xzy, yxz, yzx, zxy, zyx.  Only enqueues work (3 kernel launches). */
 int ppm_step(ppm_ctx *ctx, double dt, int sweep_order);
 
@@ -106,10 +109,12 @@ int ppm_sweep(ppm_ctx *ctx, double dt, int axis);
  * translation), for which every sweep is volume preserving.  Only enqueues work (3 kernel launches). */
 int ppm_advect(ppm_ctx *ctx, double dt, int sweep_order);
 
-/* dt = cfl*dx / max over cells of max_d(|u_d|) + c.  Synchronises the stream.  dt_out: [host]. */
+/* dt = cfl*dx / max over cells of max_d(|u_d|) + c, c from the full rho, p (the scheme is explicit, PAPER.md L55;
+ * SURVEY 8(c) C6).  Synchronises the stream.  dt_out: [host].  PPM_ESTATE if a cell has non-positive rho or p. */
 int ppm_cfl_dt(ppm_ctx *ctx, double cfl, double *dt_out);
 
-/* out[6] [host] = mass, momentum x, y, z, total energy, tracked mass (sum rho*m000), each * dx^3;
+/* (BASELINE.json north_star: conservation to round-off on periodic boxes)
+ * out[6] [host] = mass, momentum x, y, z, total energy, tracked mass (sum rho*m000), each * dx^3;
  * fp64 accumulation in a fixed order (deterministic).  Synchronises the stream. */
 int ppm_reduce_conserved(ppm_ctx *ctx, double out[6]);
 
