@@ -74,6 +74,8 @@ __device__ constexpr int PPB_PERM[3][10] = {
 // local indices whose coefficient is odd in the normal direction (C3): a1, b1, c1 = 1, 4, 6
 
 __device__ __forceinline__ float sat(float x) { return __saturatef(x); }
+// streaming read that leaves the (small: L1 is carved out as shared memory) L1 to the gravity-table lines
+__device__ __forceinline__ float ld_noalloc(const float* p) { float v; asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
 __device__ __forceinline__ float med3(float a, float b, float c) { return fmaxf(fminf(a, b), fminf(fmaxf(a, b), c)); }
 __device__ __forceinline__ float rcp(float x) { return __fdividef(1.0f, x); }
 __device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
@@ -336,7 +338,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
     if (FLAT) {
         float sg;
         const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
-        fpre = __ldg(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+        fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
     }
 #pragma unroll MARCH_UNROLL
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
@@ -364,7 +366,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             ftn = fpre;                                              // F~_{n-2}, in flight since the last iteration
             float sg;
             const int jf = image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (the detector is mirror-invariant)
-            fpre = __ldg(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+            fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
         } else {
             const float d1 = pf[3] - pf[1], dd2 = pf[4] - pf[0];
             const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
