@@ -205,54 +205,76 @@ __device__ __forceinline__ int aux_image(int i, int n, int bc_lo, int bc_hi, flo
 constexpr int F3_T = 8, F3_H = 2, F3_W = F3_T + 2 * F3_H, F3_N = F3_W * F3_W * F3_W;
 __device__ __forceinline__ int f3_idx(int lx, int ly, int lz) { return ((lz + F3_H) * F3_W + (ly + F3_H)) * F3_W + (lx + F3_H); }
 
+// one point of the tile (d < 0) or of its arms (d = axis of the arm) -> shared memory.  INSIDE: the tile and its arms
+// lie wholly inside the grid (all but the boundary tiles): no image logic at all.
+template <bool INSIDE>
+__device__ __forceinline__ void f3_point(const AuxParams& A, const float* __restrict__ st, float* sP, float (*sU)[F3_N],
+                                         int ox0, int oy0, int oz0, int lx, int ly, int lz, int d, float& rc) {
+    int gx = ox0 + lx, gy = oy0 + ly, gz = oz0 + lz;
+    const int si = f3_idx(lx, ly, lz);
+    float sgn = 1.f;
+    bool ox = false, oy = false, oz = false;
+    if (!INSIDE) {
+        // A point outside the grid along ONE axis is the boundary image of a cell along that axis (an arm point
+        // by construction, a tile point when the tile overhangs a ragged grid); outside along two axes it is
+        // never anybody's neighbour.
+        ox = (unsigned)gx >= (unsigned)A.nx; oy = (unsigned)gy >= (unsigned)A.ny; oz = (unsigned)gz >= (unsigned)A.nz;
+        const int nout = (int)ox + (int)oy + (int)oz;
+        const int dout = ox ? 0 : (oy ? 1 : (oz ? 2 : d));
+        if (nout > 1 || (d >= 0 && nout == 1 && dout != d)) {
+            sP[si] = 1.f;
+            sU[0][si] = sU[1][si] = sU[2][si] = 0.f;
+            return;
+        }
+        if (ox) gx = aux_image(gx, A.nx, A.bc[0], A.bc[1], sgn);
+        if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
+        if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
+    }
+    const long long o = cell_offset(A, gx, gy, gz);
+    const float2 b0 = base32(A, gx, gy, gz);
+    sP[si] = b0.y + st[o + 4 * 64];
+    if (d < 0) {
+        rc = b0.x + st[o];
+        const float ux = st[o + 64], uy = st[o + 2 * 64], uz = st[o + 3 * 64];
+        sU[0][si] = ox ? sgn * ux : ux; sU[1][si] = oy ? sgn * uy : uy; sU[2][si] = oz ? sgn * uz : uz;
+    } else {
+        const float u = sgn * st[o + (1 + d) * 64];
+        if (d == 0) sU[0][si] = u; else if (d == 1) sU[1][si] = u; else sU[2][si] = u;
+    }
+}
+
+template <bool INSIDE>
+__device__ __forceinline__ void f3_fill(const AuxParams& A, const float* __restrict__ st, float* sP, float (*sU)[F3_N],
+                                        int ox0, int oy0, int oz0, float& rc) {
+    const int tid = threadIdx.x;
+    {   // the tile itself: thread = (brick in tile, cell in brick) -> coalesced brick reads
+        const int b = tid >> 6, c = tid & 63;
+        f3_point<INSIDE>(A, st, sP, sU, ox0, oy0, oz0, (b & 1) * 4 + (c & 3), ((b >> 1) & 1) * 4 + ((c >> 2) & 3), (b >> 2) * 4 + (c >> 4), -1, rc);
+    }
+    // the arms: 6 faces x 2 depths x 64 points = 768 points; a warp works on one (face, depth) slab half, so the
+    // axis and the side are warp-uniform
+    float dummy;
+    for (int r = tid; r < 6 * 2 * 64; r += 512) {
+        const int f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
+        const int d = f >> 1;
+        const int along = (f & 1) ? F3_T + h : -1 - h;
+        const int lx = (d == 0) ? along : (d == 1 ? bb : a);
+        const int ly = (d == 1) ? along : (d == 2 ? bb : a);
+        const int lz = (d == 2) ? along : (d == 0 ? bb : a);
+        f3_point<INSIDE>(A, st, sP, sU, ox0, oy0, oz0, lx, ly, lz, d, dummy);
+    }
+}
+
 __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const float* __restrict__ st, float* __restrict__ F3) {
     __shared__ float sP[F3_N], sU[3][F3_N];
     const int tid = threadIdx.x;
     const int org[3] = {(int)blockIdx.x * F3_T, (int)blockIdx.y * F3_T, (int)blockIdx.z * F3_T};
     const float gam = A.gamf;
     float rc = 1.f;
-    for (int idx = tid; idx < 512 + 6 * 2 * 64; idx += 512) {
-        int lx, ly, lz, d = -1;                // (scalars and selects only: a dynamically indexed l[3] would live in local memory)
-        if (idx < 512) {                       // the tile itself: thread = (brick in tile, cell in brick) -> coalesced brick reads
-            const int b = idx >> 6, c = idx & 63;
-            lx = (b & 1) * 4 + (c & 3); ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3); lz = (b >> 2) * 4 + (c >> 4);
-        } else {                               // the arms: axis d, side, depth h, position (a, bb) on the face
-            const int r = idx - 512, f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
-            d = f >> 1;
-            const int along = (f & 1) ? F3_T + h : -1 - h;
-            lx = (d == 0) ? along : (d == 1 ? bb : a);
-            ly = (d == 1) ? along : (d == 2 ? bb : a);
-            lz = (d == 2) ? along : (d == 0 ? bb : a);
-        }
-        int gx = org[0] + lx, gy = org[1] + ly, gz = org[2] + lz;
-        // A point outside the grid along ONE axis is the boundary image of a cell along that axis (an arm point
-        // by construction, a tile point when the tile overhangs a ragged grid); outside along two axes it is
-        // never anybody's neighbour.
-        const bool ox = (unsigned)gx >= (unsigned)A.nx, oy = (unsigned)gy >= (unsigned)A.ny, oz = (unsigned)gz >= (unsigned)A.nz;
-        const int nout = (int)ox + (int)oy + (int)oz;
-        const int dout = ox ? 0 : (oy ? 1 : (oz ? 2 : d));
-        const int si = f3_idx(lx, ly, lz);
-        if (nout > 1 || (d >= 0 && nout == 1 && dout != d)) {
-            sP[si] = 1.f;
-            sU[0][si] = sU[1][si] = sU[2][si] = 0.f;
-            continue;
-        }
-        float sgn = 1.f;
-        if (ox) gx = aux_image(gx, A.nx, A.bc[0], A.bc[1], sgn);
-        if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
-        if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
-        const long long o = cell_offset(A, gx, gy, gz);
-        const float2 b0 = base32(A, gx, gy, gz);
-        sP[si] = b0.y + st[o + 4 * 64];
-        if (d < 0) {
-            rc = b0.x + st[o];
-            const float ux = st[o + 64], uy = st[o + 2 * 64], uz = st[o + 3 * 64];
-            sU[0][si] = ox ? sgn * ux : ux; sU[1][si] = oy ? sgn * uy : uy; sU[2][si] = oz ? sgn * uz : uz;
-        } else {
-            const float u = st[o + (1 + d) * 64];
-            if (d == 0) sU[0][si] = sgn * u; else if (d == 1) sU[1][si] = sgn * u; else sU[2][si] = sgn * u;
-        }
-    }
+    const bool inside = org[0] >= F3_H && org[1] >= F3_H && org[2] >= F3_H &&
+                        org[0] + F3_T + F3_H <= A.nx && org[1] + F3_T + F3_H <= A.ny && org[2] + F3_T + F3_H <= A.nz;
+    if (inside) f3_fill<true>(A, st, sP, sU, org[0], org[1], org[2], rc);
+    else f3_fill<false>(A, st, sP, sU, org[0], org[1], org[2], rc);
     __syncthreads();
     const int b = tid >> 6, c = tid & 63;
     const int lx = (b & 1) * 4 + (c & 3), ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3), lz = (b >> 2) * 4 + (c >> 4);
