@@ -362,6 +362,76 @@ def test_degenerate_grids_2d_1d_and_fewer_cells_than_ghosts(dims):
     g.close()
 
 
+def _synthetic_gravity(kind, dims, dx, rng):
+    """a smooth, mildly stratified base state with its table (hand-made, not hydrostatically exact: the scheme must
+    agree with the oracle for ANY table; the residual just acts as a source)"""
+    nx, ny, nz = dims
+    if kind == 1:                                   # CONST_Z: nodes on every cell centre and face, ghosts included
+        n = 2 * (nz + 8) + 1
+        s0, ds = -4 * dx, 0.5 * dx
+        z = s0 + ds * np.arange(n)
+        center = (0.0, 0.0, 0.0)
+    else:                                           # RADIAL about an off-centre point
+        n = 257
+        s0, ds = 0.0, 2.0 * dx * max(dims) / (n - 1)
+        z = s0 + ds * np.arange(n)
+        center = (0.45 * nx * dx, 0.55 * ny * dx, 0.5 * nz * dx)
+    H = 2.0 * dx * max(dims)
+    rho0 = (1.0 + 0.5 * np.exp(-z / H)).astype(np.float32)
+    p0 = (0.8 + 0.4 * np.exp(-z / H)).astype(np.float32)
+    g = (-0.3 * np.exp(-z / H) * (np.tanh(z / (2 * dx)) if kind == 2 else 1.0)).astype(np.float32)
+    return dict(kind=kind, s0=float(s0), ds=float(ds), center=center, g=g, rho0=rho0, p0=p0)
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_small_grids_boundaries_gravity_and_paths(seed):
+    """randomised: extents 1..21 per axis (whole-brick and ragged axes mixed, so bulk-staged and direct sweeps mix in
+    one step), every boundary combination, no / constant-z / radial gravity tables, both flattening modes, random sweep
+    orders — against the oracle, and bulk-staged == direct bitwise."""
+    PPM = _gpu()
+    from oracle import binding as ob
+    from paper_1810_13416_b200.binding import OPT_FLATTEN3D, OPT_IO_PATH
+    rng = np.random.default_rng(1000 + seed)
+    pool = [1, 2, 3, 4, 5, 7, 8, 9, 12, 13, 16, 20, 21]
+    dims = tuple(int(rng.choice(pool)) for _ in range(3))
+    bc = []
+    for d in range(3):
+        refl = bool(rng.integers(0, 2)) and dims[d] >= 4
+        bc += [1, 1] if refl else [0, 0]
+    kind = int(rng.integers(0, 3))
+    dx = 0.05
+    grav = _synthetic_gravity(kind, dims, dx, rng) if kind else None
+    flat = int(rng.integers(0, 2))
+    nx, ny, nz = dims
+    f = np.zeros((15, nz, ny, nx), dtype=np.float32)
+    f[0] = 1.6 + 0.3 * rng.random((nz, ny, nx))
+    f[1:4] = 0.2 * rng.normal(size=(3, nz, ny, nx))
+    f[4] = 1.3 + 0.3 * rng.random((nz, ny, nx))
+    f[5] = 0.2 + 0.6 * rng.random((nz, ny, nx))
+    f[6:] = 0.02 * rng.normal(size=(9, nz, ny, nx))
+    orders = [int(rng.integers(0, 6)) for _ in range(3)]
+    o = ob.Oracle(nx, ny, nz, dx, 1.4, bc, grav)
+    o.set_flatten3d(bool(flat))
+    o.set_state(f)
+    res, dts = [], []
+    for io in (0, 1):
+        g = PPM(nx, ny, nz, dx, 1.4, bc, grav)
+        g.set_option(OPT_IO_PATH, io)
+        g.set_option(OPT_FLATTEN3D, flat)
+        g.set_state(f)
+        for k, order in enumerate(orders):
+            if io == 0:
+                dts.append(0.5 * g.cfl_dt(0.8))
+            g.step(dts[k], order)
+        res.append(g.get_state().cpu().numpy().astype(np.float64))
+        g.close()
+    assert np.array_equal(res[0], res[1]), (dims, bc, kind, flat)
+    for dt, order in zip(dts, orders):
+        o.step(dt, order)
+    e = max_rel(res[0], o.get_state())
+    assert max(e.values()) <= MULTI_STEP, (dims, bc, kind, flat, e)
+
+
 def test_state_flag_reports_floor_hits_and_bad_states():
     """error behaviour of the boundary (include/ppm.h): a step that drives the pressure to its floor, or a state with
     non-positive density, is reported as PPM_ESTATE by the next synchronising call; a new ppm_set_state clears it."""
