@@ -143,6 +143,12 @@ int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* 1 if the next sweep along axis (0,1,2) will take the bulk-staged path, 0 if the direct path. */
 int ppm_axis_path(const ppm_ctx *ctx, int axis);
 
+/* Host-side planning arithmetic of the bulk-staged sweeps, exposed for tests (needs no device): the sweeps march whole
+ * pencils while the pencil tiles fill complete waves of resident CTAs; the tail_tiles pencil tiles of the ragged last
+ * wave are cut into segments of this many cells (a multiple of 4, or n itself when cutting does not pay; 0 for
+ * non-positive arguments) so that the SMs run dry together.  Each cut costs 8 redundant warm-up cells. */
+int ppm_plan_tail_chunk(int tail_tiles, int resident_ctas, int n);
+
 /* Number of kernel launches the context has enqueued so far (bench.py reports it). */
 long long ppm_launch_count(const ppm_ctx *ctx);
 

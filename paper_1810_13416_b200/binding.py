@@ -22,7 +22,7 @@ GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
-           "ppm_state_floats", "ppm_destroy", "ppm_last_error")
+           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_destroy", "ppm_last_error")
 OPT_IO_PATH, OPT_FLATTEN3D = 2, 3
 
 
@@ -64,6 +64,7 @@ def lib():
         L.ppm_set_chunk.argtypes = [C.c_void_p, C.c_int]
         L.ppm_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.ppm_axis_path.argtypes = [C.c_void_p, C.c_int]
+        L.ppm_plan_tail_chunk.argtypes = [C.c_int, C.c_int, C.c_int]
         L.ppm_launch_count.argtypes = [C.c_void_p]
         L.ppm_launch_count.restype = C.c_longlong
         L.ppm_destroy.argtypes = [C.c_void_p]

@@ -263,4 +263,9 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
 
 extern "C" int ppm_axis_path(const ppm_ctx* c, int axis) { return (c && axis >= 0 && axis <= 2 && ppm_axis_is_bulk(c, axis)) ? 1 : 0; }
 
+extern "C" int ppm_plan_tail_chunk(int tail_tiles, int resident_ctas, int n) {
+    if (tail_tiles < 1 || resident_ctas < 1 || n < 1) return 0;
+    return ppm_tail_chunk(tail_tiles, resident_ctas, n);
+}
+
 extern "C" long long ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }

@@ -69,6 +69,7 @@ struct ppm_ctx {
 // launchers (defined in the .cu files)
 cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect = false);   // advect: PPB-only sweep (NEXT-2)
 bool ppm_axis_is_bulk(const ppm_ctx* c, int axis);
+int ppm_tail_chunk(int ntail, int slots, int n);   // segment length for the pencils of the ragged last wave
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs);
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs);
 cudaError_t ppm_launch_cfl(ppm_ctx* c);

@@ -1054,7 +1054,7 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_advect_bulk_
 
 // cells per segment for the tiles of the ragged last wave: the cut that minimises (waves of segments) x (segment
 // length + 8 warm-up cells); ntail tiles, slots resident CTAs, n cells per pencil
-static int tail_chunk(int ntail, int slots, int n) {
+int ppm_tail_chunk_impl(int ntail, int slots, int n) {
     int best = n;
     double best_t = 1e300;
     for (int np = 1; np <= 8; ++np) {
@@ -1091,7 +1091,7 @@ cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_
     } else {
         P.chunk = P.n;
         P.tiles_a = ntiles / slots * slots;                        // whole pencils while they fill complete waves
-        P.chunk_b = (P.tiles_a < ntiles) ? tail_chunk(ntiles - P.tiles_a, slots, P.n) : P.n;
+        P.chunk_b = (P.tiles_a < ntiles) ? ppm_tail_chunk_impl(ntiles - P.tiles_a, slots, P.n) : P.n;
     }
     const long long grid = (long long)P.tiles_a * ((P.n + P.chunk - 1) / P.chunk) + (long long)(ntiles - P.tiles_a) * ((P.n + P.chunk_b - 1) / P.chunk_b);
     kern<<<(unsigned)grid, G::WARPS * 32, G::SMEM, st>>>(P);
@@ -1135,6 +1135,8 @@ cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cu
 }
 
 }  // namespace
+
+int ppm_tail_chunk(int ntail, int slots, int n) { return ppm_tail_chunk_impl(ntail, slots, n); }
 
 bool ppm_axis_is_bulk(const ppm_ctx* c, int axis) {
     const int ext[3] = {c->prm.nx, c->prm.ny, c->prm.nz};

@@ -77,6 +77,24 @@ def test_state_floats_is_whole_brick_records(lib):
     assert L.ppm_state_floats(0, 8, 8) == 0 and L.ppm_state_floats(8, -1, 8) == 0
 
 
+def test_tail_segment_plan(lib):
+    """host logic of the sweep scheduling: the pencils of the ragged last wave are cut so that the wave fills the
+    resident CTA slots; a cut costs 8 warm-up cells"""
+    L = lib.lib()
+    slots = 148 * 3
+    assert L.ppm_plan_tail_chunk(2048 - 4 * slots, slots, 512) == 172        # 512^3: 272 tail tiles cut in three
+    assert L.ppm_plan_tail_chunk(0, slots, 512) == 0 and L.ppm_plan_tail_chunk(5, 0, 512) == 0
+    for tail in (1, 7, 100, 200, 272, 300, 443):
+        for n in (32, 100, 512, 1024):
+            ch = L.ppm_plan_tail_chunk(tail, slots, n)
+            nch = -(-n // ch)
+            assert (ch % 4 == 0 or ch == n) and 0 < ch <= max(n, 4) and (ch >= 32 or nch == 1)
+            cost = -(-tail * nch // slots) * (ch + (8 if nch > 1 else 0))   # waves of segments x segment length
+            assert cost <= n                                                 # never worse than marching whole pencils
+    # a tail that already fills the slots is not cut
+    assert L.ppm_plan_tail_chunk(slots - 1, slots, 512) == 512
+
+
 def test_null_context_calls_return_einval(lib):
     L = lib.lib()
     v = C.c_double()
