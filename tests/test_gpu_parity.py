@@ -577,8 +577,18 @@ def test_cfg4_full_512_windows():
                          ((c, 6, c), 24), ((6, 6, 6), 24)])
 
 
+def test_cfg4_full_512_all_20_steps_window():
+    """the headline config at its full size AND its full step count (BASELINE.json configs[3]: 512^3, 20 steps), in the
+    launch configuration bench.py times: one 32^3 window in the convective shell, oracle on the window plus its
+    80-cell apron (192^3 cells, 20 steps)."""
+    c = 256
+    _window_check(4, 20, [((c + 175, c, c), 32)], tol=MULTI_STEP)
+
+
 @pytest.mark.skipif(not torch.cuda.is_available() or torch.cuda.get_device_properties(0).total_memory < 150e9,
                     reason="1024^3 needs ~129 GB of HBM")
-def test_cfg5_full_1024_windows():
+def test_cfg5_full_1024_windows_all_5_steps():
+    """BASELINE.json configs[4]: 1024^3, all of its 5 steps; windows in the core, the shell, the FV edge and a corner"""
     c = 512
-    _window_check(5, 1, [((c, c, c), 24), ((c + 340, c, c), 24), ((c, c + int(0.45 * 1024), c), 24), ((6, 6, 6), 24)], nzs_load=8)
+    _window_check(5, 5, [((c, c, c), 24), ((c + 340, c, c), 24), ((c, c + int(0.45 * 1024), c), 24), ((6, 6, 6), 24)], nzs_load=8,
+                  tol=MULTI_STEP)
