@@ -17,11 +17,15 @@
  * with the CUDA path under paper_1810_13416_b200/csrc/ and neither includes the other.
  *
  * Pins (tests/test_oracle_*.py): every routine below is pinned against closed forms,
- * invariants, brute-force quadrature or a textbook exact Riemann solver.
+ * invariants, brute-force quadrature or a textbook exact Riemann solver; the gravity /
+ * base-state source terms (base_at, the H6 half-step sources, the H9 time-centred sources,
+ * the odd image of g behind a wall, table_lookup off the nodes) by free fall, split
+ * invariance, the energy budget and the doubled periodic box (tests/test_oracle_gravity.py).
  * PARITY UNPINNED (no PPMstar code or output exists to compare with): the *constants*
  * of the readings R3 (smoothness ramp 0.1..0.3), R5 (flattening 0.75/10/3/0.05),
- * R7 (5 Newton iterations), R13 (PPB bound B) and the choices R1/R11 — they are
- * constrained only by the invariants.
+ * R7 (5 Newton iterations), R13 (PPB bound B), the choices R1/R11 and the switch-free
+ * tracing R8' (its distance from the Colella-Woodward hard-switched tracing is measured
+ * in tests/test_oracle_r8prime.py) — they are constrained only by the invariants.
  *
  * Layout: 15 fields per cell, x fastest: 0 rho', 1 ux, 2 uy, 3 uz, 4 p',
  * 5..14 = m000 m100 m010 m001 m200 m020 m002 m110 m101 m011.

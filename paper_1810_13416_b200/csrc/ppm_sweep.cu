@@ -726,8 +726,10 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     const int t = threadIdx.x;
     const int ba = blockIdx.x * (PPM_CTA / 16) + (t >> 4), bb = blockIdx.y;
     const int a = ba * 4 + (t & 3), b = bb * 4 + ((t >> 2) & 3);
+    // the lanes that march: taken by a full-warp vote BEFORE the pad lanes leave (__activemask() after a divergent
+    // return need not equal the set of lanes that stay)
+    const unsigned wmask = __ballot_sync(0xffffffffu, a < P.na && b < P.nb);
     if (a >= P.na || b >= P.nb) return;
-    const unsigned wmask = __activemask();
     const int c0 = blockIdx.z * P.chunk;
     const int c1 = min(c0 + P.chunk, P.n);
     const long long tb = (long long)ba * P.SBa + (long long)bb * P.SBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)));
