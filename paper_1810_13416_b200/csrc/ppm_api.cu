@@ -116,6 +116,19 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
             t32[k] = make_float4(g.rho0[k], g.p0[k], g.g[k], 0.f);   // (rho0, p0) is an aligned pair for the packed lerp
             t64[3 * k] = g.g[k]; t64[3 * k + 1] = g.rho0[k]; t64[3 * k + 2] = g.p0[k];
         }
+        // interval records for the sweeps: the differences are taken in fp32, as the kernel's own subtraction would
+        std::vector<float4> tp(g.n);
+        std::vector<float2> tg(g.n);
+        auto ftz = [](float x) { return fabsf(x) < 1.17549435e-38f ? 0.0f : x; };
+        for (int k = 0; k < g.n; ++k) {
+            const int k1 = k + 1 < g.n ? k + 1 : k;
+            tp[k] = make_float4(g.rho0[k], g.p0[k], ftz(g.rho0[k1] - g.rho0[k]), ftz(g.p0[k1] - g.p0[k]));
+            tg[k] = make_float2(g.g[k], ftz(g.g[k1] - g.g[k]));
+        }
+        CUC(cudaMalloc(&c->tabp, sizeof(float4) * g.n));
+        CUC(cudaMalloc(&c->tabg, sizeof(float2) * g.n));
+        CUC(cudaMemcpy(c->tabp, tp.data(), sizeof(float4) * g.n, cudaMemcpyHostToDevice));
+        CUC(cudaMemcpy(c->tabg, tg.data(), sizeof(float2) * g.n, cudaMemcpyHostToDevice));
         CUC(cudaMalloc(&c->tab, sizeof(float4) * g.n));
         CUC(cudaMalloc(&c->tab64, sizeof(double) * 3 * g.n));
         CUC(cudaMemcpy(c->tab, t32.data(), sizeof(float4) * g.n, cudaMemcpyHostToDevice));
@@ -130,7 +143,7 @@ extern "C" void ppm_destroy(ppm_ctx* c) {
     if (!c) return;
     DevGuard guard(c);
     cudaFree(c->flag); cudaFree(c->cflmax); cudaFree(c->partial); cudaFree(c->result);
-    cudaFree(c->tab); cudaFree(c->tab64); cudaFree(c->F3);
+    cudaFree(c->tab); cudaFree(c->tabp); cudaFree(c->tabg); cudaFree(c->tab64); cudaFree(c->F3);
     free(c);
 }
 

@@ -32,11 +32,15 @@ struct SweepParams {
     int chunk;                      // cells marched per thread (pencil split along the sweep axis)
     float dt, dx, dtdx, inv_dx;
     float gamma, rho_floor, p_floor;
+    float gp, gmg, g_gm1, hdt;      // (gamma+1)/2, (gamma-1)/(2 gamma), gamma/(gamma-1), dt/2: kernel-argument constants cost no registers
     // gravity / base state
     int tab_n;
     float s0, inv_ds;
     float cen_d, cen_a, cen_b;      // RADIAL centre along (sweep, a, b) axes
     const float4* __restrict__ tab; // node k: {rho0, p0, g, 0}
+    // the same table as interval records, so that a lookup is one load per quantity: interval k (nodes k, k+1):
+    const float4* __restrict__ tabp; // {rho0_k, p0_k, rho0_k+1 - rho0_k, p0_k+1 - p0_k}
+    const float2* __restrict__ tabg; // {g_k, g_k+1 - g_k}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
     // 3-D flattening mode: F~ of every cell, [brick][4z][4y][4x] (a brick is 64 floats: strides = SB / 15); else NULL
     const float* flat;
@@ -50,6 +54,8 @@ struct ppm_ctx {
     cudaStream_t stream;
     int device;                     // the device that owns buf[0], buf[1]; every entry point switches to it
     float4* tab;                    // device gravity table (fp32 nodes)
+    float4* tabp;                   // device: interval records {rho0, p0, d rho0, d p0} (the sweeps' lookups)
+    float2* tabg;                   // device: interval records {g, d g}
     double* tab64;                  // device gravity table as doubles {g, rho0, p0} x n (set/get/reductions)
     int* flag;                      // device sticky flag
     unsigned int* cflmax;           // device: ordered-uint encoded max

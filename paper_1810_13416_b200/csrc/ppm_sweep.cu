@@ -37,10 +37,25 @@
 // adds increments to rho', p' instead of rebuilding them from E.
 #include <stdlib.h>
 
+#include <type_traits>
+
 #include "ppm_internal.h"
 
 #ifndef PPM_MARCH_UNROLL
 #define PPM_MARCH_UNROLL 1
+#endif
+// bulk path: cells of the steady-state marching loop per loop body (1, 2 or 4 = one brick with compile-time phases)
+#ifndef PPM_FAST_UNROLL
+#define PPM_FAST_UNROLL 1
+#endif
+// warp-uniform shortcuts past work whose outcome is known for every lane (no shock near, star state at the face,
+// Newton converged, PPB polynomial inside its bounds); a bit mask, 0 = always the general code (A/B knob)
+// carry 1/rho (and 1/c^2) down the pipeline instead of re-taking the reciprocals where they are needed (7 MUFU per cell)
+#ifndef PPM_CARRY_IRHO
+#define PPM_CARRY_IRHO 1
+#endif
+#ifndef PPM_UNIFORM_FAST
+#define PPM_UNIFORM_FAST 2      // bits: 1 flattening, 2 converged W_K, 4 star state, 8 PPB theta
 #endif
 // direct-path CTA shape (build knobs): threads per CTA (a multiple of 16 = one brick column; the kernel uses no
 // shared memory and no block-wide sync, so the CTA size only sets the granularity of occupancy) and the register
@@ -149,16 +164,29 @@ __device__ __forceinline__ int image_face(int f, int n, int bc_lo, int bc_hi) {
 // table node k: {rho0, p0, g, 0} — (rho0, p0) is an aligned pair
 struct Base { v2 rp; float g; };
 
-__device__ __forceinline__ Base table_at(const SweepParams& P, float s) {
-    float t = (s - P.s0) * P.inv_ds;
+// interval index and weight of table position s
+__device__ __forceinline__ int table_interval(const SweepParams& P, float s, float& w) {
+    const float t = (s - P.s0) * P.inv_ds;
     int k = (int)floorf(t);
     k = min(max(k, 0), P.tab_n - 2);
-    float w = t - (float)k;
-    float4 a = __ldg(P.tab + k), b = __ldg(P.tab + k + 1);
+    w = t - (float)k;
+    return k;
+}
+// one load per quantity: the interval records hold the node value and the difference to the next node
+__device__ __forceinline__ v2 table_rp(const SweepParams& P, float s) {
+    float w;
+    const int k = table_interval(P, s, w);
+    const float4 a = __ldg(P.tabp + k);
+    return fma2(bc(w), mk(a.z, a.w), mk(a.x, a.y));
+}
+__device__ __forceinline__ Base table_at(const SweepParams& P, float s) {
+    float w;
+    const int k = table_interval(P, s, w);
+    const float4 a = __ldg(P.tabp + k);
+    const float2 g = __ldg(P.tabg + k);
     Base o;
-    const v2 ra = mk(a.x, a.y), rb = mk(b.x, b.y);
-    o.rp = fma2(bc(w), rb - ra, ra);
-    o.g = fmaf(w, b.z - a.z, a.z);
+    o.rp = fma2(bc(w), mk(a.z, a.w), mk(a.x, a.y));
+    o.g = fmaf(w, g.y, g.x);
     return o;
 }
 
@@ -200,7 +228,7 @@ template <int DIR, int GRAV> struct Geo {
         } else if (GRAV == PPM_GRAV_RADIAL) {
             float xd = (float)f * P.dx - P.cen_d;
             float r2 = fmaf(xd, xd, t2);
-            o = table_at(P, fsqrt(r2)).rp;
+            o = table_rp(P, fsqrt(r2));
         }
         return o;
     }
@@ -311,8 +339,8 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
 template <int DIR, int GRAV, bool FLAT, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
                                       const bool valid, const unsigned wmask, const float* __restrict__ pflat) {
-    const float gam = P.gamma, gp = 0.5f * (gam + 1.0f), gmg = 0.5f * (gam - 1.0f) * rcp(gam), g_gm1 = gam * rcp(gam - 1.0f);
-    const float dtdx = P.dtdx, hdt = 0.5f * P.dt;
+    const float gam = P.gamma, gp = P.gp, gmg = P.gmg, g_gm1 = P.g_gm1;
+    const float dtdx = P.dtdx, hdt = P.hdt;
 
     Geo<DIR, GRAV> geo;
     geo.init(P, a, b);
@@ -329,6 +357,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
     float Flm = 0.f, Fln = 0.f, FlE = 0.f;                              // fluxes through the left face of cell n-4
     v2 FlB = bc(0.f);
     float ft0 = 0.f, ft1 = 0.f, cs = 1.f;
+    float irw[4] = {1.f, 1.f, 1.f, 1.f}, ic2s = 1.f;                    // 1/rho of cells n-5 .. n-2; 1/c^2 of cell n-3 (PPM_CARRY_IRHO)
     v2 b0fc = bc(0.f);                                                  // (rho0, p0) at the face being solved
     PpbCell mw[3];
 #pragma unroll
@@ -340,9 +369,13 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
         fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
     }
-#pragma unroll MARCH_UNROLL
-    for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
-        io.begin(n);
+    // One iteration of the pipeline.  phase = integral_constant<int, S>:
+    //   S = -1   any iteration: the brick phase n & 3, the boundary images and the pipeline-fill tests are run-time
+    //   S = 0..3 an iteration of the steady state (bulk path only): n & 3 == S is a compile-time constant, every cell
+    //            and face it touches lies inside the grid and the pipeline is full, so no image / fill logic remains
+    auto body = [&](const int n, auto phase) {
+        constexpr int S = decltype(phase)::value;
+        io.template begin<S>(n);
         // ---- shift windows, take plane n ---------------------------------------------------------------
 #pragma unroll
         for (int s = 0; s < 4; ++s) { q[s] = q[s + 1]; pf[s] = pf[s + 1]; gw[s] = gw[s + 1]; }
@@ -351,7 +384,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         {
             float sgn, v[5];
             int j;
-            io.hydro(n, j, sgn, v);
+            io.template hydro<S>(n, j, sgn, v);
             q[4].A = mk(v[0], v[4]); q[4].B = mk(v[2], v[3]); q[4].u = v[1];
             const Base bs = geo.cell(P, j, sgn);
             const v2 full = bs.rp + q[4].A;
@@ -360,38 +393,68 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             gw[4] = bs.g;
         }
         // ---- E, F: flattening ---------------------------------------------------------------------------
+#if PPM_CARRY_IRHO
+        // 1/rho is taken once per cell and carried (tracing and the PPB masses need it again), and c and 1/c^2 come
+        // from ONE reciprocal square root: c = x rsqrt(x), 1/c^2 = rsqrt(x)^2 with x = gamma p / rho
+#pragma unroll
+        for (int s = 0; s < 3; ++s) irw[s] = irw[s + 1];
+        irw[3] = rcp(rf[3]);
+        const float xc = gam * pf[2] * irw[3];
+        const float icn = rsqrtf(fmaxf(xc, 1e-37f));
+        const float cn2 = xc * icn;                                  // c_{n-2}
+        const float ic2n = icn * icn;
+#else
         const float cn2 = fsqrt(gam * pf[2] * rcp(rf[3]));          // c_{n-2}
+#endif
         float ftn;
         if (FLAT) {
             ftn = fpre;                                              // F~_{n-2}, in flight since the last iteration
             float sg;
-            const int jf = image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (the detector is mirror-invariant)
+            const int jf = (S >= 0) ? n - 1 : image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (the detector is mirror-invariant)
             fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
         } else {
-            const float d1 = pf[3] - pf[1], dd2 = pf[4] - pf[0];
-            const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
-            const float jump = sat(fdiv(3.0f * fabsf(d1), fminf(pf[3], pf[1])) - 1.0f);
-            const float conv = sat(fdiv(q[1].u - q[3].u, 0.05f * cn2));
-            ftn = steep * jump * conv;
+            // The jump ramp clamp(3|d1|/min(p) - 1) is zero wherever the pressure changes by less than a third over two
+            // cells: everywhere but in strong shocks.  When no lane of the warp is near one, f~ = 0 without the three
+            // divisions (a warp-uniform shortcut: the result is the same zero the ramps would give).
+            const float d1 = pf[3] - pf[1];
+            const float pm = fminf(pf[3], pf[1]);
+            ftn = 0.f;
+            if (!(PPM_UNIFORM_FAST & 1) || !__all_sync(wmask, 3.0f * fabsf(d1) <= pm || !valid)) {
+                const float dd2 = pf[4] - pf[0];
+                const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
+                const float jump = sat(fdiv(3.0f * fabsf(d1), pm) - 1.0f);
+                const float conv = sat(fdiv(q[1].u - q[3].u, 0.05f * cn2));
+                ftn = steep * jump * conv;
+            }
         }
         const float fl3 = fmaxf(ft0, fmaxf(ft1, ftn));              // f_{n-3}
+        // no flattening anywhere in the warp (every smooth flow): the parabola is used as it is — f (q - L) + L with
+        // f = 0 is L bit for bit, so skipping the blend changes nothing
+        const bool noflat = (PPM_UNIFORM_FAST & 1) && __all_sync(wmask, fl3 == 0.f || !valid);
         // ---- G, H: flattened parabola and characteristic tracing of cell n-3 ---------------------------
         // Each traced quantity is a pair W = (left of face (n-3)+1/2, right of face (n-3)-1/2): the two states
         // are mirror images, F+ and F- differ only in the sign of the q6 term.
         v2 Wr, Wu, Wp, Wv, Ww;
         v2 b0fn;
         {
-            const int fi = image_face(n - 2, P.n, P.bc_lo, P.bc_hi);
+            const int fi = (S >= 0) ? n - 2 : image_face(n - 2, P.n, P.bc_lo, P.bc_hi);
             b0fn = geo.face(P, fi);
         }
         {
             const V5 qc = q[1];
-            const V5 L = fma5(qc - parL, fl3, parL);
-            const V5 R = fma5(qc - parR, fl3, parR);
+            V5 L = parL, R = parR;
+            if (!noflat) {
+                L = fma5(qc - parL, fl3, parL);
+                R = fma5(qc - parR, fl3, parR);
+            }
             const V5 dq = R - L;
             const V5 q6 = fma5(L + R, -3.0f, qc * 6.0f);
             const float rho = rf[2], c = cs, u = qc.u;
+#if PPM_CARRY_IRHO
+            const float c2 = c * c, rc = rho * c, ic2 = ic2s, ic2h = 0.5f * ic2, cor = c * irw[2];
+#else
             const float c2 = c * c, rc = rho * c, ic2 = rcp(c2), ic2h = 0.5f * ic2, cor = fdiv(c, rho);
+#endif
             const float s_m = (u - c) * dtdx, s_0 = u * dtdx, s_p = (u + c) * dtdx;
             // Each wave family k takes its amplitude from its own domain of dependence max(+-sigma^k, 0); a
             // wave moving away from the face has the zero-width domain, i.e. the edge value (reading R8',
@@ -427,7 +490,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (GRAV != PPM_GRAV_NONE) {   // half-step sources of the perturbation equations (H6)
                 const v2 db = b0fn - b0fc;
                 const float k = -hdt * u * P.inv_dx;
+#if PPM_CARRY_IRHO
+                const float su = hdt * gw[1] * (qc.A.x * irw[2]);
+#else
                 const float su = hdt * gw[1] * fdiv(qc.A.x, rho);
+#endif
                 Wr = Wr + bc(k * db.x); Wp = Wp + bc(k * db.y); Wu = Wu + bc(su);
             }
         }
@@ -462,10 +529,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // Newton on p*' with the two-shock wave speeds W_K; at most 5 iterations (reading R7).  The loop
             // stops early only when EVERY lane's last update is below fp32 resolution of p* (warp-uniform
             // exit), i.e. when further iterations could not change the result beyond rounding.
+            v2 w2, iw;                                                        // W_K^2 and 1/W_K of the latest iteration
             auto newton = [&]() -> bool {
                 const float ps = p0f + pps;
-                const v2 w2 = fma2(gpr, bc(ps), gmr);
-                const v2 iw = mk(rsqrtf(w2.x), rsqrtf(w2.y));
+                w2 = fma2(gpr, bc(ps), gmr);
+                iw = mk(rsqrtf(w2.x), rsqrtf(w2.y));
                 const v2 us = fma2(np(bc(pps) - pp), iw, Zu);               // u*_L = uL - (p*-pL)/W_L, u*_R = uR + (p*-pR)/W_R
                 const v2 iz = (w2 + C2) * ((iw * iw) * iw);                   // 1/Z_K = (W^2 + C^2) / (2 W^3), times 2
                 const float d = fdiv(2.0f * (us.y - us.x), hsum(iz));
@@ -475,14 +543,21 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // first iteration in straight-line code (the scheduler can overlap it with independent work); the
             // remaining ones only while some lane still moves (rare at low Mach: the acoustic guess is nearly exact)
             // (lanes on pad cells of a ragged grid carry garbage and do not vote)
-            if (!__all_sync(wmask, newton() || !valid)) {
+            bool conv = __all_sync(wmask, newton() || !valid);
+            if (!conv) {
 #pragma unroll 1
                 for (int it = 1; it < 5; ++it)
-                    if (__all_sync(wmask, newton() || !valid)) break;
+                    if ((conv = __all_sync(wmask, newton() || !valid))) break;
             }
             const float ps = p0f + pps;
-            const v2 w2 = fma2(gpr, bc(ps), gmr);
-            const v2 Ws = w2 * mk(rsqrtf(fmaxf(w2.x, 1e-37f)), rsqrtf(fmaxf(w2.y, 1e-37f)));
+            // "then recompute W_K" at the final p* (H7).  After a converged iteration p* moved by less than one fp32
+            // rounding of itself, so W_K of that iteration IS W_K(p*) to rounding: it is reused.  Only when the
+            // iteration cap ended the loop (strong shocks) is it evaluated again.
+            if (!(PPM_UNIFORM_FAST & 2) || !conv) {
+                w2 = fma2(gpr, bc(ps), gmr);
+                iw = mk(rsqrtf(fmaxf(w2.x, 1e-37f)), rsqrtf(fmaxf(w2.y, 1e-37f)));
+            }
+            const v2 Ws = w2 * iw;
             const float us = fdiv(hsum(Ws * Zu) + (pp.x - pp.y), hsum(Ws));
             // sampling at x/t = 0 in the frame mirrored so that the upwind side K is on the left
             const bool left = us >= 0.f;
@@ -492,16 +567,24 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const v2 vw = mk(left ? WLv : Wv.y, left ? WLw : Ww.y);
             float rs = fdiv(rK * wk2, wk2 - rK * (pps - ppK));                 // 1/(1/rK - (p*-pK)/WK^2)
             rs = fmaxf(rs, P.rho_floor);
-            const float irK = rcp(rK);
-            const float cK = fsqrt(gam * pK * irK), cst = fsqrt(gam * ps * rcp(rs));
             const float uKh = sg * uK, ush = sg * us;
             const bool shock = pps > ppK;
-            const float lam_head = uKh - (shock ? WK * irK : cK);
-            const float lam_tail = shock ? lam_head : ush - cst;
-            const float th = (lam_head >= 0.f) ? 0.f : ((lam_tail <= 0.f) ? 1.f : fdiv(-lam_head, lam_tail - lam_head));
-            const float rh = fmaf(th, rs - rK, rK);
-            const float uh = fmaf(th, us - uK, uK);
-            const float pph = fmaf(th, pps - ppK, ppK);
+            // The face lies in the star region (theta = 1) when the upwind wave runs upwind: a shock with
+            // u_K - W_K/rho_K < 0, or a fan whose head u_K - c_K AND tail u* - c*_K are negative — every face of a
+            // subsonic flow.  Written without the two sound speeds (u^2 rho < gamma p), and when it holds for every lane
+            // of the warp the sampled state is the star state itself.
+            const bool star = shock ? (uKh * rK < WK) : ((uKh < 0.f || uKh * uKh * rK < gam * pK) && ush * ush * rs <= gam * ps);
+            float rh = rs, uh = us, pph = pps;
+            if (!(PPM_UNIFORM_FAST & 4) || !__all_sync(wmask, star || !valid)) {
+                const float irK = rcp(rK);
+                const float cK = fsqrt(gam * pK * irK), cst = fsqrt(gam * ps * rcp(rs));
+                const float lam_head = uKh - (shock ? WK * irK : cK);
+                const float lam_tail = shock ? lam_head : ush - cst;
+                const float th = (lam_head >= 0.f) ? 0.f : ((lam_tail <= 0.f) ? 1.f : fdiv(-lam_head, lam_tail - lam_head));
+                rh = fmaf(th, rs - rK, rK);
+                uh = fmaf(th, us - uK, uK);
+                pph = fmaf(th, pps - ppK, ppK);
+            }
             const float ph = p0f + pph;
             const float Fm = rh * uh;
             Frm = Fm;
@@ -511,30 +594,38 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         }
         // ---- K (first half): PPB coefficients of cell n-3, pre-limited (P2) ---------------------------
         mw[0] = mw[1]; mw[1] = mw[2];
-        if (n - 3 >= c0 - 1) {
+        if (S >= 0 || n - 3 >= c0 - 1) {
             float m[10];
-            io.ppb(n - 3, m);
+            io.template ppb<S>(n - 3, m);
             // bound B: first-order terms 1/2, pure second-order 1/6, mixed 1/4.
             // local order: a1,b0,c0 are P1 terms; a2,d0,e0 are P2 terms; b1,c1,f0 are mixed P1P1 terms.
             const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
             const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
             const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
-            const float th = fminf(1.0f, fdiv(fmaxf(0.f, fminf(m[0], 1.0f - m[0])), fmaxf(B, PPM_TINY)));
+            // theta = min(1, max(0, min(m000, 1 - m000)) / B): 1 wherever the bound B already fits (the constraint is
+            // "almost never performed") — then the coefficients are taken as they are
+            const float room = fmaxf(0.f, fminf(m[0], 1.0f - m[0]));
             // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
             asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
-            mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
-            mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
+            if ((PPM_UNIFORM_FAST & 8) && __all_sync(wmask, B <= room || !valid)) {
+                mw[2].a1 = m[1]; mw[2].a2 = m[2]; mw[2].f = m[9];
+                mw[2].bc0 = bc0; mw[2].bc1 = bc1; mw[2].de = de;
+            } else {
+                const float th = (B <= room) ? 1.0f : fdiv(room, fmaxf(B, PPM_TINY));
+                mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+                mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
+            }
             io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
         }
         // ---- J, K, L: finish cell n-4 ---------------------------------------------------------------------
         const int i = n - PPM_NGHOST;
-        if (i >= c0) {
+        if (S >= 0 || i >= c0) {
             // the cell's old values: the bulk path still has them in shared memory (its results overwrite them below),
             // so the register window need not carry them for four iterations
             V5 qo = q[0];
             if (IO::HAS_OLD) {
                 float v[5];
-                io.old_hydro(i, v);
+                io.template old_hydro<S>(i, v);
                 qo.A = mk(v[0], v[4]); qo.B = mk(v[2], v[3]); qo.u = v[1];
             }
             const float r_old = rf[1], rp_old = qo.A.x, pp_old = qo.A.y, u0 = qo.u, g = gw[0];
@@ -562,15 +653,57 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
+#if PPM_CARRY_IRHO
+            ppb_remap(mw, irw[0], irw[1], irw[2], r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+#else
             ppb_remap(mw, rcp(rf[0]), rcp(rf[1]), rcp(rf[2]), r_new, irn, dtdx * Flm, dtdx * Frm, mo);
-            io.store(i, ho, mo);
+#endif
+            io.template store<S>(i, ho, mo);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
         d2a = d2b; d2b = d2n; Fc = Fn; Fcl = Fnl; parL = pLn; parR = pRn;
         WLr = Wr.x; WLu = Wu.x; WLp = Wp.x; WLv = Wv.x; WLw = Ww.x;
         Flm = Frm; Fln = Frn; FlE = FrE; FlB = FrB;
         ft0 = ft1; ft1 = ftn; cs = cn2; b0fc = b0fn;
-        io.end(n);
+#if PPM_CARRY_IRHO
+        ic2s = ic2n;
+#endif
+    };
+    using std::integral_constant;
+    if (IO::HAS_FAST) {
+        // bulk path: c0, c1 are multiples of 4.  Ghost bricks and pipeline fill [c0 - 4, c0 + 4) and the drain
+        // [c1, c1 + 4) run the generic body (ONE copy of it: the two passes of the outer loop); the bricks in between
+        // run the steady-state body, unrolled over the four cells of a brick — the sliding windows become register
+        // renaming and the brick-phase logic constant-folds.
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            const int lo = pass ? c1 : c0 - PPM_NGHOST, hi = pass ? c1 + PPM_NGHOST : c0 + 4;
+#pragma unroll 1
+            for (int n = lo; n < hi; ++n) body(n, integral_constant<int, -1>());
+            if (pass == 0) {
+#if PPM_FAST_UNROLL == 4
+#pragma unroll 1
+                for (int n = c0 + 4; n < c1; n += 4) {
+                    body(n, integral_constant<int, 0>());
+                    body(n + 1, integral_constant<int, 1>());
+                    body(n + 2, integral_constant<int, 2>());
+                    body(n + 3, integral_constant<int, 3>());
+                }
+#elif PPM_FAST_UNROLL == 2
+#pragma unroll 1
+                for (int n = c0 + 4; n < c1; n += 2) {
+                    body(n, integral_constant<int, 4>());
+                    body(n + 1, integral_constant<int, 4>());
+                }
+#else
+#pragma unroll 1
+                for (int n = c0 + 4; n < c1; ++n) body(n, integral_constant<int, 4>());
+#endif
+            }
+        }
+    } else {
+#pragma unroll MARCH_UNROLL
+        for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) body(n, integral_constant<int, -1>());
     }
     io.finish();
 }
@@ -592,20 +725,20 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
     for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
 #pragma unroll 1
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
-        io.begin(n);
+        io.template begin<-1>(n);
 #pragma unroll
         for (int s = 0; s < 4; ++s) uw[s] = uw[s + 1];
         {
             float sgn, v[5];
             int j;
-            io.hydro(n, j, sgn, v);
+            io.template hydro<-1>(n, j, sgn, v);
             uw[4] = v[1];
         }
         const float Frm = 0.5f * (uw[0] + uw[1]);           // face (n-4)+1/2
         mw[0] = mw[1]; mw[1] = mw[2];
         if (n - 3 >= c0 - 1) {
             float m[10];
-            io.ppb(n - 3, m);
+            io.template ppb<-1>(n - 3, m);
             const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
             const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
             const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
@@ -620,10 +753,9 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
             float mo[10];
             const float rn = 1.0f - dtdx * (Frm - Flm);
             ppb_remap(mw, 1.0f, 1.0f, 1.0f, rn, rcp(fmaxf(rn, PPM_TINY)), dtdx * Flm, dtdx * Frm, mo);
-            io.store_ppb(i, mo);
+            io.template store_ppb<-1>(i, mo);
         }
         Flm = Frm;
-        io.end(n);
     }
     io.finish();
 }
@@ -637,7 +769,8 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
 template <int DIR>
 struct IoDirect {
     static constexpr bool HAS_OLD = false;   // no staged copy of a cell's old values: march() carries them in registers
-    __device__ __forceinline__ void old_hydro(int, float (&)[5]) {}
+    static constexpr bool HAS_FAST = false;  // no steady-state body: any extent, any segment bounds
+    template <int S> __device__ __forceinline__ void old_hydro(int, float (&)[5]) {}
     static constexpr int SH = 2 * DIR;       // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
     const float* __restrict__ const pin;     // the thread's pencil: cell 0 of the sweep axis, field 0
@@ -663,8 +796,8 @@ struct IoDirect {
         nx5[3] = __ldg(p + 64 * Dir<DIR>::W);
         nx5[4] = __ldg(p + 64 * 4);
     }
-    __device__ __forceinline__ void begin(int) {}
-    __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
+    template <int S> __device__ __forceinline__ void begin(int) {}
+    template <int S> __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
         j = jn; sgn = sn;
 #pragma unroll
         for (int k = 0; k < 5; ++k) v[k] = nx5[k];
@@ -677,7 +810,7 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
     }
-    __device__ __forceinline__ void ppb(int, float (&m)[10]) {
+    template <int S> __device__ __forceinline__ void ppb(int, float (&m)[10]) {
 #pragma unroll
         for (int k = 0; k < 10; ++k) m[k] = nm[k];
         m[1] *= snm; m[4] *= snm; m[6] *= snm;
@@ -694,7 +827,7 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
     }
-    __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
+    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
         float* __restrict__ p = pout + off(i);
         p[0] = h[0];
         p[64 * Dir<DIR>::U] = h[1];
@@ -705,7 +838,7 @@ struct IoDirect {
         for (int k = 0; k < 10; ++k) p[64 * (5 + PPB_PERM[DIR][k])] = m[k];
     }
     // PPB-only sweep: the hydro fields of the cell are copied through unchanged
-    __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
+    template <int S> __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
         const long long o = off(i);
         float* __restrict__ p = pout + o;
         const float* __restrict__ q = pin + o;
@@ -714,7 +847,6 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) p[64 * (5 + PPB_PERM[DIR][k])] = m[k];
     }
-    __device__ __forceinline__ void end(int) {}
     __device__ __forceinline__ void finish() {}
 };
 
@@ -873,20 +1005,23 @@ struct IoBulk {
         mbar_wait(bar + j, (ph >> j) & 1);
         ph ^= 1u << j;
     }
-    __device__ __forceinline__ void begin(int n) {
-        const int s = n & 3;
+    // S = -1: run-time brick phase, ghost bricks and segment ends handled.  S = 0..3: steady state — n & 3 == S, the
+    // bricks in play are interior bricks that are neither the first nor the last of the segment (march()).
+    template <int S> __device__ __forceinline__ void begin(int n) {
+        const int s = (S >= 0 && S < 4) ? S : (n & 3);
         if (s == 0) {                                          // a new hydro brick k comes up; results of brick k - 1 start
             const int k = n >> 2;
             pst = pcur;                                        // PPB brick k - 1 is the one being read since n - 1
             hprv = hcur;
-            if (k != k0) {
+            if (S >= 0 || k != k0) {
                 hs = (hs == G::NH - 1) ? 0 : hs + 1;
                 hcur = hs * G::HSLOT;
             } else {
                 chunk_brick(k0, prev);                         // the very first PPB cell (c0 - 1) is the last cell of brick k0
                 wait_slot(G::NH);
             }
-            jb = chunk_brick(k, hrev) * 4;
+            if (S >= 0) { jb = n; hrev = 0; }
+            else jb = chunk_brick(k, hrev) * 4;
             wait_slot(hs);
         } else if (s == 1) {
             // ring refill, once per brick, one full iteration after brick k - 2 was shipped (so its bulk stores have
@@ -894,25 +1029,36 @@ struct IoBulk {
             // (receiving results) in hs - 1, so the dead hydro slot is hs + 1 (mod 3); the PPB brick being read is
             // k - 1 in slot ps, the dead one is ps ^ 1.
             const int k = n >> 2;
-            if (k != k0) {
+            if (S >= 0 || k != k0) {
                 __syncwarp();
                 if (lane == 0) {
                     tma_wait_read0();
-                    if (k + 1 >= k0 + G::NH && k + 1 <= kend) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
-                    if (k >= k0 + G::NP && k <= kend) issue_ppb(k, ps ^ 1);
+                    if (S >= 0 || (k + 1 >= k0 + G::NH && k + 1 <= kend)) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
+                    if (S >= 0 || (k >= k0 + G::NP && k <= kend)) issue_ppb(k, ps ^ 1);
                 }
             }
         } else if (s == 3) {                                   // PPB cell c = n - 3 is the first of brick c >> 2
             const int k = (n - 3) >> 2;
-            if (k > k0) {
+            if (S >= 0 || k > k0) {
                 ps ^= 1;
                 pcur = ps * G::PSLOT;
-                chunk_brick(k, prev);
+                if (S >= 0) prev = 0; else chunk_brick(k, prev);
                 wait_slot(G::NH + ps);
             }
         }
     }
-    __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
+    template <int S> __device__ __forceinline__ void hydro(int n, int& j, float& sgn, float (&v)[5]) {
+        if (S >= 0) {                                          // interior brick, cells in order
+            sgn = 1.0f;
+            j = n;
+            const float* src = hyd + hcur + (((S < 4) ? S : (n & 3)) << SH);
+            v[0] = src[0];
+            v[1] = src[64 * Dir<DIR>::U];
+            v[2] = src[64 * Dir<DIR>::V];
+            v[3] = src[64 * Dir<DIR>::W];
+            v[4] = src[64 * 4];
+            return;
+        }
         const int s = (n & 3) ^ hrev;
         sgn = hrev ? -1.0f : 1.0f;
         j = jb + s;
@@ -924,18 +1070,19 @@ struct IoBulk {
         v[3] = src[64 * Dir<DIR>::W];
         v[4] = src[64 * 4];
     }
-    __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
-        const int s = (c & 3) ^ prev;
+    template <int S> __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
+        const int s = (S >= 0 && S < 4) ? ((S + 1) & 3) : ((S == 4) ? (c & 3) : ((c & 3) ^ prev));      // c = n - 3
         const float* src = ppr + pcur + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) m[q] = src[64 * PPB_PERM[DIR][q]];
-        if (prev) { m[1] = -m[1]; m[4] = -m[4]; m[6] = -m[6]; }   // odd coefficients under the mirror (warp-uniform, rare)
+        if (S < 0 && prev) { m[1] = -m[1]; m[4] = -m[4]; m[6] = -m[6]; }   // odd coefficients under the mirror (warp-uniform, rare)
     }
     __device__ __forceinline__ void ppb_prefetch(int, const PpbCell&) {}
     static constexpr bool HAS_OLD = true;
+    static constexpr bool HAS_FAST = true;
     // the hydro input of interior cell i, still in its slot when the cell is finished (n = i + 4)
-    __device__ __forceinline__ void old_hydro(int i, float (&v)[5]) {
-        const float* src = hyd + hprv + ((i & 3) << SH);
+    template <int S> __device__ __forceinline__ void old_hydro(int i, float (&v)[5]) {
+        const float* src = hyd + hprv + (((S >= 0 && S < 4) ? S : (i & 3)) << SH);
         v[0] = src[0];
         v[1] = src[64 * Dir<DIR>::U];
         v[2] = src[64 * Dir<DIR>::V];
@@ -943,19 +1090,19 @@ struct IoBulk {
         v[4] = src[64 * 4];
     }
     // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
-    __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
-        const int s = i & 3;
+    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
+        const int s = (S >= 0 && S < 4) ? S : (i & 3);         // i = n - 4
         float* dh = hyd + hprv + (s << SH);
         dh[0] = h[0];
         dh[64 * Dir<DIR>::U] = h[1];
         dh[64 * Dir<DIR>::V] = h[2];
         dh[64 * Dir<DIR>::W] = h[3];
         dh[64 * 4] = h[4];
-        store_ppb(i, m);
+        store_ppb<S>(i, m);
     }
     // PPB part of cell i only (PPB-only sweep: the hydro slot goes back to global memory as it came in)
-    __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
-        const int s = i & 3;
+    template <int S> __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
+        const int s = (S >= 0 && S < 4) ? S : (i & 3);
         float* dp = ppr + pst + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
@@ -976,7 +1123,6 @@ struct IoBulk {
             }
         }
     }
-    __device__ __forceinline__ void end(int) {}
     __device__ __forceinline__ void finish() {
         if (lane == 0) tma_wait_all0();                        // smem must outlive the last bulk store
         __syncwarp();
@@ -1014,7 +1160,9 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sm = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (the shuffle tells the compiler that the warp index is warp-uniform: ring addresses, mbarriers and the bulk-copy
+    // operands then live in uniform registers and the copies are issued without a lane-election loop)
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
     bulk_init_barriers<DIR>(bars);
     const int nba = (P.na + 3) >> 2;
     const int ntx = (nba + 2 * G::WARPS - 1) / (2 * G::WARPS);    // tiles along a
@@ -1040,7 +1188,9 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_advect_bulk_
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sm = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // (the shuffle tells the compiler that the warp index is warp-uniform: ring addresses, mbarriers and the bulk-copy
+    // operands then live in uniform registers and the copies are issued without a lane-election loop)
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
     bulk_init_barriers<DIR>(bars);
     const int nba = (P.na + 3) >> 2;
     const int ntx = (nba + 2 * G::WARPS - 1) / (2 * G::WARPS);
@@ -1112,16 +1262,25 @@ cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStre
 template <int DIR>
 cudaError_t launch_bulk_dir(SweepParams& P, int grav, int sms, int user_chunk, cudaStream_t st) {
     const bool fl = P.flat != nullptr;
+#ifdef PPM_EXP_ONE   // experiment builds: only the radial-gravity bulk sweeps are instantiated (fast compile; bench config 4/5 only)
+    (void)fl; (void)grav;
+    return launch_bulk<DIR, PPM_GRAV_RADIAL, false>(P, sms, user_chunk, st);
+#else
     switch (grav) {
         case PPM_GRAV_NONE: return fl ? launch_bulk<DIR, PPM_GRAV_NONE, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_NONE, false>(P, sms, user_chunk, st);
         case PPM_GRAV_CONST_Z: return fl ? launch_bulk<DIR, PPM_GRAV_CONST_Z, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_CONST_Z, false>(P, sms, user_chunk, st);
         default: return fl ? launch_bulk<DIR, PPM_GRAV_RADIAL, true>(P, sms, user_chunk, st) : launch_bulk<DIR, PPM_GRAV_RADIAL, false>(P, sms, user_chunk, st);
     }
+#endif
 }
 
 template <int DIR>
 cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cudaStream_t st) {
     const bool fl = P.flat != nullptr;
+#ifdef PPM_EXP_ONE
+    (void)fl; (void)grav; (void)grid; (void)block; (void)st; (void)P;
+    return cudaErrorNotSupported;
+#else
     switch (grav) {
         case PPM_GRAV_NONE:
             if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_NONE, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_NONE, false><<<grid, block, 0, st>>>(P);
@@ -1134,6 +1293,7 @@ cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cu
             break;
     }
     return cudaGetLastError();
+#endif
 }
 
 }  // namespace
@@ -1166,9 +1326,10 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect) {
     P.chunk = chunk;
     P.dt = (float)dt; P.dx = (float)p.dx; P.dtdx = (float)(dt / p.dx); P.inv_dx = (float)(1.0 / p.dx);
     P.gamma = (float)p.gamma; P.rho_floor = (float)p.rho_floor; P.p_floor = (float)p.p_floor;
+    P.gp = (float)(0.5 * (p.gamma + 1.0)); P.gmg = (float)(0.5 * (p.gamma - 1.0) / p.gamma); P.g_gm1 = (float)(p.gamma / (p.gamma - 1.0)); P.hdt = (float)(0.5 * dt);
     P.tab_n = p.grav.n; P.s0 = (float)p.grav.s0; P.inv_ds = (float)(p.grav.kind != PPM_GRAV_NONE ? 1.0 / p.grav.ds : 0.0);
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
-    P.tab = c->tab;
+    P.tab = c->tab; P.tabp = c->tabp; P.tabg = c->tabg;
     P.flag = c->flag;
     P.flat = c->flat3d ? c->F3 : nullptr;
     P.FBd = P.SBd / PPM_NFIELDS; P.FBa = P.SBa / PPM_NFIELDS; P.FBb = P.SBb / PPM_NFIELDS;
@@ -1178,22 +1339,28 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect) {
     if (use_bulk) {
         P.ntiles = ((nba + 7) / 8) * nbb;                                     // CTA tile = 4 warps x 2 brick columns along a
         const int uc = c->chunk > 0 ? chunk : 0;                              // 0: whole pencils, the last wave cut to finish together
+#ifndef PPM_EXP_ONE
         if (advect) {
             if (axis == 0) e = launch_advect_bulk<0>(P, c->sms, uc, c->stream);
             else if (axis == 1) e = launch_advect_bulk<1>(P, c->sms, uc, c->stream);
             else e = launch_advect_bulk<2>(P, c->sms, uc, c->stream);
-        } else if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
+        } else
+#endif
+        if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
         else if (axis == 1) e = launch_bulk_dir<1>(P, p.grav.kind, c->sms, uc, c->stream);
         else e = launch_bulk_dir<2>(P, p.grav.kind, c->sms, uc, c->stream);
     } else {
         dim3 block(PPM_CTA, 1, 1);
         dim3 grid((nba + PPM_CTA / 16 - 1) / (PPM_CTA / 16), nbb, nchunks);
+#ifndef PPM_EXP_ONE
         if (advect) {
             if (axis == 0) ppm_advect_kernel<0><<<grid, block, 0, c->stream>>>(P);
             else if (axis == 1) ppm_advect_kernel<1><<<grid, block, 0, c->stream>>>(P);
             else ppm_advect_kernel<2><<<grid, block, 0, c->stream>>>(P);
             e = cudaGetLastError();
-        } else if (axis == 0) e = launch_dir<0>(P, p.grav.kind, grid, block, c->stream);
+        } else
+#endif
+        if (axis == 0) e = launch_dir<0>(P, p.grav.kind, grid, block, c->stream);
         else if (axis == 1) e = launch_dir<1>(P, p.grav.kind, grid, block, c->stream);
         else e = launch_dir<2>(P, p.grav.kind, grid, block, c->stream);
     }
