@@ -50,9 +50,8 @@
 #endif
 // warp-uniform shortcuts past work whose outcome is known for every lane (no shock near, star state at the face,
 // Newton converged, PPB polynomial inside its bounds); a bit mask, 0 = always the general code (A/B knob)
-// carry 1/rho (and 1/c^2) down the pipeline instead of re-taking the reciprocals where they are needed (7 MUFU per cell)
-#ifndef PPM_CARRY_IRHO
-#define PPM_CARRY_IRHO 1
+#ifndef PPM_NEWTON_NESTED
+#define PPM_NEWTON_NESTED 0
 #endif
 #ifndef PPM_UNIFORM_FAST
 #define PPM_UNIFORM_FAST 2      // bits: 1 flattening, 2 converged W_K, 4 star state, 8 PPB theta
@@ -116,6 +115,25 @@ __device__ __forceinline__ v2 np(v2 a) { return mk(-a.x, a.y); }              //
 __device__ __forceinline__ v2 swp(v2 a) { return mk(a.y, a.x); }
 __device__ __forceinline__ v2 abs2(v2 a) { return mk(fabsf(a.x), fabsf(a.y)); }
 __device__ __forceinline__ float hsum(v2 a) { return a.x + a.y; }
+// A register-pair copy as ONE instruction on the FMA pipe (x * 1 under flush-to-zero).  The sliding windows of the
+// marching loop are shifted once per cell; as plain copies they are ~130 MOVs on the half-rate ALU pipe, issued in one
+// burst that starves the other warps' min/max/select work.
+#ifndef PPM_PACKED_MOVES
+#define PPM_PACKED_MOVES 1
+#endif
+#ifndef PPM_PM
+#define PPM_PM 5
+#endif
+#define MV5B(x) ((PPM_PM & 1) ? mv5(x) : (x))
+#define MV5C(x) ((PPM_PM & 2) ? mv5(x) : (x))
+#define MV2D(x) ((PPM_PM & 4) ? mv2(x) : (x))
+__device__ __forceinline__ v2 mv2(v2 a) {
+#if PPM_PACKED_MOVES
+    unsigned long long r; asm("mul.rn.ftz.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(mk(1.0f, 1.0f)))); return up(r);
+#else
+    return a;
+#endif
+}
 
 // the five interpolated variables of a cell: A = (rho', p'), B = (v, w) transverse, u normal
 struct V5 { v2 A, B; float u; };
@@ -128,6 +146,8 @@ __device__ __forceinline__ V5 fma5(const V5& a, float s, const V5& c) { V5 r; r.
 __device__ __forceinline__ V5 abs5(const V5& a) { V5 r; r.A = abs2(a.A); r.B = abs2(a.B); r.u = fabsf(a.u); return r; }
 __device__ __forceinline__ V5 bc5(float s) { V5 r; r.A = bc(s); r.B = bc(s); r.u = s; return r; }
 __device__ __forceinline__ V5 zero5() { V5 r; r.A = bc(0.f); r.B = bc(0.f); r.u = 0.f; return r; }
+// window shift of a cell's five variables: the two pairs as packed copies
+__device__ __forceinline__ V5 mv5(const V5& a) { V5 r; r.A = mv2(a.A); r.B = mv2(a.B); r.u = a.u; return r; }
 template <class F> __device__ __forceinline__ V5 map3(const V5& a, const V5& b, const V5& c, F f) {
     V5 r; r.A = mk(f(a.A.x, b.A.x, c.A.x), f(a.A.y, b.A.y, c.A.y)); r.B = mk(f(a.B.x, b.B.x, c.B.x), f(a.B.y, b.B.y, c.B.y)); r.u = f(a.u, b.u, c.u); return r;
 }
@@ -260,6 +280,7 @@ __device__ __forceinline__ void parabola(const V5& q0, const V5& Lc, const V5& R
 // ---- P4: exact projection of up to three pieces onto the Legendre basis ---------------------------
 // pre-limited coefficients of one cell in local family order, stored as the pairs the remap uses
 struct PpbCell { float a0, a1, a2; v2 bc0, bc1, de; float f; };   // bc0 = (b0, c0), bc1 = (b1, c1), de = (d0, e0)
+__device__ __forceinline__ void mv_ppb(PpbCell& d, const PpbCell& s) { d.a0 = s.a0; d.a1 = s.a1; d.a2 = s.a2; d.f = s.f; d.bc0 = mv2(s.bc0); d.bc1 = mv2(s.bc1); d.de = mv2(s.de); }
 
 // S[0..2]: cells i-1, i, i+1 (masses per dx rm, r0, rp); dl, dr = mass per dx through the left / right
 // face (positive rightward).  The two donor pieces (from i-1 and from i+1) run as one packed computation for
@@ -347,17 +368,19 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 
     // sliding windows (registers).  q[s]: cell n-4+s
     V5 q[5];
-    float pf[5], rf[6], gw[5];
+    v2 fw[5];                                   // full (rho, p) of cells n-4 .. n
+    v2 gi[4];                                   // slot s: (g of cell n-3+s, 1/rho of cell n-5+s) — two windows that shift together
+    float g4 = 0.f;                             // g of cell n-4
 #pragma unroll
-    for (int s = 0; s < 5; ++s) { q[s] = zero5(); pf[s] = 1.f; gw[s] = 0.f; }
+    for (int s = 0; s < 5; ++s) { q[s] = zero5(); fw[s] = bc(1.f); }
 #pragma unroll
-    for (int s = 0; s < 6; ++s) rf[s] = 1.f;
+    for (int s = 0; s < 4; ++s) gi[s] = mk(0.f, 1.f);
     V5 d2a = zero5(), d2b = zero5(), Fc = zero5(), Fcl = zero5(), parL = zero5(), parR = zero5();
     float WLr = 0.f, WLu = 0.f, WLp = 0.f, WLv = 0.f, WLw = 0.f;      // left state of the face being solved (from cell n-4)
     float Flm = 0.f, Fln = 0.f, FlE = 0.f;                              // fluxes through the left face of cell n-4
     v2 FlB = bc(0.f);
     float ft0 = 0.f, ft1 = 0.f, cs = 1.f;
-    float irw[4] = {1.f, 1.f, 1.f, 1.f}, ic2s = 1.f;                    // 1/rho of cells n-5 .. n-2; 1/c^2 of cell n-3 (PPM_CARRY_IRHO)
+    float ic2s = 1.f;                                                   // 1/c^2 of cell n-3
     v2 b0fc = bc(0.f);                                                  // (rho0, p0) at the face being solved
     PpbCell mw[3];
 #pragma unroll
@@ -378,34 +401,28 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         io.template begin<S>(n);
         // ---- shift windows, take plane n ---------------------------------------------------------------
 #pragma unroll
-        for (int s = 0; s < 4; ++s) { q[s] = q[s + 1]; pf[s] = pf[s + 1]; gw[s] = gw[s + 1]; }
+        for (int s = 0; s < 4; ++s) { q[s] = mv5(q[s + 1]); fw[s] = mv2(fw[s + 1]); }
+        g4 = gi[0].x;
 #pragma unroll
-        for (int s = 0; s < 5; ++s) rf[s] = rf[s + 1];
+        for (int s = 0; s < 3; ++s) gi[s] = mv2(gi[s + 1]);
+        float g_new;
         {
             float sgn, v[5];
             int j;
             io.template hydro<S>(n, j, sgn, v);
             q[4].A = mk(v[0], v[4]); q[4].B = mk(v[2], v[3]); q[4].u = v[1];
             const Base bs = geo.cell(P, j, sgn);
-            const v2 full = bs.rp + q[4].A;
-            rf[5] = full.x;
-            pf[4] = full.y;
-            gw[4] = bs.g;
+            fw[4] = bs.rp + q[4].A;
+            g_new = bs.g;
         }
         // ---- E, F: flattening ---------------------------------------------------------------------------
-#if PPM_CARRY_IRHO
-        // 1/rho is taken once per cell and carried (tracing and the PPB masses need it again), and c and 1/c^2 come
+        // 1/rho is taken once per cell and carried (the tracing and the PPB masses need it again), and c and 1/c^2 come
         // from ONE reciprocal square root: c = x rsqrt(x), 1/c^2 = rsqrt(x)^2 with x = gamma p / rho
-#pragma unroll
-        for (int s = 0; s < 3; ++s) irw[s] = irw[s + 1];
-        irw[3] = rcp(rf[3]);
-        const float xc = gam * pf[2] * irw[3];
+        gi[3] = mk(g_new, rcp(fw[2].x));
+        const float xc = gam * fw[2].y * gi[3].y;
         const float icn = rsqrtf(fmaxf(xc, 1e-37f));
         const float cn2 = xc * icn;                                  // c_{n-2}
         const float ic2n = icn * icn;
-#else
-        const float cn2 = fsqrt(gam * pf[2] * rcp(rf[3]));          // c_{n-2}
-#endif
         float ftn;
         if (FLAT) {
             ftn = fpre;                                              // F~_{n-2}, in flight since the last iteration
@@ -416,11 +433,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // The jump ramp clamp(3|d1|/min(p) - 1) is zero wherever the pressure changes by less than a third over two
             // cells: everywhere but in strong shocks.  When no lane of the warp is near one, f~ = 0 without the three
             // divisions (a warp-uniform shortcut: the result is the same zero the ramps would give).
-            const float d1 = pf[3] - pf[1];
-            const float pm = fminf(pf[3], pf[1]);
+            const float d1 = fw[3].y - fw[1].y;
+            const float pm = fminf(fw[3].y, fw[1].y);
             ftn = 0.f;
             if (!(PPM_UNIFORM_FAST & 1) || !__all_sync(wmask, 3.0f * fabsf(d1) <= pm || !valid)) {
-                const float dd2 = pf[4] - pf[0];
+                const float dd2 = fw[4].y - fw[0].y;
                 const float steep = sat(10.0f * (fdiv(fabsf(d1), fmaxf(fabsf(dd2), PPM_TINY)) - 0.75f));
                 const float jump = sat(fdiv(3.0f * fabsf(d1), pm) - 1.0f);
                 const float conv = sat(fdiv(q[1].u - q[3].u, 0.05f * cn2));
@@ -449,12 +466,8 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             }
             const V5 dq = R - L;
             const V5 q6 = fma5(L + R, -3.0f, qc * 6.0f);
-            const float rho = rf[2], c = cs, u = qc.u;
-#if PPM_CARRY_IRHO
-            const float c2 = c * c, rc = rho * c, ic2 = ic2s, ic2h = 0.5f * ic2, cor = c * irw[2];
-#else
-            const float c2 = c * c, rc = rho * c, ic2 = rcp(c2), ic2h = 0.5f * ic2, cor = fdiv(c, rho);
-#endif
+            const float rho = fw[1].x, c = cs, u = qc.u;
+            const float c2 = c * c, rc = rho * c, ic2 = ic2s, ic2h = 0.5f * ic2, cor = c * gi[2].y;
             const float s_m = (u - c) * dtdx, s_0 = u * dtdx, s_p = (u + c) * dtdx;
             // Each wave family k takes its amplitude from its own domain of dependence max(+-sigma^k, 0); a
             // wave moving away from the face has the zero-width domain, i.e. the edge value (reading R8',
@@ -490,11 +503,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (GRAV != PPM_GRAV_NONE) {   // half-step sources of the perturbation equations (H6)
                 const v2 db = b0fn - b0fc;
                 const float k = -hdt * u * P.inv_dx;
-#if PPM_CARRY_IRHO
-                const float su = hdt * gw[1] * (qc.A.x * irw[2]);
-#else
-                const float su = hdt * gw[1] * fdiv(qc.A.x, rho);
-#endif
+                const float su = hdt * gi[0].x * (qc.A.x * gi[2].y);
                 Wr = Wr + bc(k * db.x); Wp = Wp + bc(k * db.y); Wu = Wu + bc(su);
             }
         }
@@ -544,11 +553,20 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // remaining ones only while some lane still moves (rare at low Mach: the acoustic guess is nearly exact)
             // (lanes on pad cells of a ragged grid carry garbage and do not vote)
             bool conv = __all_sync(wmask, newton() || !valid);
+#if PPM_NEWTON_NESTED
+            // (nested rather than looped: a loop makes ptxas copy a dozen operands into the loop's registers on every pass
+            // through here, though the loop body itself runs for strong shocks only)
+            if (!conv) { conv = __all_sync(wmask, newton() || !valid);
+                if (!conv) { conv = __all_sync(wmask, newton() || !valid);
+                    if (!conv) { conv = __all_sync(wmask, newton() || !valid);
+                        if (!conv) conv = __all_sync(wmask, newton() || !valid); } } }
+#else
             if (!conv) {
 #pragma unroll 1
                 for (int it = 1; it < 5; ++it)
                     if ((conv = __all_sync(wmask, newton() || !valid))) break;
             }
+#endif
             const float ps = p0f + pps;
             // "then recompute W_K" at the final p* (H7).  After a converged iteration p* moved by less than one fp32
             // rounding of itself, so W_K of that iteration IS W_K(p*) to rounding: it is reused.  Only when the
@@ -593,7 +611,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             FrE = uh * fmaf(g_gm1, ph, 0.5f * rh * fmaf(uh, uh, hsum(vw * vw)));
         }
         // ---- K (first half): PPB coefficients of cell n-3, pre-limited (P2) ---------------------------
-        mw[0] = mw[1]; mw[1] = mw[2];
+        mv_ppb(mw[0], mw[1]); mv_ppb(mw[1], mw[2]);
         if (S >= 0 || n - 3 >= c0 - 1) {
             float m[10];
             io.template ppb<S>(n - 3, m);
@@ -606,7 +624,8 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // "almost never performed") — then the coefficients are taken as they are
             const float room = fmaxf(0.f, fminf(m[0], 1.0f - m[0]));
             // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
-            asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
+            if (IO::HAS_FAST) mw[2].a0 = m[0];
+            else asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
             if ((PPM_UNIFORM_FAST & 8) && __all_sync(wmask, B <= room || !valid)) {
                 mw[2].a1 = m[1]; mw[2].a2 = m[2]; mw[2].f = m[9];
                 mw[2].bc0 = bc0; mw[2].bc1 = bc1; mw[2].de = de;
@@ -628,7 +647,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 io.template old_hydro<S>(i, v);
                 qo.A = mk(v[0], v[4]); qo.B = mk(v[2], v[3]); qo.u = v[1];
             }
-            const float r_old = rf[1], rp_old = qo.A.x, pp_old = qo.A.y, u0 = qo.u, g = gw[0];
+            const float r_old = fw[0].x, rp_old = qo.A.x, pp_old = qo.A.y, u0 = qo.u, g = g4;
             const v2 vw0 = qo.B;
             float drho = -dtdx * (Frm - Flm);
             int bad = 0;
@@ -649,25 +668,19 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const v2 vw1 = mB * irn;
             const float dKE = 0.5f * (r_new * fmaf(u1, u1, hsum(vw1 * vw1)) - r_old * fmaf(u0, u0, hsum(vw0 * vw0)));
             float pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
-            const float p0c = pf[0] - pp_old;
+            const float p0c = fw[0].y - pp_old;
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
-#if PPM_CARRY_IRHO
-            ppb_remap(mw, irw[0], irw[1], irw[2], r_new, irn, dtdx * Flm, dtdx * Frm, mo);
-#else
-            ppb_remap(mw, rcp(rf[0]), rcp(rf[1]), rcp(rf[2]), r_new, irn, dtdx * Flm, dtdx * Frm, mo);
-#endif
+            ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
             io.template store<S>(i, ho, mo);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
-        d2a = d2b; d2b = d2n; Fc = Fn; Fcl = Fnl; parL = pLn; parR = pRn;
+        d2a = mv5(d2b); d2b = MV5B(d2n); Fc = MV5B(Fn); Fcl = MV5B(Fnl); parL = MV5C(pLn); parR = MV5C(pRn);
         WLr = Wr.x; WLu = Wu.x; WLp = Wp.x; WLv = Wv.x; WLw = Ww.x;
-        Flm = Frm; Fln = Frn; FlE = FrE; FlB = FrB;
+        Flm = Frm; Fln = Frn; FlE = FrE; FlB = MV2D(FrB);
         ft0 = ft1; ft1 = ftn; cs = cn2; b0fc = b0fn;
-#if PPM_CARRY_IRHO
         ic2s = ic2n;
-#endif
     };
     using std::integral_constant;
     if (IO::HAS_FAST) {
