@@ -110,7 +110,8 @@ int ppm_sweep(ppm_ctx *ctx, double dt, int axis);
 int ppm_advect(ppm_ctx *ctx, double dt, int sweep_order);
 
 /* dt = cfl*dx / max over cells of max_d(|u_d|) + c, c from the full rho, p (the scheme is explicit, PAPER.md L55;
- * SURVEY 8(c) C6).  Synchronises the stream.  dt_out: [host].  PPM_ESTATE if a cell has non-positive rho or p. */
+ * SURVEY 8(c) C6).  The maximum is already on the device when the state was last changed by ppm_step (it is reduced
+ * inside the step's last sweep, see PPM_OPT_CFL_FUSED); otherwise one reduction kernel runs first.  Synchronises the stream.  dt_out: [host].  PPM_ESTATE if a cell has non-positive rho or p. */
 int ppm_cfl_dt(ppm_ctx *ctx, double cfl, double *dt_out);
 
 /* (BASELINE.json north_star: conservation to round-off on periodic boxes)
@@ -129,6 +130,11 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *  PPM_OPT_IO_PATH : 0 = automatic: a sweep along an axis whose extent is a multiple of 4 stages whole brick
  *                    records through shared memory with bulk copies (cp.async.bulk), any other axis uses the
  *                    direct global-memory path; 1 = direct path for every axis.
+ *  PPM_OPT_CFL_FUSED : 1 (default) = the last sweep of ppm_step also reduces max over cells of max_d |u_d| + c of the
+ *                    state it writes (warp max + one atomicMax per warp), so that the next ppm_cfl_dt
+ *                    only reads 4 bytes back; 0 = ppm_cfl_dt always runs its own reduction pass over the state.  The
+ *                    two agree to fp32 rounding of c (bit for bit without a base state).  Whatever else changes the
+ *                    state (ppm_set_state, ppm_sweep, a sweep on the direct path) makes ppm_cfl_dt fall back to the pass.
  *
  * Option that changes the numerical scheme ("a fully 3-D treatment of the
  * shock dissipation"; reading R5b in DESIGN.md):
@@ -138,7 +144,7 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    (ppm_sweep: on the state that sweep starts from) and spread over i-1..i+1 along the sweep.
  *                    Setting it allocates one library-owned device array of ppm_state_floats()/15 floats
  *                    (PPM_ENOMEM if that fails) and adds one light kernel launch per step. */
-enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3 };
+enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* 1 if the next sweep along axis (0,1,2) will take the bulk-staged path, 0 if the direct path. */
 int ppm_axis_path(const ppm_ctx *ctx, int axis);

@@ -23,7 +23,7 @@ NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
            "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_destroy", "ppm_last_error")
-OPT_IO_PATH, OPT_FLATTEN3D = 2, 3
+OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED = 2, 3, 4
 
 
 class ppm_gravity(C.Structure):

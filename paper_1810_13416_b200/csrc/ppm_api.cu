@@ -99,6 +99,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c->nblocks_red = 148 * 4;
     if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sms < 1) c->sms = 148;
     c->chunk = 0;
+    c->cfl_fused = 1; c->cfl_valid = 0;
     c->err[0] = 0;
     // brick records of 4x4x4 cells x 15 fields; extents are rounded up to whole bricks (ppm_state_floats)
     c->nbx = (prm->nx + 3) / 4; c->nby = (prm->ny + 3) / 4; c->nbz = (prm->nz + 3) / 4;
@@ -175,6 +176,7 @@ extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS],
     for (int f = 0; f < PPM_NFIELDS; ++f)
         CU(cudaMemcpyAsync(scratch + f * tot, fields[f], sizeof(float) * tot, kind, c->stream));
     CU(ppm_launch_to_perturbation(c, scratch, st, z0, nzs));
+    c->cfl_valid = 0;
     CU(cudaMemsetAsync(c->flag, 0, sizeof(int), c->stream));
     return PPM_OK;
 }
@@ -198,6 +200,7 @@ extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
     DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "ppm_sweep: need finite dt > 0 and axis in 0..2"); return PPM_EINVAL; }
     if (c->flat3d) CU(ppm_launch_flatten3d(c));     // the detector field of the state this sweep starts from
+    c->cfl_valid = 0;
     CU(ppm_launch_sweep(c, axis, dt));
     return PPM_OK;
 }
@@ -207,7 +210,15 @@ extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
     DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_step: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
     if (c->flat3d) CU(ppm_launch_flatten3d(c));     // once per step, on the step's starting state
-    for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt));
+    c->cfl_valid = 0;
+    for (int s = 0; s < 3; ++s) {
+        const int axis = ORDERS[sweep_order][s];
+        // S10 fused: the step's last sweep also leaves max_d |u_d| + c of the NEW state in cflmax (bulk-staged sweeps only)
+        const bool fuse = s == 2 && c->cfl_fused && ppm_axis_is_bulk(c, axis);
+        if (fuse) CU(cudaMemsetAsync(c->cflmax, 0, sizeof(unsigned int), c->stream));
+        CU(ppm_launch_sweep(c, axis, dt, false, fuse));
+        if (fuse) c->cfl_valid = 1;
+    }
     return PPM_OK;
 }
 
@@ -223,14 +234,15 @@ extern "C" int ppm_cfl_dt(ppm_ctx* c, double cfl, double* dt_out) {
     if (!c) { set_err(nullptr, "ppm_cfl_dt: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);
     if (!dt_out || !(cfl > 0.0)) { set_err(c, "ppm_cfl_dt: need cfl > 0 and dt_out"); return PPM_EINVAL; }
-    CU(ppm_launch_cfl(c));
+    if (!c->cfl_valid) CU(ppm_launch_cfl(c));       // else: the last ppm_step already reduced the maximum of this state
     unsigned int enc = 0;
     CU(cudaMemcpyAsync(&enc, c->cflmax, sizeof(enc), cudaMemcpyDeviceToHost, c->stream));
     int rc = read_flag(c);
     if (rc) return rc;
     float vmax;
     memcpy(&vmax, &enc, sizeof(float));
-    if (!(vmax > 0.f)) { set_err(c, "ppm_cfl_dt: max signal speed is not positive"); return PPM_ESTATE; }
+    if (!(vmax > 0.f)) { c->cfl_valid = 0; set_err(c, "ppm_cfl_dt: max signal speed is not positive or not a number"); return PPM_ESTATE; }
+    c->cfl_valid = 1;                               // cflmax now holds the maximum of the current state
     *dt_out = cfl * c->prm.dx / (double)vmax;
     return PPM_OK;
 }
@@ -261,6 +273,7 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
+    if (option == PPM_OPT_CFL_FUSED && (value == 0 || value == 1)) { c->cfl_fused = value; c->cfl_valid = 0; return PPM_OK; }
     if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
         if (value && !c->F3) {
             const size_t n = (size_t)c->nbx * c->nby * c->nbz * 64;

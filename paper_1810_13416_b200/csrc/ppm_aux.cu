@@ -115,34 +115,52 @@ __device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k
     return make_float2(0.f, 0.f);
 }
 
-// order-preserving float -> uint encoding for atomicMax (all values here are >= 0)
-__device__ __forceinline__ unsigned int enc(float x) { return __float_as_uint(fmaxf(x, 0.f)); }
+// streaming read: touched once, keep it out of L1
+__device__ __forceinline__ float ld_stream(const float* p) { float v; asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
 
+// One warp per brick record: a lane takes cells `lane` and `lane + 32` of the brick, i.e. the hydro part of the record
+// (5 fields x 256 B, contiguous) is read as ten fully coalesced 128-byte rows that are all in flight before the first
+// one is used.  c = x rsqrt(x), x = gamma p / rho — the formula of the reduction fused into the sweeps (ppm_sweep.cu).
 __global__ void __launch_bounds__(256) cfl_kernel(const AuxParams A, const float* __restrict__ st, unsigned int* __restrict__ out, int* flag) {
-    float vmax = 0.f;
+    const int lane = threadIdx.x & 31;
+    const long long nbricks = A.nslots >> 6;
+    const long long nwarps = (long long)gridDim.x * (blockDim.x >> 5);
     const float gam = A.gamf;
-    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
-        int i, j, k;
-        long long o;
-        if (!cell_of(A, t, i, j, k, o)) continue;
-        const float2 b0 = base32(A, i, j, k);              // fp32 base state, as the sweeps evaluate it
-        const float rho = b0.x + st[o], p = b0.y + st[o + 4 * 64];
-        const float c = sqrtf(gam * p / rho);
-        const float um = fmaxf(fabsf(st[o + 64]), fmaxf(fabsf(st[o + 2 * 64]), fabsf(st[o + 3 * 64])));
-        const float v = um + c;
-        if (!(v == v) || !(rho > 0.f) || !(p > 0.f)) atomicOr(flag, 2);
-        vmax = fmaxf(vmax, v);
-    }
+    float vmax = 0.f;
+    bool bad = false;
+    for (long long B = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; B < nbricks; B += nwarps) {
+        const float* p = st + B * PPM_BRICK_FLOATS + lane;
+        float v[2][5];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) vmax = fmaxf(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
-    __shared__ float sm[8];
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = vmax;
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int f = 0; f < 5; ++f) v[h][f] = ld_stream(p + 32 * h + 64 * f);
+        const unsigned q = (unsigned)B / (unsigned)A.nbx;
+        const int bx = (int)((unsigned)B - q * (unsigned)A.nbx);
+        const int bz = (int)(q / (unsigned)A.nby);
+        const int by = (int)(q - (unsigned)bz * (unsigned)A.nby);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int c = lane + 32 * h;
+            const int i = bx * 4 + (c & 3), j = by * 4 + ((c >> 2) & 3), k = bz * 4 + (c >> 4);
+            if (i >= A.nx || j >= A.ny || k >= A.nz) continue;             // pad cell of a ragged grid
+            const float2 b0 = base32(A, i, j, k);                          // fp32 base state, as the sweeps evaluate it
+            const float rho = b0.x + v[h][0], pr = b0.y + v[h][4];
+            const float xs = gam * pr * __fdividef(1.0f, rho);
+            const float cs = xs * rsqrtf(fmaxf(xs, 1e-37f));
+            const float sp = fmaxf(fabsf(v[h][1]), fmaxf(fabsf(v[h][2]), fabsf(v[h][3]))) + cs;
+            bad |= !(sp == sp) || !(rho > 0.f) || !(pr > 0.f);
+            vmax = fmaxf(vmax, sp);
+        }
+    }
+    if (bad) atomicOr(flag, 2);
+    const unsigned m = __reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(vmax, 0.f)));
+    __shared__ unsigned sm[8];
+    if (lane == 0) sm[threadIdx.x >> 5] = m;
     __syncthreads();
     if (threadIdx.x < 32) {
-        float v = (threadIdx.x < (blockDim.x >> 5)) ? sm[threadIdx.x] : 0.f;
-#pragma unroll
-        for (int o = 4; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
-        if (threadIdx.x == 0) atomicMax(out, enc(v));
+        const unsigned w = __reduce_max_sync(0xffffffffu, threadIdx.x < (blockDim.x >> 5) ? sm[threadIdx.x] : 0u);
+        if (threadIdx.x == 0) atomicMax(out, w);
     }
 }
 
@@ -349,7 +367,7 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c) {
     cudaError_t e = cudaMemsetAsync(c->cflmax, 0, sizeof(unsigned int), c->stream);
     if (e != cudaSuccess) return e;
     const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
-    cfl_kernel<<<grid_for(n, 148 * 8), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->cflmax, c->flag);
+    cfl_kernel<<<grid_for(n / 2, c->sms * 8), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->cflmax, c->flag);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -42,6 +42,7 @@ struct SweepParams {
     const float4* __restrict__ tabp; // {rho0_k, p0_k, rho0_k+1 - rho0_k, p0_k+1 - p0_k}
     const float2* __restrict__ tabg; // {g_k, g_k+1 - g_k}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
+    unsigned int* cflmax;           // non-NULL: fold max_d |u_d| + c of every finished cell into it (bit pattern of a float >= 0)
     // 3-D flattening mode: F~ of every cell, [brick][4z][4y][4x] (a brick is 64 floats: strides = SB / 15); else NULL
     const float* flat;
     long long FBd, FBa, FBb;
@@ -67,13 +68,15 @@ struct ppm_ctx {
     int flat3d;                     // PPM_OPT_FLATTEN3D
     float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
     int sms;                        // multiprocessors of the device
+    int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state
+    int cfl_valid;                  // cflmax holds the maximum of the CURRENT state (set by a fused step, cleared by anything else that changes the state)
     int io_path;                    // PPM_OPT_IO_PATH: 0 = bulk-staged where the sweep-axis extent is whole bricks, 1 = direct everywhere
     long long launches;
     char err[512];
 };
 
 // launchers (defined in the .cu files)
-cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect = false);   // advect: PPB-only sweep (NEXT-2)
+cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect = false, bool fuse_cfl = false);   // advect: PPB-only sweep (NEXT-2); fuse_cfl: S10 folded into this sweep (bulk path only)
 bool ppm_axis_is_bulk(const ppm_ctx* c, int axis);
 int ppm_tail_chunk(int ntail, int slots, int n);   // segment length for the pencils of the ragged last wave
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs);

@@ -357,9 +357,12 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
 // =====================================================================================================
 // FLAT: 3-D flattening mode — the un-spread coefficient of cell n-2 is read from the detector field
 // (pflat = the pencil's cell 0 in it) instead of being computed from the pencil's own pressures and velocities.
-template <int DIR, int GRAV, bool FLAT, class IO>
+// CFL: S10 fused into the sweep — every finished cell folds max_d |u_d| + c of its NEW
+// state into vmax, so that the step's last sweep leaves the next step's CFL maximum behind and ppm_cfl_dt has no pass
+// of its own to make.
+template <int DIR, int GRAV, bool FLAT, bool CFL, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
-                                      const bool valid, const unsigned wmask, const float* __restrict__ pflat) {
+                                      const bool valid, const unsigned wmask, const float* __restrict__ pflat, float& vmax) {
     const float gam = P.gamma, gp = P.gp, gmg = P.gmg, g_gm1 = P.g_gm1;
     const float dtdx = P.dtdx, hdt = P.hdt;
 
@@ -671,6 +674,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const float p0c = fw[0].y - pp_old;
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
+            if (CFL) {                                         // C6 on the new state: c from the full rho, p
+                const float xs = gam * (p0c + pp_new) * irn;
+                const float cnew = xs * rsqrtf(fmaxf(xs, 1e-37f));
+                vmax = fmaxf(vmax, fmaxf(fabsf(u1), fmaxf(fabsf(vw1.x), fabsf(vw1.y))) + cnew);
+            }
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
             ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
             io.template store<S>(i, ho, mo);
@@ -880,7 +888,8 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     const long long tb = (long long)ba * P.SBa + (long long)bb * P.SBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)));
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     const float* pflat = FLAT ? P.flat + ((long long)ba * P.FBa + (long long)bb * P.FBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)))) : nullptr;
-    march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, true, wmask, pflat);
+    float vmax = 0.f;
+    march<DIR, GRAV, FLAT, false>(P, io, a, b, c0, c1, true, wmask, pflat, vmax);
 }
 
 // PPB-only sweep (NEXT-2), direct path
@@ -1167,7 +1176,7 @@ __device__ __forceinline__ void bulk_init_barriers(uint64_t* bars) {
     __syncthreads();
 }
 
-template <int DIR, int GRAV, bool FLAT>
+template <int DIR, int GRAV, bool FLAT, bool CFL>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1191,7 +1200,15 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
     const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
-    march<DIR, GRAV, FLAT>(P, io, a, b, c0, c1, a < P.na && b < P.nb, 0xffffffffu, pflat);
+    const bool valid = a < P.na && b < P.nb;
+    float vmax = 0.f;
+    march<DIR, GRAV, FLAT, CFL>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax);
+    if (CFL) {
+        // warp max by one REDUX on the bit patterns (non-negative floats order like unsigned integers; a NaN has the
+        // largest pattern and so survives: ppm_cfl_dt reports it), then one atomicMax per warp
+        const unsigned m = __reduce_max_sync(0xffffffffu, valid ? __float_as_uint(fmaxf(vmax, 0.f)) : 0u);
+        if (lane == 0) atomicMax(P.cflmax, m);
+    }
 }
 
 // PPB-only sweep (NEXT-2), bulk-staged path: same rings; the hydro slots travel through unchanged
@@ -1264,8 +1281,9 @@ cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_
 }
 template <int DIR, int GRAV, bool FLAT>
 cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ[MAX_DEV] = {};
-    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT>, occ, P, sms, user_chunk, st);
+    static int occ[2][MAX_DEV] = {};
+    if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, true>, occ[1], P, sms, user_chunk, st);
+    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
@@ -1318,7 +1336,7 @@ bool ppm_axis_is_bulk(const ppm_ctx* c, int axis) {
     return c->io_path == 0 && ext[axis] % 4 == 0;
 }
 
-cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect) {
+cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool fuse_cfl) {
     const ppm_params& p = c->prm;
     SweepParams P;
     P.in = c->buf[c->cur];
@@ -1344,6 +1362,7 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect) {
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
     P.tab = c->tab; P.tabp = c->tabp; P.tabg = c->tabg;
     P.flag = c->flag;
+    P.cflmax = (fuse_cfl && !advect && ppm_axis_is_bulk(c, axis)) ? c->cflmax : nullptr;
     P.flat = c->flat3d ? c->F3 : nullptr;
     P.FBd = P.SBd / PPM_NFIELDS; P.FBa = P.SBa / PPM_NFIELDS; P.FBb = P.SBb / PPM_NFIELDS;
     const int nchunks = (P.n + chunk - 1) / chunk;

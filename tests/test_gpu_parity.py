@@ -130,6 +130,43 @@ def test_pencil_chunking_does_not_change_results(chunk):
     assert np.array_equal(res[0], res[1])
 
 
+def test_cfl_reduction_fused_into_the_last_sweep_equals_the_standalone_pass():
+    """the last sweep of ppm_step reduces max_d |u_d| + c of the state it writes, so ppm_cfl_dt launches
+    nothing after a step.  The standalone pass (PPM_OPT_CFL_FUSED = 0, and always after ppm_set_state / ppm_sweep) uses the
+    same formula on the stored state: without a base state the two maxima are the same bits; with one, the sweep's full
+    pressure comes from its (rho, p) window instead of a fresh table lookup and they agree to fp32 rounding."""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_CFL_FUSED
+    for cfg, n, tol in ((1, 32, 0.0), (3, 32, 0.0), (4, 32, 3e-7), (2, 32, 3e-7)):
+        w = W.make(cfg, n=n)
+        f = w.fields().cuda()
+        dts = {}
+        for fused in (1, 0):
+            g = PPM.from_workload(w)
+            g.set_option(OPT_CFL_FUSED, fused)
+            g.set_state(f)
+            dts[fused] = []
+            n0 = g.launch_count()
+            for s in range(4):
+                dt = g.cfl_dt(w.cfl)
+                dts[fused].append(dt)
+                g.step(dts[1][s], s)                      # both runs take the same steps
+            dts[fused].append(g.cfl_dt(w.cfl))
+            # launches: fused = 1 pass after set_state + 4 x 3 sweeps; standalone = 5 passes + 12 sweeps
+            assert g.launch_count() - n0 == (13 if fused else 17)
+            state = g.get_state().cpu().numpy()
+            g.close()
+            dts[(fused, "state")] = state
+        assert np.array_equal(dts[(1, "state")], dts[(0, "state")])
+        a, b = np.array(dts[1]), np.array(dts[0])
+        assert a[0] == b[0]                                # both from the standalone pass after set_state
+        if tol == 0.0:
+            assert np.array_equal(a, b), (cfg, a, b)
+        else:
+            assert np.max(np.abs(a - b) / b) <= tol, (cfg, a, b)
+        assert len(set(a)) == len(a)                       # the maximum really changes from step to step
+
+
 # ---------------------------------------------------------------- reduced-size, full step counts ------
 def test_cfg2_stratified_reduced_64_100_steps():
     w = W.make(2, n=64)
@@ -180,7 +217,7 @@ def test_flatten3d_smooth_flow_equals_1d_mode_bitwise():
         for s in range(3):
             g.step(g.cfl_dt(0.8), s * 2)
         res.append(g.get_state().cpu().numpy())
-        assert g.launch_count() == (3 * (3 + mode) + 3 + 2)       # per step: 3 sweeps (+ 1 detector), 3 cfl, set + get
+        assert g.launch_count() == (3 * (3 + mode) + 1 + 2)       # per step: 3 sweeps (+ 1 detector); 1 cfl pass (the others are fused into the sweeps); set + get
         g.close()
     assert np.array_equal(res[0], res[1])
 
