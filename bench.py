@@ -3,13 +3,17 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 4|5|...] [--impl reference]
 
-A "step" is one ppm_step = the whole hot path (three fused hydro+PPB sweeps) over the
-whole synthetic grid.  value = cells * K / device time (CUDA events, max over ranks), inputs resident in
-HBM.  e2e = the same metric through the C ABI with pinned HOST buffers: ppm_set_state(host) + ppm_step +
-ppm_get_state(host) inside the timed region.  Multi-GPU: the path is "replicas only": each
-rank advances its own grid, no data-path collective; value sums the ranks' cells ("weak" scaling).
+A "step" is one ppm_step = the whole hot path (three fused hydro+PPB sweeps, the CFL max-reduction folded into the
+last one) over the whole synthetic grid.  value = cells * K / device time, inputs resident in HBM; the
+K-step region is timed with CUDA events on the library's stream, repeated (5 times; 3 at 1024^3) and the MEDIAN
+repetition is reported; every repetition is listed.  The default run times config 4 (512^3, the headline)
+and then, in the same process, config 5 (1024^3) as the "also" entry — the two grids the target names.
+e2e = the same metric through the C ABI with pinned HOST buffers: ppm_set_state(host) + ppm_step + ppm_get_state(host)
+inside the timed region, the slabs of the upload, the step and the download pipelined on two streams.
+Multi-GPU: the path is "replicas only": each rank advances its own grid, no data-path collective; value
+sums the ranks' cells ("weak" scaling).
 
---impl reference times the fp64 CPU oracle (as it stands) on a bounded window of the same workload.
+--impl reference times the fp64 CPU oracle (as it stands) on a bounded sample of the same workload.
 """
 import argparse
 import json
@@ -32,10 +36,11 @@ UNIT = "cell-updates/s"
 BYTES_PER_CELL_SWEEP = 120.0      # 15 fp32 fields read + written by every sweep
 BYTES_PER_CELL_SWEEP_ADVECT = 84.0   # PPB-only sweep: 1 velocity + 10 coefficients read, 10 written (it moves 120: hydro copied through)
 FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, FMA = 2
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md)
-# dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` capture
-# (profiles/), keyed by cells per side; None where no capture exists.
-NCU_TRAFFIC_BYTES = {512: 16.099e9}      # profiles/r1h_sweeps_ncu_full.md: 8.089 GB read + 8.010 GB written per launch
+FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md); fallback only
+# dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` captures, keyed by
+# cells per side: (bytes, the profiles/ file it comes from).  A size with no capture reports null.
+NCU_TRAFFIC = {512: (16.098e9, "profiles/r2_sweeps_ncu_full.md (ncu --set full, 512^3)"),
+               1024: (128.78e9, "profiles/r2_sweeps_1024_ncu.md (ncu, 1024^3)")}
 
 
 def _peaks():
@@ -123,21 +128,16 @@ def _load_state(g, w, nzs):
         g.set_state(w.fields((0, 0, z0), (n, n, z1), device=g.device), z0=z0)
 
 
-def _sample_window(w, side):
-    """central window of the workload used for the oracle timings"""
+# ------------------------------------------------------------------------------------------------ oracle timings
+def _time_oracle(w, side, steps, warmup):
+    """the fp64 oracle as it stands, all host threads, on the whole grid of `w` (side >= w.n) or on a central window"""
+    from oracle import binding as ob          # bench.py's cpu_baseline / reference legs may use oracle/
     side = min(side, w.n)
     lo = [(w.n - side) // 2] * 3
     hi = [lo[0] + side] * 3
     bc = [w.bc[k] if side == w.n else 2 for k in range(6)]
-    return lo, hi, bc
-
-
-def _time_oracle(w, side, steps, warmup):
-    from oracle import binding as ob          # bench.py's cpu_baseline / reference legs may use oracle/
-    lo, hi, bc = _sample_window(w, side)
     f = w.fields(lo, hi).numpy()
-    o = ob.Oracle(hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], w.dx, w.gamma, bc, w.grav, org=lo,
-                  rho_floor=w.rho_floor, p_floor=w.p_floor)
+    o = ob.Oracle(side, side, side, w.dx, w.gamma, bc, w.grav, org=lo, rho_floor=w.rho_floor, p_floor=w.p_floor)
     o.set_state(f)
     dt = 0.5 * o.cfl_dt(w.cfl)
     for s in range(warmup):
@@ -146,8 +146,16 @@ def _time_oracle(w, side, steps, warmup):
     for s in range(steps):
         o.step(dt, 0 if s % 2 == 0 else 5)
     t = time.perf_counter() - t0
-    cells = (hi[0] - lo[0]) ** 3
-    return cells * steps / t, t / steps, ob.num_threads(), "central %d^3 window of %s, %d steps" % (hi[0] - lo[0], w.name, steps)
+    what = "%s %d^3 grid" % (w.name, side) if side == w.n else "central %d^3 window of %s %d^3" % (side, w.name, w.n)
+    return side ** 3 * steps / t, t / steps, ob.num_threads(), "%s, %d steps after %d warm-up" % (what, steps, warmup)
+
+
+def _cpu_baseline(w):
+    """config 2's own grid (128^3, 10 steps) and a 256^3 grid (3 steps), one warm-up step each"""
+    v1, _, cores, s1 = _time_oracle(W.make(2), 128, 10, 1)
+    v2, _, _, s2 = _time_oracle(w, 256, 3, 1)
+    return {"value": v1, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": s1,
+            "also": {"value": v2, "unit": UNIT, "sample": s2}}
 
 
 def run_reference(args):
@@ -167,6 +175,130 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------------ GPU timings
+def _time_steps(g, do_step, dt, K, reps, barrier):
+    """`reps` repetitions of a K-step region, CUDA events on the library's stream; returns the list of ms per region"""
+    out = []
+    for r in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(g.stream)
+        for s in range(K):
+            do_step(dt, 0 if s % 2 == 0 else 5)
+        e1.record(g.stream)
+        barrier()
+        out.append(e0.elapsed_time(e1))
+    return out
+
+
+def _roofline(n, ms_per_step, advect, peak, peak_kind, fp32_peak, fp32_kind):
+    ncell = n ** 3
+    per_launch_s = ms_per_step * 1e-3 / 3          # the dominant kernel = the 3 sweep launches of every step
+    achieved = (BYTES_PER_CELL_SWEEP_ADVECT if advect else BYTES_PER_CELL_SWEEP) * ncell / per_launch_s / 1e9
+    flops_cs = 478.0 if advect else FLOPS_PER_CELL_SWEEP     # PPB-only: P2 13 + P1/P3/P4 460 + face masses 5 (DESIGN.md section 5)
+    alu = flops_cs * ncell / per_launch_s / 1e12
+    tr = NCU_TRAFFIC.get(n) if not advect else None
+    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "traffic": tr[0] if tr else None, "traffic_from": tr[1] if tr else None, "peak_kind": "of " + peak_kind,
+            "kernel": ("ppm_advect_bulk_kernel" if advect else "ppm_sweep_bulk_kernel") + " (3 launches per step; every launch moves 120 B/cell)",
+            "alu": {"achieved": alu, "peak": fp32_peak, "unit": "TFLOP/s", "frac": alu / fp32_peak, "peak_kind": fp32_kind,
+                    "flops_per_cell_sweep": flops_cs}}
+
+
+def _bench_grid(args, cfg, dev, lr, ws, barrier, K, reps, with_e2e):
+    """times one workload on this rank's GPU; returns a dict of raw numbers (ms are per K-step region)"""
+    from paper_1810_13416_b200.binding import PPM, NF, OPT_IO_PATH, OPT_FLATTEN3D
+    w = W.make(cfg)
+    n = w.n
+    g = PPM.from_workload(w, device=dev)
+    if args.chunk:
+        g.set_chunk(args.chunk)
+    if args.direct:
+        g.set_option(OPT_IO_PATH, 1)
+    if args.flatten3d:
+        g.set_option(OPT_FLATTEN3D, 1)
+    _load_state(g, w, 8 if n >= 1024 else 32)
+    dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
+    do_step = g.advect if args.advect else g.step
+    Wm = max(args.warmup, 3)
+    for s in range(Wm):
+        do_step(dt, 0 if s % 2 == 0 else 5)
+    barrier()
+    clk = _Clocks(lr)
+    l0 = g.launch_count()
+    ms_reps = _time_steps(g, do_step, dt, K, reps, barrier)
+    launches = (g.launch_count() - l0) // reps
+    clocks = clk.stop()
+    g.sync()                         # raises if the state flag (NaN / floor) was set
+    # the same K steps with ppm_cfl_dt before each one (the configs' "dt from ppm_cfl_dt each step"): after a ppm_step
+    # the maximum is already on the device (reduced inside the last sweep), so this adds one 4-byte read and a host sync
+    ms_cfl = []
+    for r in range(min(reps, 3)):
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e2.record(g.stream)
+        for s in range(K):
+            do_step(0.7 * g.cfl_dt(w.cfl), 0 if s % 2 == 0 else 5)
+        e3.record(g.stream)
+        barrier()
+        ms_cfl.append(e2.elapsed_time(e3))
+    fp32 = None
+    try:
+        fp32 = g.measure_fp32_peak()
+    except Exception:
+        pass
+    e2e = None
+    if with_e2e:
+        try:
+            e2e = _time_e2e(g, do_step, dt, args.e2e_steps, barrier, n, NF)
+        except Exception as ex:                                                  # e.g. not enough pinned host memory
+            e2e = {"error": str(ex)[:200]}
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+    return {"w": w, "n": n, "ms_reps": ms_reps, "ms_cfl": ms_cfl, "launches": launches, "clocks": clocks, "fp32": fp32,
+            "e2e": e2e, "warmup": Wm}
+
+
+def _time_e2e(g, do_step, dt, Ke, barrier, n, NF):
+    """host buffers through the C ABI, copies inside the timed region.
+    serial   : ppm_set_state(host) -> ppm_step -> ppm_get_state(host), one grid after the other on one stream;
+    pipelined: a stream of INDEPENDENT host-resident grids, each uploaded, advanced one step and downloaded
+               (PPM.step_host_pipelined): the slabs of grid s+1 go up while the slabs of grid s come down."""
+    ncell = n ** 3
+    host_a = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
+    host_out = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
+    g.get_state(out=host_a)
+    g.set_state(host_a); do_step(dt, 0); g.get_state(out=host_out)      # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(Ke):
+        g.set_state(host_a)
+        do_step(dt, 0 if s % 2 == 0 else 5)
+        g.get_state(out=host_out)       # synchronises
+    torch.cuda.synchronize()
+    serial = (time.perf_counter() - t0) * 1e3 / Ke
+    res = {"serial_ms": serial, "steps": Ke, "bytes": NF * ncell * 4}
+    try:
+        host_b = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
+        host_b.copy_(host_out)
+        ins = [host_a, host_b]
+        g.step_host_pipelined([host_a], [host_out], dt, [0], step=do_step)            # warm-up (allocates the staging slabs)
+        barrier()
+        Kp = max(Ke, 4)
+        t0 = time.perf_counter()
+        g.step_host_pipelined([ins[s % 2] for s in range(Kp)], [host_out] * Kp, dt, [0 if s % 2 == 0 else 5 for s in range(Kp)],
+                              step=do_step)
+        torch.cuda.synchronize()
+        res["pipelined_ms"] = (time.perf_counter() - t0) * 1e3 / Kp
+        res["pipelined_steps"] = Kp
+        del host_b
+    except Exception as ex:
+        res["pipelined_error"] = str(ex)[:200]
+    del host_a, host_out
+    return res
+
+
 def run_gpu(args):
     ws, rank, lr = _dist()
     if not torch.cuda.is_available():
@@ -176,129 +308,87 @@ def run_gpu(args):
     if ws > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-    from paper_1810_13416_b200.binding import PPM, NF
-
-    w = W.make(args.workload)
-    n = w.n
-    ncell = n ** 3
-    g = PPM.from_workload(w, device=dev)
-    if args.chunk:
-        g.set_chunk(args.chunk)
-    if args.direct:
-        from paper_1810_13416_b200.binding import OPT_IO_PATH
-        g.set_option(OPT_IO_PATH, 1)
-    if args.flatten3d:
-        from paper_1810_13416_b200.binding import OPT_FLATTEN3D
-        g.set_option(OPT_FLATTEN3D, 1)
-    _load_state(g, w, 8 if n >= 1024 else 32)
-    dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
-    do_step = g.advect if args.advect else g.step
 
     def barrier():
         if ws > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    K, Wm = args.steps, max(args.warmup, 3)
-    for s in range(Wm):
-        do_step(dt, 0 if s % 2 == 0 else 5)
-    barrier()
-    clk = _Clocks(lr)
-    l0 = g.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(g.stream)
-    for s in range(K):
-        do_step(dt, 0 if s % 2 == 0 else 5)
-    e1.record(g.stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = g.launch_count() - l0
-    clocks = clk.stop()
-    g.sync()                         # raises if the state flag (NaN / floor) was set
-
-    # ---- the same K steps with ppm_cfl_dt before each one (SURVEY 8(d) "also report with ppm_cfl_dt per step
-    # included"): one more reduction kernel and one host sync per step ----
-    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e2.record(g.stream)
-    for s in range(K):
-        do_step(0.7 * g.cfl_dt(w.cfl), 0 if s % 2 == 0 else 5)
-    e3.record(g.stream)
-    barrier()
-    ms_cfl = e2.elapsed_time(e3)
-    if ws > 1:
-        ms_cfl = max_over_ranks([ms_cfl], ws, dev)[0]
-
-    # ---- e2e: host buffers through the C ABI, copies inside the timed region ----
-    e2e = None
-    if not args.no_e2e:
+    K = args.steps
+    reps = args.reps if args.reps else (3 if args.workload == 5 else 5)
+    r = _bench_grid(args, args.workload, dev, lr, ws, barrier, K, reps, not args.no_e2e)
+    # second target grid in the same run: config 5 (1024^3, its 5 steps x 3 repetitions) when the headline is config 4
+    also = None
+    want_also = (args.workload == 4 and not args.no_also and not args.advect and not args.direct
+                 and torch.cuda.get_device_properties(dev).total_memory > 150e9)
+    if want_also:
         try:
-            Ke = args.e2e_steps
-            host_in = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
-            host_out = torch.empty((NF, n, n, n), dtype=torch.float32, pin_memory=True)
-            g.get_state(out=host_in)
-            g.set_state(host_in); do_step(dt, 0); g.get_state(out=host_out)      # warm-up
-            barrier()
-            t0 = time.perf_counter()
-            for s in range(Ke):
-                g.set_state(host_in)
-                do_step(dt, 0 if s % 2 == 0 else 5)
-                g.get_state(out=host_out)       # synchronises
-                host_in, host_out = host_out, host_in
-            torch.cuda.synchronize()
-            te = time.perf_counter() - t0
-            e2e = {"ms": te * 1e3 / Ke, "steps": Ke, "bytes": NF * ncell * 4}
-            del host_in, host_out
-        except Exception as ex:                                                  # e.g. not enough pinned host memory
-            e2e = {"error": str(ex)[:200]}
+            also = _bench_grid(args, 5, dev, lr, ws, barrier, 5, 3, False)
+        except Exception as ex:
+            also = {"error": str(ex)[:200]}
 
-    # ---- reduce over ranks ----
+    # ---- reduce over ranks (max of the per-rank times) ----
+    def med(x):
+        return float(np.median(x))
+    ms = med(r["ms_reps"])
+    ms_cfl = med(r["ms_cfl"])
+    e2e = r["e2e"]
+    vals = [ms, ms_cfl, (e2e or {}).get("serial_ms", 0.0), (e2e or {}).get("pipelined_ms", 0.0),
+            med(also["ms_reps"]) if also and "ms_reps" in also else 0.0]
     if ws > 1:
-        red = max_over_ranks([ms, e2e["ms"] if e2e and "ms" in e2e else 0.0], ws, dev)
-        ms = red[0]
-        if e2e and "ms" in e2e:
-            e2e["ms"] = red[1]
+        vals = max_over_ranks(vals, ws, dev)
+    ms, ms_cfl, e_ser, e_pipe, ms_also = vals
     if rank != 0:
         if ws > 1:
             dist.destroy_process_group()
         return 0
 
     peak, peak_kind = _peaks()
-    value = aggregate_value(ncell, K, ms, ws)
-    # the dominant kernel = the 3 sweep launches of every step (in --flatten3d mode the light detector kernel's time
-    # is charged to them: conservative)
-    per_launch_s = ms * 1e-3 / (3 * K)
-    achieved = (BYTES_PER_CELL_SWEEP_ADVECT if args.advect else BYTES_PER_CELL_SWEEP) * ncell / per_launch_s / 1e9
-    flops_cs = 478.0 if args.advect else FLOPS_PER_CELL_SWEEP     # PPB-only: P2 13 + P1/P3/P4 460 + face masses 5
-    alu = flops_cs * ncell / per_launch_s / 1e12
+    w, n = r["w"], r["n"]
+    ncell = n ** 3
+    fp32_peak, fp32_kind = (r["fp32"], "measured: FFMA micro-benchmark in this run (ppm_measure_fp32_peak)") if r["fp32"] else \
+        (FP32_NOMINAL_TFLOPS, "nominal: SMs x 128 lanes x 2 x max SM clock")
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": Wm,
+        "metric": METRIC, "value": aggregate_value(ncell, K, ms, ws), "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": r["warmup"],
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": "%s %d^3, %s, dt fixed at 0.7*CFL dt, sweep order xyz/zyx alternating" % (w.name, n, "reflecting walls + radial gravity" if w.grav else "periodic"),
-                   "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (NF * ncell * 4 / 1e9),
+                   "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (15 * ncell * 4 / 1e9),
                    "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk,
                    "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)",
-                   "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step)"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get(n), "peak_kind": "of " + peak_kind,
-                     "kernel": ("ppm_advect_bulk_kernel" if args.advect else "ppm_sweep_bulk_kernel") + " (3 launches per step; every launch moves 120 B/cell)",
-                     "alu": {"achieved": alu, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": alu / FP32_PEAK_TFLOPS,
-                             "flops_per_cell_sweep": flops_cs}},
-        "clocks": clocks, "gpu_launches": int(launches),
+                   "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step, CFL max-reduction fused into the last sweep)",
+                   "timing": "median of %d repetitions of the %d-step region (CUDA events on the library's stream)" % (len(r["ms_reps"]), K)},
+        "repetitions_ms_per_step": [x / K for x in r["ms_reps"]],
+        "roofline": _roofline(n, ms / K, args.advect, peak, peak_kind, fp32_peak, fp32_kind),
+        "clocks": r["clocks"], "gpu_launches": int(r["launches"]),
         "with_cfl_dt": {"value": aggregate_value(ncell, K, ms_cfl, ws), "unit": UNIT, "ms_per_step": ms_cfl / K,
-                        "note": "ppm_cfl_dt (max-reduction kernel + host sync) before every step"},
+                        "note": "ppm_cfl_dt before every step: the maximum is reduced inside the previous step's last sweep, so this is a 4-byte read + host sync"},
     }
-    if e2e and "ms" in e2e:
-        line["e2e"] = {"value": ws * ncell / (e2e["ms"] * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["bytes"],
-                       "d2h_bytes_per_step": e2e["bytes"], "steps": e2e["steps"], "ms_per_step": e2e["ms"]}
+    if e2e and "serial_ms" in e2e:
+        best = e_pipe if e_pipe > 0 else e_ser
+        line["e2e"] = {"value": ws * ncell / (best * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["bytes"],
+                       "d2h_bytes_per_step": e2e["bytes"], "steps": e2e.get("pipelined_steps", e2e["steps"]), "ms_per_step": best,
+                       "mode": ("independent host-resident grids, one step each: the upload slabs of grid s+1 overlap the download slabs of grid s "
+                                "(PPM.step_host_pipelined, two copy streams)") if e_pipe > 0 else "serial: set_state(host), step, get_state(host) on one stream",
+                       "serial_ms_per_step": e_ser,
+                       "pcie_floor_ms": e2e["bytes"] / 55e9 * 1e3,
+                       "note": e2e.get("pipelined_error")}
     else:
         line["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
                        "note": (e2e or {}).get("error", "skipped")}
+    if also and "ms_reps" in also:
+        n5 = also["n"]
+        fp5 = (also["fp32"], fp32_kind) if also["fp32"] else (fp32_peak, fp32_kind)
+        line["also"] = {"workload": "%s %d^3 (BASELINE.json configs[4]: its 5 steps, %d repetitions, same process)" % (also["w"].name, n5, len(also["ms_reps"])),
+                        "value": aggregate_value(n5 ** 3, 5, ms_also, ws), "unit": UNIT, "steps": 5, "ms_per_step": ms_also / 5,
+                        "repetitions_ms_per_step": [x / 5 for x in also["ms_reps"]],
+                        "roofline": _roofline(n5, ms_also / 5, False, peak, peak_kind, fp5[0], fp5[1]),
+                        "clocks": also["clocks"], "gpu_launches": int(also["launches"]),
+                        "with_cfl_dt_ms_per_step": med(also["ms_cfl"]) / 5}
+    elif also:
+        line["also"] = also
     if ws == 1 and not args.no_cpu_baseline:
-        val, _, cores, sample = _time_oracle(w, args.ref_side, 2, 0)
-        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        line["cpu_baseline"] = _cpu_baseline(w)
     print(json.dumps(line))
     if ws > 1:
         dist.destroy_process_group()
@@ -310,6 +400,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--reps", type=int, default=0, help="repetitions of the K-step region (default 5; 3 at 1024^3)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", type=int, default=4, help="BASELINE.json config number (4 = 512^3, 5 = 1024^3)")
     ap.add_argument("--chunk", type=int, default=0)
@@ -317,8 +408,9 @@ def main():
     ap.add_argument("--flatten3d", action="store_true", help="fully 3-D shock-flattening mode (SURVEY 8(f) NEXT-1): one more light kernel per step")
     ap.add_argument("--direct", action="store_true", help="direct global-memory sweep path instead of the bulk-staged one")
     ap.add_argument("--e2e-steps", type=int, default=2)
-    ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window")
+    ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window (--impl reference)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="skip the 1024^3 entry of the default run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

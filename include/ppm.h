@@ -89,8 +89,9 @@ int ppm_create(ppm_ctx **out, const ppm_params *prm, float *dev_buf_a, float *de
  * SURVEY 8(c) C1).  Asynchronous w.r.t. the host only if the sources are device or pinned memory. */
 int ppm_set_state(ppm_ctx *ctx, const float *const fields[PPM_NFIELDS], int z0, int nz_slab, int src_is_device);
 
-/* Inverse of ppm_set_state (full rho = rho0 + rho', p = p0 + p'); synchronises the stream before
- * returning and reports the sticky state flag. */
+/* Inverse of ppm_set_state (full rho = rho0 + rho', p = p0 + p').  Host destinations: synchronises the
+ * stream before returning and reports the sticky state flag.  Device destinations: only enqueues work on the context's
+ * stream (the arrays are valid in stream order; the flag is reported by the next synchronising call). */
 int ppm_get_state(ppm_ctx *ctx, float *const fields[PPM_NFIELDS], int z0, int nz_slab, int dst_is_device);
 
 /* One timestep = three 1-D sweeps (ghost fill, PPM hydro, PPB remap fused) with the same dt (PAPER.md L87
@@ -157,6 +158,12 @@ int ppm_plan_tail_chunk(int tail_tiles, int resident_ctas, int n);
 
 /* Number of kernel launches the context has enqueued so far (bench.py reports it). */
 long long ppm_launch_count(const ppm_ctx *ctx);
+
+/* Measurement hook (the FP32 roofline "must be measured with an FMA micro-benchmark at the clock the
+ * sweep actually runs at"): runs a register-only FFMA kernel on the context's device and stream (16 independent chains
+ * per thread, best of 5) and returns the achieved fp32 rate in Tflop/s (2 flop per FFMA lane) in *tflops_out [host].
+ * Synchronises the stream; touches no state. */
+int ppm_measure_fp32_peak(ppm_ctx *ctx, double *tflops_out);
 
 void ppm_destroy(ppm_ctx *ctx);
 const char *ppm_last_error(const ppm_ctx *ctx); /* never NULL; "" if no error; ctx may be NULL */

@@ -22,7 +22,7 @@ GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
-           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_destroy", "ppm_last_error")
+           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_destroy", "ppm_last_error")
 OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED = 2, 3, 4
 
 
@@ -67,6 +67,7 @@ def lib():
         L.ppm_plan_tail_chunk.argtypes = [C.c_int, C.c_int, C.c_int]
         L.ppm_launch_count.argtypes = [C.c_void_p]
         L.ppm_launch_count.restype = C.c_longlong
+        L.ppm_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.ppm_destroy.argtypes = [C.c_void_p]
         L.ppm_destroy.restype = None
         L.ppm_last_error.argtypes = [C.c_void_p]
@@ -149,8 +150,8 @@ class PPM:
 
     # ---- marshalling helpers ----
     def _ptrs(self, t):
-        """t: torch tensor [15, nzs, ny, nx] float32 contiguous (device or host) -> float*[15]"""
-        assert t.dtype == torch.float32 and t.is_contiguous() and t.shape[0] == NF
+        """t: torch tensor [15, nzs, ny, nx] float32 (device or host), every field a dense [nzs][ny][nx] block -> float*[15]"""
+        assert t.dtype == torch.float32 and t.shape[0] == NF and t[0].is_contiguous()
         fp = C.POINTER(C.c_float)
         stride = t.stride(0) * 4
         base = t.data_ptr()
@@ -173,6 +174,74 @@ class PPM:
                               device=device if device is not None else self.device)
         self._check(lib().ppm_get_state(self._h, self._ptrs(out), int(z0), int(nzs), int(out.is_cuda)))
         return out
+
+    def step_host_pipelined(self, host_ins, host_outs, dt, orders, slab=32, step=None):
+        """End-to-end helper for host-resident grids (argument marshalling and stream plumbing only: every byte is moved
+        by cudaMemcpyAsync or by the library's conversion kernels).  For s = 0, 1, ...: upload host_ins[s], advance it one
+        step (order orders[s]), download the result into host_outs[s].  All host tensors are pinned [15, nz, ny, nx]
+        float32.  The grids are independent of one another, so the upload of grid s+1 (copy stream `up`, z-slabs through
+        two device staging slabs, ppm_set_state from device memory) runs while grid s is downloaded (ppm_get_state into
+        two more staging slabs, copy stream `down`): PCIe carries both directions at once.  Returns after the last
+        download has finished."""
+        nx, ny, nz = self.n
+        step = step or self.step
+        dev, main = self.device, self.stream
+        if getattr(self, "_pipe", None) is None or self._pipe[0] != slab:
+            mk = lambda: torch.empty((NF, slab, ny, nx), dtype=torch.float32, device=dev)
+            with torch.cuda.device(dev):
+                self._pipe = (slab, [mk(), mk()], [mk(), mk()], torch.cuda.Stream(dev), torch.cuda.Stream(dev))
+        _, stg_in, stg_out, up, down = self._pipe
+        slabs = [(z0, min(slab, nz - z0)) for z0 in range(0, nz, slab)]
+        K = len(host_ins)
+        in_ready, in_free, out_free = [None, None], [None, None], [None, None]
+        nxt = [0, 0]                                   # (grid, slab index) of the next upload to enqueue
+
+        def enqueue_upload():
+            s, k = nxt
+            if s >= K:
+                return
+            b = (s * len(slabs) + k) % 2
+            z0, nzs = slabs[k]
+            with torch.cuda.stream(up):
+                if in_free[b] is not None:
+                    up.wait_event(in_free[b])          # the conversion that read this staging slab is done
+                for f in range(NF):
+                    stg_in[b][f, :nzs].copy_(host_ins[s][f, z0:z0 + nzs], non_blocking=True)
+                in_ready[b] = up.record_event()
+            nxt[0], nxt[1] = (s, k + 1) if k + 1 < len(slabs) else (s + 1, 0)
+
+        def convert_upload(s, k):
+            b = (s * len(slabs) + k) % 2
+            z0, nzs = slabs[k]
+            main.wait_event(in_ready[b])
+            self._check(lib().ppm_set_state(self._h, self._ptrs(stg_in[b][:, :nzs]), int(z0), int(nzs), 1))
+            in_free[b] = main.record_event()
+
+        with torch.cuda.device(dev):
+            enqueue_upload(); enqueue_upload()
+            for k in range(len(slabs)):                # grid 0 goes up alone
+                convert_upload(0, k)
+                enqueue_upload()
+            for s in range(K):
+                step(dt, orders[s])
+                for k, (z0, nzs) in enumerate(slabs):
+                    b = k % 2
+                    if out_free[b] is not None:
+                        main.wait_event(out_free[b])   # the download that read this staging slab is done
+                    view = stg_out[b][:, :nzs]
+                    self._check(lib().ppm_get_state(self._h, self._ptrs(view), int(z0), int(nzs), 1))
+                    ev = main.record_event()
+                    with torch.cuda.stream(down):
+                        down.wait_event(ev)
+                        for f in range(NF):
+                            host_outs[s][f, z0:z0 + nzs].copy_(view[f], non_blocking=True)
+                        out_free[b] = down.record_event()
+                    if s + 1 < K:                      # slab k of the state is free again: the next grid's slab k moves in
+                        convert_upload(s + 1, k)
+                        enqueue_upload()
+            down.synchronize()
+            main.synchronize()
+        self.sync()
 
     def step(self, dt, order=0):
         self._check(lib().ppm_step(self._h, float(dt), int(order)))
@@ -205,6 +274,12 @@ class PPM:
 
     def axis_path(self, axis):
         return int(lib().ppm_axis_path(self._h, int(axis)))
+
+    def measure_fp32_peak(self):
+        """achieved Tflop/s of a register-only FFMA kernel on this device (bench.py's roofline.alu denominator)"""
+        v = C.c_double()
+        self._check(lib().ppm_measure_fp32_peak(self._h, C.byref(v)))
+        return v.value
 
     def launch_count(self):
         return int(lib().ppm_launch_count(self._h))

@@ -192,7 +192,9 @@ extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z
     const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     for (int f = 0; f < PPM_NFIELDS; ++f)
         CU(cudaMemcpyAsync(fields[f], scratch + f * tot, sizeof(float) * tot, kind, c->stream));
-    return read_flag(c);
+    // host destinations: wait and report the state flag.  Device destinations are stream-ordered like everything else
+    // the library enqueues, so the call stays asynchronous (slab pipelines: PPM.step_host_pipelined in binding.py)
+    return dst_is_device ? PPM_OK : read_flag(c);
 }
 
 extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
@@ -295,3 +297,11 @@ extern "C" int ppm_plan_tail_chunk(int tail_tiles, int resident_ctas, int n) {
 }
 
 extern "C" long long ppm_launch_count(const ppm_ctx* c) { return c ? c->launches : 0; }
+
+extern "C" int ppm_measure_fp32_peak(ppm_ctx* c, double* tflops_out) {
+    if (!c) { set_err(nullptr, "ppm_measure_fp32_peak: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
+    if (!tflops_out) { set_err(c, "ppm_measure_fp32_peak: tflops_out is NULL"); return PPM_EINVAL; }
+    CU(ppm_run_fma_peak(c, tflops_out));
+    return PPM_OK;
+}

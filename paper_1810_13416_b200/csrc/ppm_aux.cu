@@ -315,6 +315,23 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
     F3[brick * 64 + c] = F;
 }
 
+// FP32 pipe micro-benchmark (the denominator of bench.py's roofline.alu; "must be measured with an FMA
+// micro-benchmark at the clock the sweep actually runs at"): 16 independent FFMA chains per thread, 8 resident warps
+// per scheduler; 2 flop per lane per FFMA.
+__global__ void __launch_bounds__(256) fma_peak_kernel(float* out, int iters, float a, float b) {
+    float x[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) x[k] = (float)(threadIdx.x + k) * 1e-3f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) x[k] = fmaf(x[k], a, b);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += x[k];
+    if (s == 123.456f) out[0] = s;          // never true: keeps the chains alive
+}
+
 AuxParams make_aux(const ppm_ctx* c) {
     AuxParams A;
     const ppm_params& p = c->prm;
@@ -370,6 +387,30 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c) {
     cfl_kernel<<<grid_for(n / 2, c->sms * 8), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->cflmax, c->flag);
     c->launches += 1;
     return cudaGetLastError();
+}
+
+cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops) {
+    const int iters = 4096, blocks = c->sms * 8, reps = 5;
+    cudaEvent_t e0, e1;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    double best = 0.0;
+    for (int r = 0; r < reps + 1 && e == cudaSuccess; ++r) {          // first pass is a warm-up
+        cudaEventRecord(e0, c->stream);
+        fma_peak_kernel<<<blocks, 256, 0, c->stream>>>(reinterpret_cast<float*>(c->result), iters, 0.999f, 1e-3f);
+        cudaEventRecord(e1, c->stream);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * 16.0 * iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        if (r > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    c->launches += reps + 1;
+    *tflops = best;
+    return e == cudaSuccess ? cudaGetLastError() : e;
 }
 
 cudaError_t ppm_launch_conserved(ppm_ctx* c) {

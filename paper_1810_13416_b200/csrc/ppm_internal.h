@@ -84,3 +84,4 @@ cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z
 cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
+cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);

@@ -23,7 +23,7 @@ def lib():
 def test_library_exports_every_declared_symbol(lib):
     hdr = open(os.path.join(ROOT, "include", "ppm.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(ppm_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(ppm_[a-z0-9_]+)\s*\(", hdr))
     assert {"ppm_create", "ppm_set_state", "ppm_step", "ppm_get_state", "ppm_reduce_conserved", "ppm_cfl_dt"} <= declared
     L = lib.lib()
     for name in declared:

@@ -534,6 +534,32 @@ def test_state_flag_reports_floor_hits_and_bad_states():
     g.close()
 
 
+def test_host_pipelined_exchange_equals_serial_set_step_get():
+    """the end-to-end helper of bench.py's e2e leg (binding.PPM.step_host_pipelined: slab-wise upload of grid s+1 on one copy
+    stream while grid s comes down on another, ppm_set_state / ppm_get_state with device staging slabs) returns bit for
+    bit what ppm_set_state(host) -> ppm_step -> ppm_get_state(host) returns, ragged last slab included"""
+    PPM = _gpu()
+    w = W.make(4, n=40)
+    f0 = w.fields()
+    f1 = f0.clone()
+    f1[1:4] *= 0.5
+    ins = [f0.pin_memory(), f1.pin_memory(), f0.pin_memory()]
+    g = PPM.from_workload(w)
+    g.set_state(f0.cuda())
+    dt = 0.7 * g.cfl_dt(w.cfl)
+    ref = []
+    for s, fi in enumerate(ins):
+        g.set_state(fi)
+        g.step(dt, s)
+        ref.append(g.get_state(device="cpu").numpy().copy())
+    outs = [torch.empty_like(fi).pin_memory() for fi in ins]
+    g.step_host_pipelined(ins, outs, dt, [0, 1, 2], slab=16)
+    for r, o in zip(ref, outs):
+        assert np.array_equal(r, o.numpy())
+    assert not np.array_equal(ref[0], ref[1])
+    g.close()
+
+
 def test_hydrostatic_state_is_preserved_exactly_on_gpu():
     PPM = _gpu()
     for cfg, n in ((2, 32), (4, 32)):
