@@ -22,12 +22,16 @@ def _deps():
     return deps
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, poison: bool = False) -> str:
+    """poison=True: the debug variant libppm_b200_poison.so (-DPPM_DEBUG_POISON: dead ring slots of the bulk-staged sweeps
+    are filled with NaN before they are refilled, so a read that races a bulk copy shows up as NaN in the parity tests);
+    load it with PPM_B200_LIB=<path>."""
+    LIB = globals()["LIB"] if not poison else os.path.join(HERE, "libppm_b200_poison.so")
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
     cmd = [NVCC, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-ftz=true",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-           "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+           "-o", LIB] + (["-DPPM_DEBUG_POISON"] if poison else []) + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")
@@ -36,4 +40,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="--verbose" in sys.argv))
+    print(build(force=True, verbose="--verbose" in sys.argv, poison="--poison" in sys.argv))

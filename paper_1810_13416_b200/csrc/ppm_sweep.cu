@@ -1053,6 +1053,22 @@ struct IoBulk {
             const int k = n >> 2;
             if (S >= 0 || k != k0) {
                 __syncwarp();
+#ifdef PPM_DEBUG_POISON
+                // debug build (compute-sanitizer's racecheck is not available on this pool): once the bulk stores that read
+                // the two dead slots have completed, every lane fills them with NaN before the refill is issued.  A lane
+                // that reads a slot before its load has landed, or a slot other than the one it should, then produces NaN
+                // instead of plausible stale data, and the parity tests fail loudly.
+                if (lane == 0) tma_wait_read0();
+                __syncwarp();
+                {
+                    const int dh = (hs == G::NH - 1 ? 0 : hs + 1) * G::HSLOT, dp = (ps ^ 1) * G::PSLOT;
+                    const bool rh = S >= 0 || (k + 1 >= k0 + G::NH && k + 1 <= kend), rp = S >= 0 || (k >= k0 + G::NP && k <= kend);
+                    for (int e = lane; e < G::HSLOT; e += 32) if (rh) hyd0[dh + e] = __int_as_float(0x7fc00000);
+                    for (int e = lane; e < G::PSLOT; e += 32) if (rp) ppr0[dp + e] = __int_as_float(0x7fc00000);
+                    fence_async_smem();
+                    __syncwarp();
+                }
+#endif
                 if (lane == 0) {
                     tma_wait_read0();
                     if (S >= 0 || (k + 1 >= k0 + G::NH && k + 1 <= kend)) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
