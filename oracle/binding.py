@@ -44,6 +44,9 @@ def lib():
         L.oracle_flatten3d_field.argtypes = [C.c_void_p]
         L.oracle_flatten3d_field.restype = C.POINTER(C.c_double)
         L.oracle_cfl_dt.argtypes = [C.c_void_p, C.c_double, dp]
+        L.oracle_set_sphere.argtypes = [C.c_void_p, C.c_int, C.c_double, dp]
+        L.oracle_cell_is_solid.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+        L.oracle_spin_up.argtypes = [C.c_void_p, C.c_double]
         L.oracle_reduce_conserved.argtypes = [C.c_void_p, dp]
         L.oracle_h1_face.restype = C.c_double
         L.oracle_h1_face.argtypes = [C.c_double] * 4
@@ -252,6 +255,25 @@ class Oracle:
             lib().oracle_flatten3d_update(self._h)
         ptr = lib().oracle_flatten3d_field(self._h)
         return np.ctypeslib.as_array(ptr, shape=self.shape).copy()
+
+    def set_sphere(self, radius, center):
+        """NEXT-3: confining sphere; radius <= 0 switches it off"""
+        cen = (C.c_double * 3)(*[float(v) for v in center])
+        rc = lib().oracle_set_sphere(self._h, int(radius > 0), float(radius), cen)
+        if rc:
+            raise ValueError("oracle_set_sphere rc=%d" % rc)
+
+    def solid_mask(self):
+        """bool [nz][ny][nx]: cells whose centre lies outside the confining sphere"""
+        nz, ny, nx = self.shape
+        L = lib()
+        return np.array([[[bool(L.oracle_cell_is_solid(self._h, i, j, k)) for i in range(nx)] for j in range(ny)]
+                         for k in range(nz)])
+
+    def spin_up(self, domega):
+        """NEXT-3: one increment of the solid-body rotation ramp about z"""
+        rc = lib().oracle_spin_up(self._h, float(domega))
+        assert rc == 0
 
     def sweep(self, d, dt):
         rc = lib().oracle_sweep(self._h, d, dt)

@@ -57,6 +57,8 @@ typedef struct oracle_ctx {
     double *qn[NF];      /* sweep output */
     int flat3d;          /* NEXT-1: fully 3-D shock detector instead of the per-sweep 1-D one */
     double *F3;          /* F~ of every cell (flat3d only), evaluated on the state at the start of the call */
+    int sphere;          /* NEXT-3: confining sphere */
+    double sph_r, sph_c[3]; /* its radius and centre (physical units) */
 } oracle_ctx;
 
 static double clamp01(double x) { return fmin(1.0, fmax(0.0, x)); }
@@ -569,6 +571,9 @@ int oracle_get_state(const oracle_ctx *c, double *const fields[NF]) {
 /* raw perturbation-form access (for tests) */
 double *oracle_raw_field(oracle_ctx *c, int f) { return c->q[f]; }
 
+static int sweep_impl_sphere(oracle_ctx *c, int d, double dt);   /* NEXT-3, below */
+static int cell_is_solid(const oracle_ctx *c, int gi, int gj, int gk);
+
 /* C2/C3/C4/C5: one sweep along d over every pencil of the window. */
 static int sweep_impl(oracle_ctx *c, int d, double dt) {
     const int n = c->n[d];
@@ -684,6 +689,7 @@ const double *oracle_flatten3d_field(const oracle_ctx *c) { return c ? c->F3 : N
 /* one sweep on its own; in 3-D flattening mode F~ is evaluated on the state this sweep starts from */
 int oracle_sweep(oracle_ctx *c, int d, double dt) {
     if (!c || d < 0 || d > 2 || !(dt > 0.0)) return 1;
+    if (c->sphere) return c->flat3d ? 1 : sweep_impl_sphere(c, d, dt);   /* (the two NEXT modes are not combined) */
     if (c->flat3d) oracle_flatten3d_update(c);
     return sweep_impl(c, d, dt);
 }
@@ -692,9 +698,10 @@ int oracle_sweep(oracle_ctx *c, int d, double dt) {
 static const int ORDERS[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
 int oracle_step(oracle_ctx *c, double dt, int sweep_order) {
     if (!c || !(dt > 0.0) || sweep_order < 0 || sweep_order > 5) return 1;
+    if (c->sphere && c->flat3d) return 1;
     if (c->flat3d) oracle_flatten3d_update(c);      /* once per step, on the step's starting state */
     for (int s = 0; s < 3; ++s) {
-        int rc = sweep_impl(c, ORDERS[sweep_order][s], dt);
+        int rc = c->sphere ? sweep_impl_sphere(c, ORDERS[sweep_order][s], dt) : sweep_impl(c, ORDERS[sweep_order][s], dt);
         if (rc) return rc;
     }
     return 0;
@@ -747,6 +754,170 @@ int oracle_advect(oracle_ctx *c, double dt, int sweep_order) {
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT-3: "our star is enclosed in an impenetrable and immovable sphere that is
+ * inscribed in the cubical domain of our uniform Cartesian grid ... a very simple boundary condition at the sphere".
+ * [reading R23, DESIGN.md]  A cell is SOLID when its centre lies outside the sphere,
+ *     ((X - cx)^2 + (Y - cy)^2) + (Z - cz)^2 > R^2      (fp64, each operation rounded, this association),
+ * and is never changed.  Along a pencil the fluid cells form one segment [lo, hi] (the sphere is convex); each face
+ * between a fluid and a solid cell is a reflecting wall for that sweep: the ghost cells beyond it are the mirror images
+ * ALONG THE PENCIL of the segment's own cells (C3: normal velocity and the FV coefficients odd in the normal direction
+ * change sign; base state of the mirror-image position, normal g odd), reflected again at the segment's other end when
+ * the segment is shorter than the four ghost cells.  So no mass crosses a solid face and a state at rest stays at rest.
+ * A segment end that lies on the window boundary keeps the boundary's own rule (REFLECT: the same mirror; OPEN).
+ * Reduces to the plain reflecting box when the sphere contains the whole grid.
+ * ---------------------------------------------------------------------------------------- */
+int oracle_set_sphere(oracle_ctx *c, int on, double radius, const double center[3]) {
+    if (!c) return 1;
+    if (on) {
+        if (!(radius > 0.0) || !center) return 1;
+        for (int d = 0; d < 3; ++d)
+            if (c->bc[2 * d] == OR_BC_PERIODIC) return 1;     /* a wall all round: periodic faces make no sense here */
+        c->sph_r = radius;
+        for (int d = 0; d < 3; ++d) c->sph_c[d] = center[d];
+    }
+    c->sphere = on ? 1 : 0;
+    return 0;
+}
+
+/* global cell (gi, gj, gk): 1 if its centre is outside the sphere */
+static int cell_is_solid(const oracle_ctx *c, int gi, int gj, int gk) {
+    if (!c->sphere) return 0;
+    double x = (gi + 0.5) * c->dx - c->sph_c[0], y = (gj + 0.5) * c->dx - c->sph_c[1], z = (gk + 0.5) * c->dx - c->sph_c[2];
+    double xx = x * x, yy = y * y, zz = z * z;
+    double s = xx + yy;
+    s = s + zz;
+    return s > c->sph_r * c->sph_r;
+}
+int oracle_cell_is_solid(const oracle_ctx *c, int i, int j, int k) {
+    return cell_is_solid(c, c->org[0] + i, c->org[1] + j, c->org[2] + k);
+}
+
+/* image of window-local cell index i along d for a fluid segment [lo, hi] whose ends are walls (lw / hw = 1) or the
+ * window's OPEN sides: source index, sign, and the global index whose position supplies the base state */
+static int segment_image_cell(const oracle_ctx *c, int d, int lo, int hi, int lw, int hw, int i, int *sgn, int *gpos) {
+    int s = i, sg = 1;
+    for (int it = 0; it < 64; ++it) {
+        if (s < lo) {
+            if (!lw) { *sgn = 1; *gpos = c->org[d] + i; return lo; }         /* OPEN: zero gradient, true position */
+            s = 2 * lo - 1 - s; sg = -sg;
+        } else if (s > hi) {
+            if (!hw) { *sgn = 1; *gpos = c->org[d] + i; return hi; }
+            s = 2 * hi + 1 - s; sg = -sg;
+        } else break;
+    }
+    *sgn = sg; *gpos = c->org[d] + s;
+    return s;
+}
+/* image of face index f (faces lo .. hi+1 bound the segment) -> global face index */
+static int segment_image_face(const oracle_ctx *c, int d, int lo, int hi, int lw, int hw, int f) {
+    int s = f;
+    for (int it = 0; it < 64; ++it) {
+        if (s < lo) { if (!lw) return c->org[d] + f; s = 2 * lo - s; }
+        else if (s > hi + 1) { if (!hw) return c->org[d] + f; s = 2 * (hi + 1) - s; }
+        else break;
+    }
+    return c->org[d] + s;
+}
+
+/* one sweep along d with the confining sphere: every pencil is cut down to its fluid segment */
+static int sweep_impl_sphere(oracle_ctx *c, int d, double dt) {
+    const int n = c->n[d];
+    const int d1 = (d == 0) ? 1 : 0, d2 = (d == 2) ? 1 : 2;
+    const int n1 = c->n[d1], n2 = c->n[d2];
+    const int iu = 1 + d, iv = 1 + d1, iw = 1 + d2;
+    int fail = 0;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int b = 0; b < n2; ++b)
+        for (int a = 0; a < n1; ++a) {
+            int ijk[3], gidx[3];
+            ijk[d1] = a; ijk[d2] = b;
+            gidx[d1] = c->org[d1] + a; gidx[d2] = c->org[d2] + b;
+            /* the solid cells keep their state */
+            for (int i = 0; i < n; ++i) {
+                ijk[d] = i;
+                size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                for (int f = 0; f < NF; ++f) c->qn[f][id] = c->q[f][id];
+            }
+            int lo = -1, hi = -2;
+            for (int i = 0; i < n; ++i) {
+                gidx[d] = c->org[d] + i;
+                if (!cell_is_solid(c, gidx[0], gidx[1], gidx[2])) { if (lo < 0) lo = i; hi = i; }
+            }
+            if (lo < 0) continue;                                   /* no fluid on this pencil */
+            const int L = hi - lo + 1, nt = L + 2 * NG;
+            const int lw = (lo > 0) || c->bc[2 * d] == OR_BC_REFLECT, hw = (hi < n - 1) || c->bc[2 * d + 1] == OR_BC_REFLECT;
+            double *buf = (double *)malloc(sizeof(double) * ((size_t)nt * 21 + 2 + (size_t)L * 15));
+            if (!buf) { fail = 1; continue; }
+            double *qa[5], *ma[10], *r0c, *p0c, *gd, *r0f, *p0f, *qo[5], *mo[10];
+            double *cur = buf;
+            for (int k = 0; k < 5; ++k) { qa[k] = cur; cur += nt; }
+            for (int k = 0; k < 10; ++k) { ma[k] = cur; cur += nt; }
+            r0c = cur; cur += nt; p0c = cur; cur += nt; gd = cur; cur += nt;
+            r0f = cur; cur += nt + 1; p0f = cur; cur += nt + 1;
+            cur += nt;
+            for (int k = 0; k < 5; ++k) { qo[k] = cur; cur += L; }
+            for (int k = 0; k < 10; ++k) { mo[k] = cur; cur += L; }
+            for (int j = 0; j < nt; ++j) {
+                int sgn, gpos;
+                int s = segment_image_cell(c, d, lo, hi, lw, hw, lo + j - NG, &sgn, &gpos);
+                ijk[d] = s; gidx[d] = gpos;
+                size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                qa[0][j] = c->q[0][id];
+                qa[1][j] = sgn * c->q[iu][id];
+                qa[2][j] = c->q[iv][id];
+                qa[3][j] = c->q[iw][id];
+                qa[4][j] = c->q[4][id];
+                for (int k = 0; k < 10; ++k) ma[k][j] = (ppb_is_odd(d, k) ? sgn : 1) * c->q[5 + k][id];
+                double gv[3];
+                cell_base(c, gidx[0], gidx[1], gidx[2], &r0c[j], &p0c[j], gv);
+                gd[j] = sgn * gv[d];
+            }
+            for (int f = 0; f <= nt; ++f) {
+                int gf = segment_image_face(c, d, lo, hi, lw, hw, lo + f - NG);
+                double X[3], gv[3];
+                X[d1] = (gidx[d1] + 0.5) * c->dx; X[d2] = (gidx[d2] + 0.5) * c->dx; X[d] = gf * c->dx;
+                base_at(c, X, &r0f[f], &p0f[f], gv);
+            }
+            oracle_sweep_pencil(L, d, c->dx, dt, c->gamma, c->rho_floor, c->p_floor,
+                                (const double *const *)qa, (const double *const *)ma, r0c, p0c, gd, r0f, p0f, qo, mo, NULL);
+            for (int i = 0; i < L; ++i) {
+                ijk[d] = lo + i;
+                size_t id = cidx(c, ijk[0], ijk[1], ijk[2]);
+                c->qn[0][id] = qo[0][i];
+                c->qn[iu][id] = qo[1][i];
+                c->qn[iv][id] = qo[2][i];
+                c->qn[iw][id] = qo[3][i];
+                c->qn[4][id] = qo[4][i];
+                for (int k = 0; k < 10; ++k) c->qn[5 + k][id] = mo[k][i];
+            }
+            free(buf);
+        }
+    if (fail) return 2;
+    for (int f = 0; f < NF; ++f) { double *t = c->q[f]; c->q[f] = c->qn[f]; c->qn[f] = t; }
+    return 0;
+}
+
+/* NEXT-3 ("We treat the rotation by adding a solid body rotational flow component to our simulation
+ * gradually over the first several thousand time steps").  [reading R24]  One increment of that ramp: every fluid
+ * cell gets du = domega e_z x (X - centre), i.e. du_x = -domega (Y - cy), du_y = +domega (X - cx), about the sphere's
+ * centre (the gravity centre, else the origin, without a sphere); density and pressure are left as they are.  The
+ * caller applies it once per step, domega = Omega_target / N_ramp, for the first N_ramp steps. */
+int oracle_spin_up(oracle_ctx *c, double domega) {
+    if (!c) return 1;
+    const double *cen = c->sphere ? c->sph_c : c->center;
+    for (int k = 0; k < c->n[2]; ++k)
+        for (int j = 0; j < c->n[1]; ++j)
+            for (int i = 0; i < c->n[0]; ++i) {
+                if (cell_is_solid(c, c->org[0] + i, c->org[1] + j, c->org[2] + k)) continue;
+                size_t id = cidx(c, i, j, k);
+                double x = (c->org[0] + i + 0.5) * c->dx - cen[0], y = (c->org[1] + j + 0.5) * c->dx - cen[1];
+                c->q[1][id] += -domega * y;
+                c->q[2][id] += domega * x;
+            }
+    return 0;
+}
+
 /* C6 */
 int oracle_cfl_dt(const oracle_ctx *c, double cfl, double *dt_out) {
     double vmax = 0.0;
@@ -755,6 +926,7 @@ int oracle_cfl_dt(const oracle_ctx *c, double cfl, double *dt_out) {
             for (int i = 0; i < c->n[0]; ++i) {
                 size_t id = cidx(c, i, j, k);
                 double r0, p0, gv[3];
+                if (cell_is_solid(c, c->org[0] + i, c->org[1] + j, c->org[2] + k)) continue;     /* NEXT-3: fluid cells only */
                 cell_base(c, c->org[0] + i, c->org[1] + j, c->org[2] + k, &r0, &p0, gv);
                 double rho = r0 + c->q[0][id], p = p0 + c->q[4][id];
                 double cs = sqrt(c->gamma * p / rho);
@@ -772,6 +944,7 @@ int oracle_reduce_conserved(const oracle_ctx *c, double out[6]) {
             for (int i = 0; i < c->n[0]; ++i) {
                 size_t id = cidx(c, i, j, k);
                 double r0, p0, gv[3];
+                if (cell_is_solid(c, c->org[0] + i, c->org[1] + j, c->org[2] + k)) continue;     /* NEXT-3: fluid cells only */
                 cell_base(c, c->org[0] + i, c->org[1] + j, c->org[2] + k, &r0, &p0, gv);
                 double rho = r0 + c->q[0][id], p = p0 + c->q[4][id];
                 double u = c->q[1][id], v = c->q[2][id], w = c->q[3][id];
