@@ -147,6 +147,24 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    (PPM_ENOMEM if that fails) and adds one light kernel launch per step. */
 enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
+/* Confining sphere ("our star is enclosed in an impenetrable and immovable sphere that
+ * is inscribed in the cubical domain of our uniform Cartesian grid ... a very simple boundary condition at the sphere";
+ * reading R23 in DESIGN.md).  A cell whose centre lies outside the sphere of this radius about center[3] [host] (physical
+ * units; the paper's case: radius = half the box, centre = box centre) is SOLID: it is never changed and never read by
+ * the flow.  In every sweep each grid pencil is cut down to its fluid segment, whose two ends are reflecting walls (the
+ * ghost cells are the mirror images along the pencil, C3), so no mass crosses the sphere.  ppm_cfl_dt and
+ * ppm_reduce_conserved then run over the fluid cells only.  radius <= 0 switches the sphere off.
+ * PPM_EINVAL unless all six faces are PPM_BC_REFLECT, the extents are multiples of 4, gravity is NONE or RADIAL, and
+ * neither PPM_OPT_FLATTEN3D nor PPM_OPT_IO_PATH = 1 is set.  Host-side state only (no launch). */
+int ppm_set_sphere(ppm_ctx *ctx, double radius, const double center[3]);
+
+/* One increment of the rotation spin-up ("We treat the rotation by adding a solid body rotational flow
+ * component to our simulation gradually over the first several thousand time steps"; reading R24): every fluid cell gets
+ * du = domega e_z x (X - centre), i.e. du_x = -domega (Y - cy), du_y = +domega (X - cx), about the sphere's centre (the
+ * gravity centre without a sphere); rho and p are left as they are.  The caller applies it once per step with
+ * domega = Omega_target / N_ramp during the first N_ramp steps.  Only enqueues work (1 light kernel launch). */
+int ppm_spin_up(ppm_ctx *ctx, double domega);
+
 /* 1 if the next sweep along axis (0,1,2) will take the bulk-staged path, 0 if the direct path. */
 int ppm_axis_path(const ppm_ctx *ctx, int axis);
 

@@ -228,6 +228,7 @@ extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
     if (!c) { set_err(nullptr, "ppm_advect: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_advect: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
+    if (c->sphere) { set_err(c, "ppm_advect: the PPB-only mode has no confining sphere"); return PPM_EINVAL; }
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt, true));
     return PPM_OK;
 }
@@ -274,6 +275,9 @@ extern "C" int ppm_set_chunk(ppm_ctx* c, int chunk_cells) {
 extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (!c) { set_err(nullptr, "ppm_set_option: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);
+    if (c->sphere && ((option == PPM_OPT_IO_PATH && value == 1) || (option == PPM_OPT_FLATTEN3D && value == 1))) {
+        set_err(c, "ppm_set_option: not together with the confining sphere"); return PPM_EINVAL;
+    }
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
     if (option == PPM_OPT_CFL_FUSED && (value == 0 || value == 1)) { c->cfl_fused = value; c->cfl_valid = 0; return PPM_OK; }
     if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
@@ -287,6 +291,31 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     }
     set_err(c, "ppm_set_option: unknown option %d or value %d", option, value);
     return PPM_EINVAL;
+}
+
+extern "C" int ppm_set_sphere(ppm_ctx* c, double radius, const double center[3]) {
+    if (!c) { set_err(nullptr, "ppm_set_sphere: ctx is NULL"); return PPM_EINVAL; }
+    if (!(radius > 0.0)) { c->sphere = 0; c->cfl_valid = 0; return PPM_OK; }
+    if (!center) { set_err(c, "ppm_set_sphere: center is NULL"); return PPM_EINVAL; }
+    for (int k = 0; k < 6; ++k)
+        if (c->prm.bc[k] != PPM_BC_REFLECT) { set_err(c, "ppm_set_sphere: the confining sphere needs reflecting walls on all six faces"); return PPM_EINVAL; }
+    if ((c->prm.nx | c->prm.ny | c->prm.nz) & 3) { set_err(c, "ppm_set_sphere: grid extents must be multiples of 4 (the sphere runs on the bulk-staged sweeps)"); return PPM_EINVAL; }
+    if (c->prm.grav.kind == PPM_GRAV_CONST_Z) { set_err(c, "ppm_set_sphere: not with plane-parallel (CONST_Z) gravity"); return PPM_EINVAL; }
+    if (c->flat3d) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_FLATTEN3D"); return PPM_EINVAL; }
+    if (c->io_path != 0) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_IO_PATH = 1"); return PPM_EINVAL; }
+    c->sphere = 1; c->sph_r = radius;
+    for (int d = 0; d < 3; ++d) c->sph_c[d] = center[d];
+    c->cfl_valid = 0;
+    return PPM_OK;
+}
+
+extern "C" int ppm_spin_up(ppm_ctx* c, double domega) {
+    if (!c) { set_err(nullptr, "ppm_spin_up: ctx is NULL"); return PPM_EINVAL; }
+    DevGuard guard(c);
+    if (!isfinite(domega)) { set_err(c, "ppm_spin_up: domega is not finite"); return PPM_EINVAL; }
+    c->cfl_valid = 0;
+    CU(ppm_launch_spin_up(c, domega));
+    return PPM_OK;
 }
 
 extern "C" int ppm_axis_path(const ppm_ctx* c, int axis) { return (c && axis >= 0 && axis <= 2 && ppm_axis_is_bulk(c, axis)) ? 1 : 0; }

@@ -15,7 +15,18 @@ struct AuxParams {
     int bc[6];
     const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
     float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
+    int sphere;                         // NEXT-3: confining sphere on
+    double sph_r2, sph_cx, sph_cy, sph_cz;
 };
+
+// NEXT-3 (reading R23): a cell is solid when its centre lies outside the sphere — the oracle's criterion, operation by
+// operation in fp64 with no contraction: ((X-cx)^2 + (Y-cy)^2) + (Z-cz)^2 > R^2
+__device__ __forceinline__ bool aux_is_solid(const AuxParams& A, int i, int j, int k) {
+    if (!A.sphere) return false;
+    const double x = __dsub_rn(__dmul_rn((double)i + 0.5, A.dx), A.sph_cx), y = __dsub_rn(__dmul_rn((double)j + 0.5, A.dx), A.sph_cy),
+                 z = __dsub_rn(__dmul_rn((double)k + 0.5, A.dx), A.sph_cz);
+    return __dadd_rn(__dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)), __dmul_rn(z, z)) > A.sph_r2;
+}
 
 // float offset of field 0 of cell (i,j,k): brick record [bz][by][bx][15][4z][4y][4x]; field f is 64*f further
 __device__ __forceinline__ long long cell_offset(const AuxParams& A, int i, int j, int k) {
@@ -144,6 +155,7 @@ __global__ void __launch_bounds__(256) cfl_kernel(const AuxParams A, const float
             const int c = lane + 32 * h;
             const int i = bx * 4 + (c & 3), j = by * 4 + ((c >> 2) & 3), k = bz * 4 + (c >> 4);
             if (i >= A.nx || j >= A.ny || k >= A.nz) continue;             // pad cell of a ragged grid
+            if (aux_is_solid(A, i, j, k)) continue;                        // outside the confining sphere: not part of the flow
             const float2 b0 = base32(A, i, j, k);                          // fp32 base state, as the sweeps evaluate it
             const float rho = b0.x + v[h][0], pr = b0.y + v[h][4];
             const float xs = gam * pr * __fdividef(1.0f, rho);
@@ -171,6 +183,7 @@ __global__ void __launch_bounds__(256) conserved_kernel(AuxParams A, const float
         int i, j, k;
         long long o;
         if (!cell_of(A, t, i, j, k, o)) continue;
+        if (aux_is_solid(A, i, j, k)) continue;            // NEXT-3: the sums run over the fluid cells
         double r0, p0;
         base64(A, i, j, k, r0, p0);
         const double rho = r0 + (double)st[o], p = p0 + (double)st[o + 4 * 64];
@@ -315,6 +328,19 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
     F3[brick * 64 + c] = F;
 }
 
+// NEXT-3 ("adding a solid body rotational flow component ... gradually over the first several thousand
+// time steps"; reading R24): one increment of the ramp, du = domega e_z x (X - centre) on every fluid cell.
+__global__ void __launch_bounds__(256) spin_up_kernel(const AuxParams A, float* __restrict__ st, double domega, double cx, double cy) {
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
+        int i, j, k;
+        long long o;
+        if (!cell_of(A, t, i, j, k, o) || aux_is_solid(A, i, j, k)) continue;
+        const double x = ((double)i + 0.5) * A.dx - cx, y = ((double)j + 0.5) * A.dx - cy;
+        st[o + 64] = (float)((double)st[o + 64] - domega * y);
+        st[o + 2 * 64] = (float)((double)st[o + 2 * 64] + domega * x);
+    }
+}
+
 // FP32 pipe micro-benchmark (the denominator of bench.py's roofline.alu; "must be measured with an FMA
 // micro-benchmark at the clock the sweep actually runs at"): 16 independent FFMA chains per thread, 8 resident warps
 // per scheduler; 2 flop per lane per FFMA.
@@ -347,6 +373,7 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.tab32 = c->tab;
     A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
     A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
+    A.sphere = c->sphere; A.sph_r2 = c->sph_r * c->sph_r; A.sph_cx = c->sph_c[0]; A.sph_cy = c->sph_c[1]; A.sph_cz = c->sph_c[2];
     return A;
 }
 
@@ -385,6 +412,14 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c) {
     if (e != cudaSuccess) return e;
     const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
     cfl_kernel<<<grid_for(n / 2, c->sms * 8), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->cflmax, c->flag);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega) {
+    const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
+    const double cx = c->sphere ? c->sph_c[0] : c->prm.grav.center[0], cy = c->sphere ? c->sph_c[1] : c->prm.grav.center[1];
+    spin_up_kernel<<<grid_for(n, c->sms * 16), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], domega, cx, cy);
     c->launches += 1;
     return cudaGetLastError();
 }

@@ -43,6 +43,9 @@ struct SweepParams {
     const float2* __restrict__ tabg; // {g_k, g_k+1 - g_k}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
     unsigned int* cflmax;           // non-NULL: fold max_d |u_d| + c of every finished cell into it (bit pattern of a float >= 0)
+    // confining sphere (NEXT-3): centre along the (sweep, a, b) axes, radius^2, cell size — fp64, the oracle's criterion
+    int sphere;
+    double sph_dx, sph_r2, sph_cd, sph_ca, sph_cb;
     // 3-D flattening mode: F~ of every cell, [brick][4z][4y][4x] (a brick is 64 floats: strides = SB / 15); else NULL
     const float* flat;
     long long FBd, FBa, FBb;
@@ -66,6 +69,8 @@ struct ppm_ctx {
     int chunk;
     int nbx, nby, nbz;              // bricks per axis (extents rounded up to multiples of 4)
     int flat3d;                     // PPM_OPT_FLATTEN3D
+    int sphere;                     // ppm_set_sphere: confining sphere on (NEXT-3)
+    double sph_r, sph_c[3];         // its radius and centre
     float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
     int sms;                        // multiprocessors of the device
     int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state
@@ -85,3 +90,4 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
 cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);
+cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega);

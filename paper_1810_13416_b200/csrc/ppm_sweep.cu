@@ -352,6 +352,70 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
 }
 
 // =====================================================================================================
+// NEXT-3 (reading R23): the confining sphere.  A cell whose centre lies outside the sphere is
+// solid and never changes; along a pencil the fluid cells form one segment [lo, hi] whose ends are reflecting walls.
+// The rings of the bulk path stay warp-uniform (whole brick records travel, solid cells included); what is per lane
+// is only the image of the <= 4 ghost cells beyond each end of the lane's own segment, which are read straight from the
+// input buffer (the mirror cells have long left, or not yet entered, the register windows), and the predicate on the store.
+// =====================================================================================================
+struct Segment { int lo, hi; };     // empty: lo > hi
+
+// the oracle's criterion, operation by operation in fp64 with no contraction: ((X-cx)^2 + (Y-cy)^2) + (Z-cz)^2 > R^2
+template <int DIR>
+__device__ __forceinline__ bool sphere_inside(const SweepParams& P, double ta, double tb, int j) {
+    const double xd = __dsub_rn(__dmul_rn((double)j + 0.5, P.sph_dx), P.sph_cd);
+    const double dd = __dmul_rn(xd, xd);
+    // ta, tb: squared offsets along the transverse axes a < b (in axis order); assemble in x, y, z order
+    double sum;
+    if (DIR == 0) sum = __dadd_rn(__dadd_rn(dd, ta), tb);
+    else if (DIR == 1) sum = __dadd_rn(__dadd_rn(ta, dd), tb);
+    else sum = __dadd_rn(__dadd_rn(ta, tb), dd);
+    return !(sum > P.sph_r2);
+}
+template <int DIR>
+__device__ __forceinline__ Segment sphere_segment(const SweepParams& P, int a, int b) {
+    const double xa = __dsub_rn(__dmul_rn((double)a + 0.5, P.sph_dx), P.sph_ca), xb = __dsub_rn(__dmul_rn((double)b + 0.5, P.sph_dx), P.sph_cb);
+    const double ta = __dmul_rn(xa, xa), tb = __dmul_rn(xb, xb);
+    Segment sg; sg.lo = P.n; sg.hi = -1;
+    // the inside set is an interval around the cell nearest the centre (every operation above is monotone in |x - c|)
+    int seed = min(max((int)floor(P.sph_cd / P.sph_dx), 0), P.n - 1);
+    if (!sphere_inside<DIR>(P, ta, tb, seed)) {
+        if (seed + 1 < P.n && sphere_inside<DIR>(P, ta, tb, seed + 1)) seed += 1;
+        else if (seed > 0 && sphere_inside<DIR>(P, ta, tb, seed - 1)) seed -= 1;
+        else return sg;
+    }
+    const double h2 = P.sph_r2 - ta - tb;
+    const int reach = h2 > 0.0 ? (int)(sqrt(h2) / P.sph_dx) : 0;
+    int lo = max(seed - reach, 0), hi = min(seed + reach, P.n - 1);
+    while (lo < seed && !sphere_inside<DIR>(P, ta, tb, lo)) ++lo;          // the estimate is within a cell or two
+    while (lo > 0 && sphere_inside<DIR>(P, ta, tb, lo - 1)) --lo;
+    while (hi > seed && !sphere_inside<DIR>(P, ta, tb, hi)) --hi;
+    while (hi < P.n - 1 && sphere_inside<DIR>(P, ta, tb, hi + 1)) ++hi;
+    sg.lo = lo; sg.hi = hi;
+    return sg;
+}
+// image of cell index j / face index f under reflection at the segment's ends (again, if the segment is short)
+__device__ __forceinline__ int fold_cell(const Segment& g, int j, float& sgn) {
+    sgn = 1.0f;
+#pragma unroll 1
+    for (int it = 0; it < 16; ++it) {
+        if (j < g.lo) { j = 2 * g.lo - 1 - j; sgn = -sgn; }
+        else if (j > g.hi) { j = 2 * g.hi + 1 - j; sgn = -sgn; }
+        else break;
+    }
+    return j;
+}
+__device__ __forceinline__ int fold_face(const Segment& g, int f) {
+#pragma unroll 1
+    for (int it = 0; it < 16; ++it) {
+        if (f < g.lo) f = 2 * g.lo - f;
+        else if (f > g.hi + 1) f = 2 * (g.hi + 1) - f;
+        else break;
+    }
+    return f;
+}
+
+// =====================================================================================================
 // The marching body, shared by every data path.  IO supplies plane n (hydro), cell n-3 (PPB coefficients,
 // local family order, mirror signs applied) and takes the finished cell n-4.
 // =====================================================================================================
@@ -360,9 +424,11 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
 // CFL: S10 fused into the sweep — every finished cell folds max_d |u_d| + c of its NEW
 // state into vmax, so that the step's last sweep leaves the next step's CFL maximum behind and ppm_cfl_dt has no pass
 // of its own to make.
-template <int DIR, int GRAV, bool FLAT, bool CFL, class IO>
+// SPH: confining sphere (above); seg = this lane's fluid segment, gpen = the lane's pencil in the INPUT buffer (cell 0, field 0).
+template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
-                                      const bool valid, const unsigned wmask, const float* __restrict__ pflat, float& vmax) {
+                                      const bool valid, const unsigned wmask, const float* __restrict__ pflat, float& vmax,
+                                      const Segment seg = Segment(), const float* __restrict__ gpen = nullptr) {
     const float gam = P.gamma, gp = P.gp, gmg = P.gmg, g_gm1 = P.g_gm1;
     const float dtdx = P.dtdx, hdt = P.hdt;
 
@@ -413,6 +479,16 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             float sgn, v[5];
             int j;
             io.template hydro<S>(n, j, sgn, v);
+            if (SPH && (n < seg.lo || n > seg.hi) && n >= seg.lo - PPM_NGHOST && n <= seg.hi + PPM_NGHOST) {
+                // a ghost cell of this lane's segment: the mirror image along the pencil, from the input buffer
+                j = fold_cell(seg, n, sgn);
+                const float* __restrict__ src = gpen + (long long)(j >> 2) * P.SBd + ((j & 3) << (2 * DIR));
+                v[0] = __ldg(src);
+                v[1] = sgn * __ldg(src + 64 * Dir<DIR>::U);
+                v[2] = __ldg(src + 64 * Dir<DIR>::V);
+                v[3] = __ldg(src + 64 * Dir<DIR>::W);
+                v[4] = __ldg(src + 64 * 4);
+            }
             q[4].A = mk(v[0], v[4]); q[4].B = mk(v[2], v[3]); q[4].u = v[1];
             const Base bs = geo.cell(P, j, sgn);
             fw[4] = bs.rp + q[4].A;
@@ -457,7 +533,8 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         v2 Wr, Wu, Wp, Wv, Ww;
         v2 b0fn;
         {
-            const int fi = (S >= 0) ? n - 2 : image_face(n - 2, P.n, P.bc_lo, P.bc_hi);
+            int fi = (S >= 0) ? n - 2 : image_face(n - 2, P.n, P.bc_lo, P.bc_hi);
+            if (SPH && (n - 2 < seg.lo || n - 2 > seg.hi + 1) && seg.lo <= seg.hi) fi = fold_face(seg, n - 2);
             b0fn = geo.face(P, fi);
         }
         {
@@ -618,6 +695,14 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         if (S >= 0 || n - 3 >= c0 - 1) {
             float m[10];
             io.template ppb<S>(n - 3, m);
+            if (SPH && (n - 3 < seg.lo || n - 3 > seg.hi) && n - 3 >= seg.lo - PPM_NGHOST && n - 3 <= seg.hi + PPM_NGHOST) {
+                float sg;
+                const int j = fold_cell(seg, n - 3, sg);
+                const float* __restrict__ src = gpen + (long long)(j >> 2) * P.SBd + ((j & 3) << (2 * DIR));
+#pragma unroll
+                for (int k = 0; k < 10; ++k) m[k] = __ldg(src + 64 * (5 + PPB_PERM[DIR][k]));
+                m[1] *= sg; m[4] *= sg; m[6] *= sg;            // the coefficients odd in the normal direction
+            }
             // bound B: first-order terms 1/2, pure second-order 1/6, mixed 1/4.
             // local order: a1,b0,c0 are P1 terms; a2,d0,e0 are P2 terms; b1,c1,f0 are mixed P1P1 terms.
             const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
@@ -673,15 +758,16 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             float pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
             const float p0c = fw[0].y - pp_old;
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
-            if (bad && valid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
-            if (CFL) {                                         // C6 on the new state: c from the full rho, p
+            const bool fluid = !SPH || (i >= seg.lo && i <= seg.hi);
+            if (bad && valid && fluid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
+            if (CFL && fluid) {                                         // C6 on the new state: c from the full rho, p
                 const float xs = gam * (p0c + pp_new) * irn;
                 const float cnew = xs * rsqrtf(fmaxf(xs, 1e-37f));
                 vmax = fmaxf(vmax, fmaxf(fabsf(u1), fmaxf(fabsf(vw1.x), fabsf(vw1.y))) + cnew);
             }
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
             ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
-            io.template store<S>(i, ho, mo);
+            io.template store<S>(i, ho, mo, fluid);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
         d2a = mv5(d2b); d2b = MV5B(d2n); Fc = MV5B(Fn); Fcl = MV5B(Fnl); parL = MV5C(pLn); parR = MV5C(pRn);
@@ -848,7 +934,7 @@ struct IoDirect {
 #pragma unroll
         for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
     }
-    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
+    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10], bool = true) {
         float* __restrict__ p = pout + off(i);
         p[0] = h[0];
         p[64 * Dir<DIR>::U] = h[1];
@@ -889,7 +975,7 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     const float* pflat = FLAT ? P.flat + ((long long)ba * P.FBa + (long long)bb * P.FBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)))) : nullptr;
     float vmax = 0.f;
-    march<DIR, GRAV, FLAT, false>(P, io, a, b, c0, c1, true, wmask, pflat, vmax);
+    march<DIR, GRAV, FLAT, false, false>(P, io, a, b, c0, c1, true, wmask, pflat, vmax);
 }
 
 // PPB-only sweep (NEXT-2), direct path
@@ -1128,22 +1214,27 @@ struct IoBulk {
         v[4] = src[64 * 4];
     }
     // finished cell i, written over its own input (already consumed: hydro at n = i, PPB at n = i + 3 < i + 4)
-    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10]) {
+    // (keep = false: a solid cell of the confining sphere — its slot entries stay what they are, the input)
+    template <int S> __device__ __forceinline__ void store(int i, const float (&h)[5], const float (&m)[10], bool keep = true) {
         const int s = (S >= 0 && S < 4) ? S : (i & 3);         // i = n - 4
         float* dh = hyd + hprv + (s << SH);
-        dh[0] = h[0];
-        dh[64 * Dir<DIR>::U] = h[1];
-        dh[64 * Dir<DIR>::V] = h[2];
-        dh[64 * Dir<DIR>::W] = h[3];
-        dh[64 * 4] = h[4];
-        store_ppb<S>(i, m);
+        if (keep) {
+            dh[0] = h[0];
+            dh[64 * Dir<DIR>::U] = h[1];
+            dh[64 * Dir<DIR>::V] = h[2];
+            dh[64 * Dir<DIR>::W] = h[3];
+            dh[64 * 4] = h[4];
+        }
+        store_ppb<S>(i, m, keep);
     }
     // PPB part of cell i only (PPB-only sweep: the hydro slot goes back to global memory as it came in)
-    template <int S> __device__ __forceinline__ void store_ppb(int i, const float (&m)[10]) {
+    template <int S> __device__ __forceinline__ void store_ppb(int i, const float (&m)[10], bool keep = true) {
         const int s = (S >= 0 && S < 4) ? S : (i & 3);
         float* dp = ppr + pst + (s << SH);
+        if (keep) {
 #pragma unroll
-        for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
+            for (int q = 0; q < 10; ++q) dp[64 * PPB_PERM[DIR][q]] = m[q];
+        }
         if (s == 3) {                                          // brick i >> 2 is complete: ship it
             fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
             __syncwarp();
@@ -1192,7 +1283,7 @@ __device__ __forceinline__ void bulk_init_barriers(uint64_t* bars) {
     __syncthreads();
 }
 
-template <int DIR, int GRAV, bool FLAT, bool CFL>
+template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1218,7 +1309,12 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
     const bool valid = a < P.na && b < P.nb;
     float vmax = 0.f;
-    march<DIR, GRAV, FLAT, CFL>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax);
+    if (SPH) {
+        const Segment seg = sphere_segment<DIR>(P, a, b);
+        const float* gpen = P.in + gcol + (long long)(lane >> 4) * P.SBa + (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)));
+        march<DIR, GRAV, FLAT, CFL, true>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax, seg, gpen);
+    } else
+    march<DIR, GRAV, FLAT, CFL, false>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax);
     if (CFL) {
         // warp max by one REDUX on the bit patterns (non-negative floats order like unsigned integers; a NaN has the
         // largest pattern and so survives: ppm_cfl_dt reports it), then one atomicMax per warp
@@ -1297,9 +1393,15 @@ cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_
 }
 template <int DIR, int GRAV, bool FLAT>
 cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ[2][MAX_DEV] = {};
-    if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, true>, occ[1], P, sms, user_chunk, st);
-    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false>, occ[0], P, sms, user_chunk, st);
+    static int occ[4][MAX_DEV] = {};
+    if (P.sphere) {     // confining sphere (NEXT-3): no plane-parallel gravity, no 3-D flattening (ppm_set_sphere checks)
+        if constexpr (GRAV != PPM_GRAV_CONST_Z && !FLAT) {
+            if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, true, true>, occ[3], P, sms, user_chunk, st);
+            return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, false, true>, occ[2], P, sms, user_chunk, st);
+        } else return cudaErrorNotSupported;
+    }
+    if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, true, false>, occ[1], P, sms, user_chunk, st);
+    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
@@ -1378,6 +1480,11 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
     P.tab = c->tab; P.tabp = c->tabp; P.tabg = c->tabg;
     P.flag = c->flag;
+    P.sphere = c->sphere;
+    if (c->sphere) {
+        P.sph_dx = p.dx; P.sph_r2 = c->sph_r * c->sph_r;
+        P.sph_cd = c->sph_c[axis]; P.sph_ca = c->sph_c[ia]; P.sph_cb = c->sph_c[ib];
+    }
     P.cflmax = (fuse_cfl && !advect && ppm_axis_is_bulk(c, axis)) ? c->cflmax : nullptr;
     P.flat = c->flat3d ? c->F3 : nullptr;
     P.FBd = P.SBd / PPM_NFIELDS; P.FBa = P.SBa / PPM_NFIELDS; P.FBb = P.SBb / PPM_NFIELDS;

@@ -579,12 +579,97 @@ def test_hydrostatic_state_is_preserved_exactly_on_gpu():
         g.close()
 
 
+# ---------------------------------------------------------------- NEXT-3: confining sphere, spin-up ---
+def test_sphere_random_flow_matches_oracle_and_solid_cells_are_untouched():
+    """violent random flow inside an off-centre sphere (reading R23): fluid cells against the oracle's sphere
+    mode, solid cells bit for bit what was loaded, mass of the fluid conserved, all six sweep orders"""
+    PPM = _gpu()
+    from oracle import binding as ob
+    rng = np.random.default_rng(41)
+    n = 24
+    f = np.zeros((15, n, n, n), dtype=np.float32)
+    f[0] = 1.0 + 0.3 * rng.random((n, n, n))
+    f[1:4] = 0.3 * rng.normal(size=(3, n, n, n))
+    f[4] = 0.8 + 0.3 * rng.random((n, n, n))
+    f[5] = 0.2 + 0.6 * rng.random((n, n, n))
+    f[6:] = 0.02 * rng.normal(size=(9, n, n, n))
+    for rad, cen in ((0.47, (0.5, 0.52, 0.48)), (0.5, (0.5, 0.5, 0.5)), (0.12, (0.3, 0.6, 0.5))):     # the last: segments of 1..6 cells
+        o = ob.Oracle(n, n, n, 1.0 / n, 1.4, (1,) * 6, None)
+        g = PPM(n, n, n, 1.0 / n, 1.4, (1,) * 6)
+        o.set_sphere(rad, cen)
+        g.set_sphere(rad, cen)
+        o.set_state(f)
+        g.set_state(f)
+        m = o.solid_mask()
+        c0 = g.reduce_conserved()
+        assert abs(c0[0] - o.reduce_conserved()[0]) <= 1e-6 * c0[0]
+        for order in range(6):
+            dt = 0.5 * g.cfl_dt(0.8)
+            assert abs(dt - 0.5 * o.cfl_dt(0.8)) <= DT_TOL * dt
+            g.step(dt, order)
+            o.step(dt, order)
+        gs = g.get_state().cpu().numpy()
+        os_ = o.get_state()
+        assert np.array_equal(gs[:, m], f[:, m])
+        fl = ~m
+        e = max_rel(gs[:, fl].astype(np.float64)[:, None, None, :], os_[:, fl][:, None, None, :])
+        assert max(e.values()) <= MULTI_STEP, (rad, e)
+        c1 = g.reduce_conserved()
+        assert abs(c1[0] - c0[0]) <= 3e-6 * c0[0] and abs(c1[5] - c0[5]) <= 3e-6 * c0[5]
+        g.close()
+
+
+def test_sphere_cfg4_star_in_its_sphere_64_20_steps():
+    """config 4 in the paper's run geometry: the star inside the sphere inscribed in the cube, gravity
+    already tapered to zero before it; 64^3, the config's 20 steps, with the spin-up ramp running during the first ten"""
+    PPM = _gpu()
+    w = W.make(4, n=64)
+    f = w.fields()
+    o = _oracle(w)
+    g = PPM.from_workload(w)
+    o.set_sphere(0.5, (0.5, 0.5, 0.5))
+    g.set_sphere(0.5, (0.5, 0.5, 0.5))
+    o.set_state(f.numpy())
+    g.set_state(f.cuda())
+    m = o.solid_mask()
+    for s in range(20):
+        if s < 10:
+            g.spin_up(0.02)
+            o.spin_up(0.02)
+        dt = g.cfl_dt(w.cfl)
+        assert abs(dt - o.cfl_dt(w.cfl)) <= DT_TOL * dt
+        g.step(dt, 0 if s % 2 == 0 else 5)
+        o.step(dt, 0 if s % 2 == 0 else 5)
+        if s == 0:
+            e1 = max_rel(g.get_state().cpu().numpy().astype(np.float64)[:, ~m][:, None, None, :], o.get_state()[:, ~m][:, None, None, :])
+            assert max(e1.values()) <= ONE_STEP, e1
+    gs = g.get_state().cpu().numpy()
+    os_ = o.get_state()
+    assert np.array_equal(gs[:, m], f.numpy()[:, m])
+    e = max_rel(gs[:, ~m].astype(np.float64)[:, None, None, :], os_[:, ~m][:, None, None, :])
+    assert max(e.values()) <= MULTI_STEP, e
+    assert conserved_rel(g.reduce_conserved(), o.reduce_conserved(), np.where(m, 0.0, os_), w.dx, w.gamma).max() <= CONS
+    x = (np.arange(64) + 0.5) / 64 - 0.5
+    assert np.abs(os_[2][32, 32, :] - 0.2 * x).max() < 0.1 and np.abs(os_[2][32, 32, 40]) > 0.01        # it rotates
+    g.close()
+
+
+def test_sphere_cfg4_full_512_windows_that_straddle_the_sphere():
+    """the headline grid in the sphere geometry, bench launch configuration: windows at a pole of the sphere, on its 45-degree
+    flank, and in the shell, two steps, oracle windows with the same sphere"""
+    c = 256
+    _window_check(4, 2, [((c + 248, c, c), 24), ((c + 178, c + 178, c), 24), ((c + 150, c + 140, c + 150), 24), ((c + 175, c, c), 24)],
+                  sphere=(0.5, (0.5, 0.5, 0.5)))
+
+
 # ---------------------------------------------------------------- full-size configs on windows --------
-def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max"):
+def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sphere=None):
     PPM = _gpu()
     w = W.make(cfg)
     n = w.n
     g = PPM.from_workload(w)
+    if sphere:
+        g.set_sphere(*sphere)
     _load(g, w, nzs=nzs_load)
     dts = []
     for s in range(steps):
@@ -603,6 +688,8 @@ def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max"):
             bc += [w.bc[2 * d] if lo[d] == 0 and (w.bc[2 * d] == 1 or hi[d] == n) else 2,
                    w.bc[2 * d + 1] if hi[d] == n and (w.bc[2 * d + 1] == 1 or lo[d] == 0) else 2]
         o = _oracle(w, n=[hi[d] - lo[d] for d in range(3)], org=lo, bc=bc)
+        if sphere:
+            o.set_sphere(*sphere)
         o.set_state(w.fields(lo, hi, device="cuda").cpu().numpy())
         for s, dt in enumerate(dts):
             o.step(dt, 0 if s % 2 == 0 else 5)
