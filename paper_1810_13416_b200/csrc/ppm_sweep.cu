@@ -1283,6 +1283,49 @@ __device__ __forceinline__ void bulk_init_barriers(uint64_t* bars) {
     __syncthreads();
 }
 
+// Confining sphere: a warp none of whose pencils holds a fluid cell (48 % of the pencils of a cube lie wholly outside its
+// inscribed sphere) only has to pass its brick records on to the other buffer: whole-record bulk copies through two
+// slots of the warp's ring memory, no arithmetic.
+template <int DIR>
+__device__ __forceinline__ unsigned bulk_copy_through(const SweepParams& P, float* wsm, uint64_t* bar, int lane, long long gcol, int ncol, int c0, int c1,
+                                                      unsigned ph) {      // ph: mbarrier phases (bits 0, 1 are used), handed on to the caller
+    constexpr int REC = PPM_BRICK_FLOATS;                      // floats per brick record
+    const int kb = c0 >> 2, ke = c1 >> 2;
+    if (kb >= ke) return ph;
+    if (lane == 0) {
+#pragma unroll 1
+        for (int j = 0; j < 2 && kb + j < ke; ++j) {
+            const float* src = P.in + gcol + (long long)(kb + j) * P.SBd;
+            mbar_expect_tx(bar + j, ncol * REC * 4);
+            bulk_g2s(wsm + j * 2 * REC, src, REC * 4, bar + j);
+            if (ncol > 1) bulk_g2s(wsm + j * 2 * REC + REC, src + P.SBa, REC * 4, bar + j);
+        }
+    }
+#pragma unroll 1
+    for (int k = kb; k < ke; ++k) {
+        const int j = (k - kb) & 1;
+        mbar_wait(bar + j, (ph >> j) & 1);
+        ph ^= 1u << j;
+        if (lane == 0) {
+            float* dst = P.out + gcol + (long long)k * P.SBd;
+            bulk_s2g(dst, wsm + j * 2 * REC, REC * 4);
+            if (ncol > 1) bulk_s2g(dst + P.SBa, wsm + j * 2 * REC + REC, REC * 4);
+            tma_commit();
+            if (k + 2 < ke) {
+                tma_wait_read0();                              // the store just issued has read the slot: refill it
+                const float* src = P.in + gcol + (long long)(k + 2) * P.SBd;
+                mbar_expect_tx(bar + j, ncol * REC * 4);
+                bulk_g2s(wsm + j * 2 * REC, src, REC * 4, bar + j);
+                if (ncol > 1) bulk_g2s(wsm + j * 2 * REC + REC, src + P.SBa, REC * 4, bar + j);
+            }
+        }
+        __syncwarp();
+    }
+    if (lane == 0) tma_wait_all0();
+    __syncwarp();
+    return ph;
+}
+
 template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
@@ -1303,16 +1346,36 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     const int a = (ba0 + (lane >> 4)) * 4 + (lane & 3);
     const int b = bb * 4 + ((lane >> 2) & 3);
     const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
-    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
+    Segment seg;
+    unsigned ph0 = 0;
+    const int c0s = c0, c1s = c1;                                  // this CTA's pencil segment
+    if (SPH) {
+        // The warp marches only the bricks that hold fluid cells of its 32 pencils; the bricks before and after pass through
+        // untouched (the ghost cells beyond a lane's segment are mirror images read per lane, never these bricks).
+        seg = sphere_segment<DIR>(P, a, b);
+        const bool has = a < P.na && b < P.nb && seg.lo <= seg.hi;
+        const int lo_w = __reduce_min_sync(0xffffffffu, has ? seg.lo : 0x7fffffff), hi_w = __reduce_max_sync(0xffffffffu, has ? seg.hi : -1);
+        const int c0w = max(c0, lo_w & ~3), c1w = min(c1, (hi_w + 4) & ~3);
+        float* wsm = sm + warp * G::WARP_FLOATS;
+        uint64_t* wbar = bars + warp * (G::NH + G::NP);
+        if (hi_w < 0 || c0w >= c1w) {                               // nothing but solid cells under this warp in this segment
+            bulk_copy_through<DIR>(P, wsm, wbar, lane, gcol, min(2, nba - ba0), c0, c1, 0u);
+            return;
+        }
+        ph0 = bulk_copy_through<DIR>(P, wsm, wbar, lane, gcol, min(2, nba - ba0), c0, c0w, 0u);
+        c0 = c0w; c1 = c1w;
+    }
+    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), ph0, lane, gcol, min(2, nba - ba0), c0, c1);
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
     const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
     const bool valid = a < P.na && b < P.nb;
     float vmax = 0.f;
     if (SPH) {
-        const Segment seg = sphere_segment<DIR>(P, a, b);
         const float* gpen = P.in + gcol + (long long)(lane >> 4) * P.SBa + (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)));
         march<DIR, GRAV, FLAT, CFL, true>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax, seg, gpen);
+        bulk_copy_through<DIR>(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), lane, gcol, min(2, nba - ba0), c1, c1s, io.ph);
+        (void)c0s;
     } else
     march<DIR, GRAV, FLAT, CFL, false>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax);
     if (CFL) {
