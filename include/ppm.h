@@ -136,6 +136,10 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    only reads 4 bytes back; 0 = ppm_cfl_dt always runs its own reduction pass over the state.  The
  *                    two agree to fp32 rounding of c (bit for bit without a base state).  Whatever else changes the
  *                    state (ppm_set_state, ppm_sweep, a sweep on the direct path) makes ppm_cfl_dt fall back to the pass.
+ *  PPM_OPT_STATE_FORM : 0 (default) = ppm_set_state / ppm_get_state exchange the FULL rho and p; 1 = they exchange the
+ *                    perturbations rho' = rho - rho0, p' = p - p0 exactly as the library stores and evolves them (PAPER.md L35:
+ *                    "perturbations to a base, hydrostatic state"), so that no digit of a small perturbation is lost to the
+ *                    fp32 rounding of rho0 + rho' at the boundary (the parity tests compare the perturbation fields this way).
  *
  * Option that changes the numerical scheme ("a fully 3-D treatment of the
  * shock dissipation"; reading R5b in DESIGN.md):
@@ -145,7 +149,7 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    (ppm_sweep: on the state that sweep starts from) and spread over i-1..i+1 along the sweep.
  *                    Setting it allocates one library-owned device array of ppm_state_floats()/15 floats
  *                    (PPM_ENOMEM if that fails) and adds one light kernel launch per step. */
-enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4 };
+enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4, PPM_OPT_STATE_FORM = 5 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* Confining sphere ("our star is enclosed in an impenetrable and immovable sphere that
  * is inscribed in the cubical domain of our uniform Cartesian grid ... a very simple boundary condition at the sphere";

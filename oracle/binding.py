@@ -48,6 +48,12 @@ def lib():
         L.oracle_cell_is_solid.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.oracle_spin_up.argtypes = [C.c_void_p, C.c_double]
         L.oracle_reduce_conserved.argtypes = [C.c_void_p, dp]
+        L.oracle_set_two_fluid.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double]
+        L.oracle_mix_beta.restype = C.c_double
+        L.oracle_mix_beta.argtypes = [C.c_double] * 3
+        L.oracle_mix_gamma.restype = C.c_double
+        L.oracle_mix_gamma.argtypes = [C.c_double] * 3
+        L.oracle_h7_riemann_2f.argtypes = [dp, dp, C.c_double, C.c_double, C.c_double, C.c_double, dp, dp, dp, dp]
         L.oracle_h1_face.restype = C.c_double
         L.oracle_h1_face.argtypes = [C.c_double] * 4
         L.oracle_h2_limit.argtypes = [C.c_double] * 5 + [dp, dp]
@@ -129,6 +135,23 @@ def h7_riemann(L, R, gamma, rho_floor=1e-30, p_floor=1e-30):
     ps, us = C.c_double(), C.c_double()
     lib().oracle_h7_riemann(_d(L), _d(R), gamma, rho_floor, p_floor, _d(out), C.byref(ps), C.byref(us))
     return out, ps.value, us.value
+
+
+def h7_riemann_2f(L, R, gamL, gamR, rho_floor=1e-30, p_floor=1e-30):
+    """NEXT-4: H7 with one adiabatic index per side.  Returns (sampled[5], gamma of the sampled side, pstar, ustar)."""
+    L, R = _arr(L), _arr(R)
+    out = np.zeros(5)
+    gh, ps, us = C.c_double(), C.c_double(), C.c_double()
+    lib().oracle_h7_riemann_2f(_d(L), _d(R), gamL, gamR, rho_floor, p_floor, _d(out), C.byref(gh), C.byref(ps), C.byref(us))
+    return out, gh.value, ps.value, us.value
+
+
+def mix_beta(f, gamma1, gamma2):
+    return lib().oracle_mix_beta(f, gamma1, gamma2)
+
+
+def mix_gamma(f, gamma1, gamma2):
+    return lib().oracle_mix_gamma(f, gamma1, gamma2)
 
 
 def p2_theta(m10):
@@ -262,6 +285,13 @@ class Oracle:
         rc = lib().oracle_set_sphere(self._h, int(radius > 0), float(radius), cen)
         if rc:
             raise ValueError("oracle_set_sphere rc=%d" % rc)
+
+    def set_two_fluid(self, gamma1, gamma2):
+        """NEXT-4: two-fluid EOS (reading R25): gamma1 = the tracked fluid (FV), gamma2 =
+        the rest.  gamma1 = None switches it off."""
+        rc = lib().oracle_set_two_fluid(self._h, int(gamma1 is not None), float(gamma1 or 0.0), float(gamma2 or 0.0))
+        if rc:
+            raise ValueError("oracle_set_two_fluid rc=%d" % rc)
 
     def solid_mask(self):
         """bool [nz][ny][nx]: cells whose centre lies outside the confining sphere"""

@@ -59,6 +59,8 @@ typedef struct oracle_ctx {
     double *F3;          /* F~ of every cell (flat3d only), evaluated on the state at the start of the call */
     int sphere;          /* NEXT-3: confining sphere */
     double sph_r, sph_c[3]; /* its radius and centre (physical units) */
+    int twofluid;        /* NEXT-4 ("multifluid"): two-fluid equation of state */
+    double gamma1, gamma2; /* adiabatic index of the tracked fluid (volume fraction FV) and of the rest */
 } oracle_ctx;
 
 static double clamp01(double x) { return fmin(1.0, fmax(0.0, x)); }
@@ -453,6 +455,209 @@ void oracle_sweep_pencil(int n, int d, double dx, double dt, double gamma, doubl
     free(buf);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * NEXT-4 ("multifluid", L87 "fv ... gives the fraction of the volume of a cell that
+ * is occupied by a special, tracked multifluid constituent"): two-fluid equation of state.  The paper prints no
+ * EOS, so this is reading R25:
+ *   the tracked fluid (volume fraction f = FV) and the rest are ideal gases with adiabatic indices gamma1 and
+ *   gamma2 in pressure equilibrium inside a cell, so the internal energy per volume is
+ *       e = f p/(gamma1-1) + (1-f) p/(gamma2-1) = p beta(f),   beta(f) = f/(gamma1-1) + (1-f)/(gamma2-1),
+ *   i.e. the cell behaves as an ideal gas with Gamma(f) = 1 + 1/beta(f), and f is the PPB cell mean m000
+ *   clamped to [0,1].  Everything else is the single-fluid scheme with gamma -> Gamma of the cell it belongs to:
+ *   c_i = sqrt(Gamma_i p_i/rho_i) (H0, used by H4 and H6); the Riemann problem at a face takes Gamma of its left
+ *   cell for the left state and of its right cell for the right state (H7: the contact separates them); the
+ *   energy flux carries the enthalpy with Gamma of the upwind side the sampled state lies on (H8); and the new
+ *   pressure is recovered from the conserved energy with beta of the NEW f, i.e. after this sweep's PPB remap
+ *   (H9: p = (E - KE)/beta(f_new)).  Total energy sum(p beta(f) + KE) is conserved to round-off; a contact at
+ *   rest in pressure equilibrium stays exactly so; with gamma1 = gamma2 the scheme is the single-fluid one.
+ *   (Known limit of every conservative gamma-model: a MOVING contact between different gammas picks up a
+ *   pressure ripple of first order in the gamma jump; quantified in tests/test_oracle_twofluid.py.)
+ * ---------------------------------------------------------------------------------------- */
+double oracle_mix_beta(double f, double gamma1, double gamma2) {
+    f = clamp01(f);
+    return f / (gamma1 - 1.0) + (1.0 - f) / (gamma2 - 1.0);
+}
+double oracle_mix_gamma(double f, double gamma1, double gamma2) { return 1.0 + 1.0 / oracle_mix_beta(f, gamma1, gamma2); }
+
+/* H7 with one adiabatic index per side; *gam_out = the index of the side the sampled state lies on */
+void oracle_h7_riemann_2f(const double L[5], const double R[5], double gamL, double gamR, double rho_floor, double p_floor,
+                          double out[5], double *gam_out, double *pstar_out, double *ustar_out) {
+    const double rl = L[0], ul = L[1], pl = L[4], rr = R[0], ur = R[1], pr = R[4];
+    const double CL = sqrt(gamL * pl * rl), CR = sqrt(gamR * pr * rr);
+    const double gpL = 0.5 * (gamL + 1.0), gmL = 0.5 * (gamL - 1.0), gpR = 0.5 * (gamR + 1.0), gmR = 0.5 * (gamR - 1.0);
+    double ps = fmax(p_floor, (CR * pl + CL * pr + CL * CR * (ul - ur)) / (CL + CR));
+    double WL, WR;
+    for (int it = 0; it < 5; ++it) {
+        WL = sqrt(rl * (gpL * ps + gmL * pl));
+        WR = sqrt(rr * (gpR * ps + gmR * pr));
+        double usl = ul - (ps - pl) / WL;
+        double usr = ur + (ps - pr) / WR;
+        double ZL = 2.0 * WL * WL * WL / (WL * WL + CL * CL);
+        double ZR = 2.0 * WR * WR * WR / (WR * WR + CR * CR);
+        ps = fmax(p_floor, ps - ZL * ZR * (usr - usl) / (ZL + ZR));
+    }
+    WL = sqrt(rl * (gpL * ps + gmL * pl));
+    WR = sqrt(rr * (gpR * ps + gmR * pr));
+    const double us = (WL * ul + WR * ur + pl - pr) / (WL + WR);
+    if (pstar_out) *pstar_out = ps;
+    if (ustar_out) *ustar_out = us;
+    double s, rK, uK, pK, WK, gK;
+    const double *K;
+    if (us >= 0.0) { s = 1.0; K = L; rK = rl; uK = ul; pK = pl; WK = WL; gK = gamL; }
+    else           { s = -1.0; K = R; rK = rr; uK = ur; pK = pr; WK = WR; gK = gamR; }
+    double rs = 1.0 / (1.0 / rK - (ps - pK) / (WK * WK));
+    rs = fmax(rs, rho_floor);
+    const double cK = sqrt(gK * pK / rK), cs = sqrt(gK * ps / rs);
+    const double uKh = s * uK, ush = s * us;
+    double lam_head, lam_tail;
+    if (ps > pK) { lam_head = lam_tail = uKh - WK / rK; }
+    else { lam_head = uKh - cK; lam_tail = ush - cs; }
+    double th;
+    if (lam_head >= 0.0) th = 0.0;
+    else if (lam_tail <= 0.0) th = 1.0;
+    else th = -lam_head / (lam_tail - lam_head);
+    out[0] = (1.0 - th) * rK + th * rs;
+    out[1] = (1.0 - th) * uK + th * us;
+    out[4] = (1.0 - th) * pK + th * ps;
+    out[2] = K[2];
+    out[3] = K[3];
+    *gam_out = gK;
+}
+
+/* C4 + C5 for the two-fluid EOS: oracle_sweep_pencil step by step, with Gamma of the cell / side in place of gamma
+ * and the pressure taken from the energy AFTER the PPB remap (same arguments, same array conventions). */
+void oracle_sweep_pencil_2f(int n, int d, double dx, double dt, double gamma1, double gamma2, double rho_floor, double p_floor,
+                            const double *const q[5], const double *const m[10],
+                            const double *rho0c, const double *p0c, const double *gd,
+                            const double *rho0f, const double *p0f,
+                            double *const qn[5], double *const mn[10], const double *ft_ext) {
+    const int nt = n + 2 * NG;
+    const double dtdx = dt / dx;
+    double *buf = (double *)calloc((size_t)nt * 43 + 64, sizeof(double));
+    double *rho = buf, *p = rho + nt, *c = p + nt, *ft = c + nt, *fl = ft + nt;
+    double *qu[5], *ql[5], *qr[5], *WL[5], *WR[5], *F[5];
+    double *cur = fl + nt;
+    for (int k = 0; k < 5; ++k) { qu[k] = cur; cur += nt + 1; }
+    for (int k = 0; k < 5; ++k) { ql[k] = cur; cur += nt; }
+    for (int k = 0; k < 5; ++k) { qr[k] = cur; cur += nt; }
+    for (int k = 0; k < 5; ++k) { WL[k] = cur; cur += nt; }
+    for (int k = 0; k < 5; ++k) { WR[k] = cur; cur += nt; }
+    for (int k = 0; k < 5; ++k) { F[k] = cur; cur += nt + 1; }
+    double *dM = cur; cur += nt + 1;
+    double *theta = cur; cur += nt;
+    double *Gam = cur; cur += nt;          /* Gamma(f_i) of every cell, from the PPB cell mean the sweep starts from */
+    double *E1 = cur; cur += nt;           /* new total energy of the interior cells */
+    double *KE1 = cur; cur += nt;          /* their new kinetic energy */
+
+    /* H0 */
+    for (int j = 0; j < nt; ++j) {
+        Gam[j] = oracle_mix_gamma(m[0][j], gamma1, gamma2);
+        rho[j] = rho0c[j] + q[0][j];
+        p[j] = p0c[j] + q[4][j];
+        c[j] = sqrt(Gam[j] * p[j] / rho[j]);
+    }
+    /* H1 */
+    for (int f = 3; f <= nt - 3; ++f)
+        for (int k = 0; k < 5; ++k) qu[k][f] = oracle_h1_face(q[k][f - 2], q[k][f - 1], q[k][f], q[k][f + 1]);
+    /* H4 */
+    for (int j = 2; j <= nt - 3; ++j) {
+        double p5[5] = {p[j - 2], p[j - 1], p[j], p[j + 1], p[j + 2]};
+        ft[j] = oracle_h4_ftilde(p5, q[1][j - 1], q[1][j + 1], c[j]);
+        if (ft_ext) ft[j] = ft_ext[j];
+    }
+    for (int j = 3; j <= nt - 4; ++j) fl[j] = fmax(ft[j - 1], fmax(ft[j], ft[j + 1]));
+    /* H2, H3, H4 applied */
+    for (int j = 3; j <= nt - 4; ++j)
+        for (int k = 0; k < 5; ++k) {
+            double Lm, Rm;
+            oracle_h2_limit(q[k][j - 1], q[k][j], q[k][j + 1], qu[k][j], qu[k][j + 1], &Lm, &Rm);
+            double q5[5] = {q[k][j - 2], q[k][j - 1], q[k][j], q[k][j + 1], q[k][j + 2]};
+            double om = oracle_h3_omega(oracle_h3_S(q5));
+            double L = (1.0 - om) * qu[k][j] + om * Lm;
+            double R = (1.0 - om) * qu[k][j + 1] + om * Rm;
+            ql[k][j] = fl[j] * q[k][j] + (1.0 - fl[j]) * L;
+            qr[k][j] = fl[j] * q[k][j] + (1.0 - fl[j]) * R;
+        }
+    /* H5, H6 (the cell's own sound speed c_i carries Gamma_i) */
+    for (int j = 3; j <= nt - 4; ++j) {
+        double a[5], b[5], ci[5], wl[5], wr[5], src[3];
+        for (int k = 0; k < 5; ++k) { a[k] = ql[k][j]; b[k] = qr[k][j]; ci[k] = q[k][j]; }
+        src[0] = 0.5 * dt * (-q[1][j] * (rho0f[j + 1] - rho0f[j]) / dx);
+        src[2] = 0.5 * dt * (-q[1][j] * (p0f[j + 1] - p0f[j]) / dx);
+        src[1] = 0.5 * dt * gd[j] * q[0][j] / rho[j];
+        oracle_h6_trace(a, b, ci, rho[j], c[j], dtdx, src, wl, wr);
+        for (int k = 0; k < 5; ++k) { WL[k][j] = wl[k]; WR[k][j] = wr[k]; }
+    }
+    /* H7, H8: face f lies between cells f-1 (Gamma_L) and f (Gamma_R) */
+    for (int f = NG; f <= nt - NG; ++f) {
+        double L[5], R[5], o[5], gh;
+        L[0] = fmax(rho0f[f] + WL[0][f - 1], rho_floor); R[0] = fmax(rho0f[f] + WR[0][f], rho_floor);
+        L[4] = fmax(p0f[f] + WL[4][f - 1], p_floor);     R[4] = fmax(p0f[f] + WR[4][f], p_floor);
+        for (int k = 1; k <= 3; ++k) { L[k] = WL[k][f - 1]; R[k] = WR[k][f]; }
+        oracle_h7_riemann_2f(L, R, Gam[f - 1], Gam[f], rho_floor, p_floor, o, &gh, NULL, NULL);
+        double Fm = o[0] * o[1];
+        double pprime = o[4] - p0f[f];
+        F[0][f] = Fm;
+        F[1][f] = Fm * o[1] + pprime;
+        F[2][f] = Fm * o[2];
+        F[3][f] = Fm * o[3];
+        F[4][f] = o[1] * (gh / (gh - 1.0) * o[4] + 0.5 * o[0] * (o[1] * o[1] + o[2] * o[2] + o[3] * o[3]));
+        dM[f] = dt * Fm;     /* P1 */
+    }
+    /* H9, first part: density, momenta and the conserved energy (E0 with beta of the OLD f) */
+    for (int j = NG; j < nt - NG; ++j) {
+        const int i = j - NG;
+        const double r0 = rho[j], u0 = q[1][j], v0 = q[2][j], w0 = q[3][j];
+        const double E0 = p[j] / (Gam[j] - 1.0) + 0.5 * r0 * (u0 * u0 + v0 * v0 + w0 * w0);
+        double r1 = r0 - dtdx * (F[0][j + 1] - F[0][j]);
+        r1 = fmax(r1, rho_floor);
+        const double rp1 = r1 - rho0c[j];
+        const double mu0 = r0 * u0;
+        const double mu1 = mu0 - dtdx * (F[1][j + 1] - F[1][j]) + dt * 0.5 * (q[0][j] + rp1) * gd[j];
+        const double mv1 = r0 * v0 - dtdx * (F[2][j + 1] - F[2][j]);
+        const double mw1 = r0 * w0 - dtdx * (F[3][j + 1] - F[3][j]);
+        E1[j] = E0 - dtdx * (F[4][j + 1] - F[4][j]) + dt * 0.5 * (mu0 + mu1) * gd[j];
+        const double u1 = mu1 / r1, v1 = mv1 / r1, w1 = mw1 / r1;
+        KE1[j] = 0.5 * r1 * (u1 * u1 + v1 * v1 + w1 * w1);
+        qn[0][i] = rp1; qn[1][i] = u1; qn[2][i] = v1; qn[3][i] = w1;
+    }
+    /* P2 */
+    for (int j = 3; j <= nt - 4; ++j) {
+        double mm[10];
+        for (int k = 0; k < 10; ++k) mm[k] = m[k][j];
+        theta[j] = oracle_p2_theta(mm);
+    }
+    /* P1, P3, P4 */
+    for (int j = NG; j < nt - NG; ++j) {
+        const int i = j - NG;
+        double M[3] = {rho[j - 1] * dx, rho[j] * dx, rho[j + 1] * dx};
+        for (int f = 0; f < 6; ++f) {
+            const int deg = PPB_FAM[d][f][0];
+            double a[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}}, out[3];
+            for (int s = 0; s < 3; ++s)
+                for (int nn = 0; nn <= deg; ++nn) {
+                    int idx = PPB_FAM[d][f][1 + nn];
+                    double v = m[idx][j - 1 + s];
+                    if (idx != 0) v *= theta[j - 1 + s];
+                    a[s][nn] = v;
+                }
+            int ok = oracle_p4_remap(deg, a, M, dM[j], dM[j + 1], out);
+            for (int nn = 0; nn <= deg; ++nn) {
+                int idx = PPB_FAM[d][f][1 + nn];
+                mn[idx][i] = ok ? out[nn] : m[idx][j];
+            }
+        }
+    }
+    /* H9, second part: the pressure from the conserved energy with beta of the NEW f (the cell mean just remapped) */
+    for (int j = NG; j < nt - NG; ++j) {
+        const int i = j - NG;
+        const double beta1 = oracle_mix_beta(mn[0][i], gamma1, gamma2);
+        const double p1 = fmax(p_floor, (E1[j] - KE1[j]) / beta1);
+        qn[4][i] = p1 - p0c[j];
+    }
+    free(buf);
+}
+
 /* NEXT-2 (Fig. 3: "a velocity field is applied ... this is linear advection").
  * PPB-only sweep of one pencil: the hydro state is held fixed and FV is advected by the stored velocity field.
  * [reading R22, DESIGN.md]  The gas is taken as uniform (rho = 1: M_i = dx), the velocity at face i+1/2 is the mean
@@ -571,6 +776,20 @@ int oracle_get_state(const oracle_ctx *c, double *const fields[NF]) {
 /* raw perturbation-form access (for tests) */
 double *oracle_raw_field(oracle_ctx *c, int f) { return c->q[f]; }
 
+/* adiabatic index of a cell: gamma, or Gamma(f) of the two-fluid EOS (NEXT-4, reading R25) with f = its PPB cell mean */
+static double cell_gamma(const oracle_ctx *c, size_t id) {
+    return c->twofluid ? oracle_mix_gamma(c->q[5][id], c->gamma1, c->gamma2) : c->gamma;
+}
+
+/* NEXT-4: switch the two-fluid EOS on (gamma1: the tracked fluid, gamma2: the rest; both > 1) or off */
+int oracle_set_two_fluid(oracle_ctx *c, int on, double gamma1, double gamma2) {
+    if (!c) return 1;
+    if (!on) { c->twofluid = 0; return 0; }
+    if (!(gamma1 > 1.0) || !(gamma2 > 1.0) || c->sphere) return 1;     /* (not combined with the confining sphere) */
+    c->twofluid = 1; c->gamma1 = gamma1; c->gamma2 = gamma2;
+    return 0;
+}
+
 static int sweep_impl_sphere(oracle_ctx *c, int d, double dt);   /* NEXT-3, below */
 static int cell_is_solid(const oracle_ctx *c, int gi, int gj, int gk);
 
@@ -622,6 +841,11 @@ static int sweep_impl(oracle_ctx *c, int d, double dt) {
                 X[d1] = (gidx[d1] + 0.5) * c->dx; X[d2] = (gidx[d2] + 0.5) * c->dx; X[d] = gf * c->dx;
                 base_at(c, X, &r0f[f], &p0f[f], gv);
             }
+            if (c->twofluid)
+                oracle_sweep_pencil_2f(n, d, c->dx, dt, c->gamma1, c->gamma2, c->rho_floor, c->p_floor,
+                                       (const double *const *)qa, (const double *const *)ma, r0c, p0c, gd, r0f, p0f, qo, mo,
+                                       (c->flat3d && c->F3) ? f3 : NULL);
+            else
             oracle_sweep_pencil(n, d, c->dx, dt, c->gamma, c->rho_floor, c->p_floor,
                                 (const double *const *)qa, (const double *const *)ma, r0c, p0c, gd, r0f, p0f, qo, mo,
                                 (c->flat3d && c->F3) ? f3 : NULL);
@@ -675,7 +899,7 @@ int oracle_flatten3d_update(oracle_ctx *c) {
                         cell_base(c, g[0], g[1], g[2], &r0, &p0, gv);
                         p5[o + 2] = p0 + c->q[4][id];
                         if (o >= -1 && o <= 1) u3[o + 1] = sgn * c->q[1 + d][id];
-                        if (o == 0) ci = sqrt(c->gamma * p5[2] / (r0 + c->q[0][id]));
+                        if (o == 0) ci = sqrt(cell_gamma(c, id) * p5[2] / (r0 + c->q[0][id]));
                     }
                     F = fmax(F, oracle_h4_ftilde(p5, u3[0], u3[2], ci));
                 }
@@ -770,7 +994,7 @@ int oracle_advect(oracle_ctx *c, double dt, int sweep_order) {
 int oracle_set_sphere(oracle_ctx *c, int on, double radius, const double center[3]) {
     if (!c) return 1;
     if (on) {
-        if (!(radius > 0.0) || !center) return 1;
+        if (!(radius > 0.0) || !center || c->twofluid) return 1;
         for (int d = 0; d < 3; ++d)
             if (c->bc[2 * d] == OR_BC_PERIODIC) return 1;     /* a wall all round: periodic faces make no sense here */
         c->sph_r = radius;
@@ -929,7 +1153,7 @@ int oracle_cfl_dt(const oracle_ctx *c, double cfl, double *dt_out) {
                 if (cell_is_solid(c, c->org[0] + i, c->org[1] + j, c->org[2] + k)) continue;     /* NEXT-3: fluid cells only */
                 cell_base(c, c->org[0] + i, c->org[1] + j, c->org[2] + k, &r0, &p0, gv);
                 double rho = r0 + c->q[0][id], p = p0 + c->q[4][id];
-                double cs = sqrt(c->gamma * p / rho);
+                double cs = sqrt(cell_gamma(c, id) * p / rho);
                 for (int d = 0; d < 3; ++d) vmax = fmax(vmax, fabs(c->q[1 + d][id]) + cs);
             }
     *dt_out = cfl * c->dx / vmax;
@@ -949,7 +1173,7 @@ int oracle_reduce_conserved(const oracle_ctx *c, double out[6]) {
                 double rho = r0 + c->q[0][id], p = p0 + c->q[4][id];
                 double u = c->q[1][id], v = c->q[2][id], w = c->q[3][id];
                 acc[0] += rho; acc[1] += rho * u; acc[2] += rho * v; acc[3] += rho * w;
-                acc[4] += p / (c->gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w);
+                acc[4] += p / (cell_gamma(c, id) - 1.0) + 0.5 * rho * (u * u + v * v + w * w);
                 acc[5] += rho * c->q[5][id];
             }
     double dv = c->dx * c->dx * c->dx;

@@ -24,7 +24,7 @@ EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_swee
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
            "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_destroy",
            "ppm_last_error")
-OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED = 2, 3, 4
+OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED, OPT_STATE_FORM = 2, 3, 4, 5
 
 
 class ppm_gravity(C.Structure):

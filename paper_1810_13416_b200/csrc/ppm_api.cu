@@ -279,6 +279,7 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
         set_err(c, "ppm_set_option: not together with the confining sphere"); return PPM_EINVAL;
     }
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
+    if (option == PPM_OPT_STATE_FORM && (value == 0 || value == 1)) { c->pert_io = value; return PPM_OK; }
     if (option == PPM_OPT_CFL_FUSED && (value == 0 || value == 1)) { c->cfl_fused = value; c->cfl_valid = 0; return PPM_OK; }
     if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
         if (value && !c->F3) {

@@ -16,6 +16,7 @@ struct AuxParams {
     const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
     float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
     int sphere;                         // NEXT-3: confining sphere on
+    int pert_io;                        // PPM_OPT_STATE_FORM = 1: the boundary arrays carry rho', p' as stored (no base state added / removed)
     double sph_r2, sph_cx, sph_cy, sph_cz;
 };
 
@@ -78,8 +79,8 @@ __global__ void __launch_bounds__(256) to_perturbation_kernel(AuxParams A, const
 #pragma unroll
         for (int f = 0; f < PPM_NFIELDS; ++f) {
             float v = src[f * tot + t];
-            if (f == 0) v = (float)((double)v - r0);
-            if (f == 4) v = (float)((double)v - p0);
+            if (f == 0 && !A.pert_io) v = (float)((double)v - r0);
+            if (f == 4 && !A.pert_io) v = (float)((double)v - p0);
             st[id + 64 * f] = v;
         }
     }
@@ -98,8 +99,8 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
 #pragma unroll
         for (int f = 0; f < PPM_NFIELDS; ++f) {
             float v = st[id + 64 * f];
-            if (f == 0) v = (float)((double)v + r0);
-            if (f == 4) v = (float)((double)v + p0);
+            if (f == 0 && !A.pert_io) v = (float)((double)v + r0);
+            if (f == 4 && !A.pert_io) v = (float)((double)v + p0);
             dst[f * tot + t] = v;
         }
     }
@@ -373,6 +374,7 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.tab32 = c->tab;
     A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
     A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
+    A.pert_io = c->pert_io;
     A.sphere = c->sphere; A.sph_r2 = c->sph_r * c->sph_r; A.sph_cx = c->sph_c[0]; A.sph_cy = c->sph_c[1]; A.sph_cz = c->sph_c[2];
     return A;
 }

@@ -76,6 +76,7 @@ struct ppm_ctx {
     int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state
     int cfl_valid;                  // cflmax holds the maximum of the CURRENT state (set by a fused step, cleared by anything else that changes the state)
     int io_path;                    // PPM_OPT_IO_PATH: 0 = bulk-staged where the sweep-axis extent is whole bricks, 1 = direct everywhere
+    int pert_io;                    // PPM_OPT_STATE_FORM: 1 = ppm_set_state / ppm_get_state exchange rho', p' (perturbation form, as stored)
     long long launches;
     char err[512];
 };

@@ -800,7 +800,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 #pragma unroll 1
                 for (int n = c0 + 4; n < c1; n += 2) {
                     body(n, integral_constant<int, 4>());
-                    body(n + 1, integral_constant<int, 4>());
+                    body(n + 1, integral_constant<int, 5>());       // (a second type, so that the body is inlined twice)
                 }
 #else
 #pragma unroll 1
@@ -1195,7 +1195,7 @@ struct IoBulk {
         v[4] = src[64 * 4];
     }
     template <int S> __device__ __forceinline__ void ppb(int c, float (&m)[10]) {
-        const int s = (S >= 0 && S < 4) ? ((S + 1) & 3) : ((S == 4) ? (c & 3) : ((c & 3) ^ prev));      // c = n - 3
+        const int s = (S >= 0 && S < 4) ? ((S + 1) & 3) : ((S >= 4) ? (c & 3) : ((c & 3) ^ prev));      // c = n - 3
         const float* src = ppr + pcur + (s << SH);
 #pragma unroll
         for (int q = 0; q < 10; ++q) m[q] = src[64 * PPB_PERM[DIR][q]];

@@ -1,6 +1,8 @@
 """Textbook EXACT Riemann solver for the ideal-gas Euler equations (iterative, Toro ch. 4), written
 separately for the tests: it pins the oracle's two-shock solver and the
-shock-tube convergence test.  Shares nothing with oracle/ or the CUDA path."""
+shock-tube convergence test.  Shares nothing with oracle/ or the CUDA path.
+Every function takes an optional `gr`: the adiabatic index of the gas RIGHT of the contact (two-fluid shock tube, NEXT-4;
+the contact separates the two gases, so each side's wave uses its own index); default: the same gas on both sides."""
 import math
 
 import numpy as np
@@ -16,24 +18,27 @@ def _f(p, rk, pk, g):
             1.0 / (rk * ck) * (p / pk) ** (-(g + 1.0) / (2.0 * g)))
 
 
-def star(rl, ul, pl, rr, ur, pr, g):
+def star(rl, ul, pl, rr, ur, pr, g, gr=None):
+    gr = g if gr is None else gr
     p = max(1e-12, 0.5 * (pl + pr))
     for _ in range(200):
         fl, dfl = _f(p, rl, pl, g)
-        fr, dfr = _f(p, rr, pr, g)
+        fr, dfr = _f(p, rr, pr, gr)
         pn = max(1e-14, p - (fl + fr + ur - ul) / (dfl + dfr))
         if abs(pn - p) <= 1e-15 * (pn + p):
             p = pn
             break
         p = pn
     fl, _ = _f(p, rl, pl, g)
-    fr, _ = _f(p, rr, pr, g)
+    fr, _ = _f(p, rr, pr, gr)
     return p, 0.5 * (ul + ur) + 0.5 * (fr - fl)
 
 
-def sample(rl, ul, pl, rr, ur, pr, g, xi):
+def sample(rl, ul, pl, rr, ur, pr, g, xi, gr=None):
     """(rho, u, p) of the exact solution at x/t = xi."""
-    ps, us = star(rl, ul, pl, rr, ur, pr, g)
+    ps, us = star(rl, ul, pl, rr, ur, pr, g, gr)
+    if xi > us and gr is not None:
+        g = gr                      # right of the contact: the other gas
     gm = (g - 1.0) / (g + 1.0)
     if xi <= us:
         cl = math.sqrt(g * pl / rl)
@@ -68,5 +73,5 @@ def sample(rl, ul, pl, rr, ur, pr, g, xi):
     return rr * (c / cr) ** (2.0 / (g - 1.0)), 2.0 / (g + 1.0) * (-cr + 0.5 * (g - 1.0) * ur + xi), pr * (c / cr) ** (2.0 * g / (g - 1.0))
 
 
-def profile(rl, ul, pl, rr, ur, pr, g, x, x0, t):
-    return np.array([sample(rl, ul, pl, rr, ur, pr, g, (xx - x0) / t) for xx in x])
+def profile(rl, ul, pl, rr, ur, pr, g, x, x0, t, gr=None):
+    return np.array([sample(rl, ul, pl, rr, ur, pr, g, (xx - x0) / t, gr) for xx in x])

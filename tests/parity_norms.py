@@ -32,6 +32,20 @@ def max_rel(g, o, scale=None):
     return {"rho": e[0], "u": e[1:4].max(), "p": e[4], "FV": e[5:].max()}
 
 
+def pert_rel(gp, op):
+    """The perturbation fields themselves: gp, op = (rho', p') as the GPU stores them
+    (ppm_get_state with PPM_OPT_STATE_FORM = 1) and as the oracle stores them (oracle_raw_field 0, 4).
+    max |gpu - oracle| / max |oracle| per field — in the low-Mach configs rho', p' are 1e-3 .. 1e-6 of the base state, so
+    this norm is that much stricter than the full-value norm of R20; a field the oracle leaves at round-off level
+    (max |q'| below 1e-12 of the base scale `floor`) has no scale and reports 0."""
+    out = {}
+    for name, g, o in (("rho'", gp[0], op[0]), ("p'", gp[1], op[1])):
+        sc = np.abs(o).max()
+        out[name] = float(np.abs(g - o).max() / sc) if sc > 0 else 0.0
+        out[name + " scale"] = float(sc)
+    return out
+
+
 def abs_err(g, o):
     return np.array([np.abs(g[f] - o[f]).max() for f in range(15)])
 

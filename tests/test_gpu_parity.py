@@ -14,11 +14,16 @@ import torch
 
 from paper_1810_13416_b200 import workloads as W
 
-from parity_norms import conserved_rel, l1_rel, max_rel, merge_scales
+from parity_norms import conserved_rel, l1_rel, max_rel, merge_scales, pert_rel
 
 pytestmark = pytest.mark.gpu
 
 ONE_STEP, MULTI_STEP, L1_SHOCK, CONS, DT_TOL = 1e-5, 1e-4, 1e-4, 1e-6, 1e-6
+# The perturbation fields rho' = rho - rho0, p' = p - p0 compared directly (ppm_get_state in perturbation form against the
+# oracle's stored perturbations), relative to max |rho'|, max |p'|: the bar for the low-Mach gravity configs, where the
+# full-value norm above would let rho', p' be wrong by their own size.  fp32 carries 6e-8 of the FULL rho, p
+# through every flux difference, i.e. 6e-8 / (max|q'| / q0) of the perturbation per operation; DESIGN.md section 2 (R20b).
+PERT_TOL = 1e-4       # measured on a B200: <= 5.1e-6 on every config (profiles/r2_parity_perturbation.md)
 
 
 def _gpu():
@@ -70,6 +75,13 @@ def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False):
             os_ = o.get_state()
             out[s + 1] = (max_rel(gs, os_), l1_rel(gs, os_))
     out["cons1"] = conserved_rel(g.reduce_conserved(), o.reduce_conserved(), o.get_state(), w.dx, w.gamma)
+    # the perturbation fields as stored on both sides (no base state added, no rounding of rho0 + rho')
+    from paper_1810_13416_b200.binding import OPT_STATE_FORM
+    g.set_option(OPT_STATE_FORM, 1)
+    gp = g.get_state().cpu().numpy().astype(np.float64)
+    g.set_option(OPT_STATE_FORM, 0)
+    out["pert"] = pert_rel((gp[0], gp[4]), (o.raw_field(0), o.raw_field(4)))
+    print("perturbation-form parity after %d steps (%s %d^3): %s" % (steps, w.name, w.n, {k: float("%.3g" % v) for k, v in out["pert"].items()}))
     out["drift_gpu"] = np.abs(g.reduce_conserved() - c0g)
     out["c0"] = c0g
     out["final"] = (gs, os_)
@@ -174,6 +186,7 @@ def test_cfg2_stratified_reduced_64_100_steps():
     assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
     assert max(r[100][0].values()) <= MULTI_STEP, r[100][0]
     assert r["cons1"].max() <= CONS
+    assert r["pert"]["rho'"] <= PERT_TOL and r["pert"]["p'"] <= PERT_TOL, r["pert"]
 
 
 def test_cfg3_blast_reduced_64_50_steps_L1():
@@ -368,6 +381,7 @@ def test_cfg4_convection_reduced_64_20_steps():
     assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
     assert max(r[20][0].values()) <= MULTI_STEP, r[20][0]
     assert r["cons1"].max() <= CONS
+    assert r["pert"]["rho'"] <= PERT_TOL and r["pert"]["p'"] <= PERT_TOL, r["pert"]
 
 
 @pytest.mark.parametrize("dims", [(37, 29, 23), (36, 30, 22)])
@@ -679,7 +693,7 @@ def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sp
     g.sync()
     apron = 4 * steps
     worst = {}
-    pairs = []
+    pairs, perts = [], []
     for (c, size) in windows:
         lo = [max(0, c[d] - size // 2 - apron) for d in range(3)]
         hi = [min(n, c[d] + size // 2 + apron) for d in range(3)]
@@ -701,6 +715,14 @@ def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sp
         gs = gs[:, :, lo[1] + sl[1].start:lo[1] + sl[1].stop, lo[0] + sl[0].start:lo[0] + sl[0].stop]
         os_ = os_[:, sl[2], sl[1], sl[0]]
         pairs.append((gs, os_))
+        if w.grav is not None and norm == "max":
+            # the perturbation fields as both sides store them (PERT_TOL above)
+            from paper_1810_13416_b200.binding import OPT_STATE_FORM
+            g.set_option(OPT_STATE_FORM, 1)
+            gp = g.get_state(z0=zs.start, nzs=zs.stop - zs.start).cpu().numpy().astype(np.float64)
+            g.set_option(OPT_STATE_FORM, 0)
+            gp = gp[:, :, lo[1] + sl[1].start:lo[1] + sl[1].stop, lo[0] + sl[0].start:lo[0] + sl[0].stop]
+            perts.append(((gp[0], gp[4]), (o.raw_field(0)[sl[2], sl[1], sl[0]].copy(), o.raw_field(4)[sl[2], sl[1], sl[0]].copy())))
     g.close()
     scale = merge_scales([o_ for _, o_ in pairs])      # a window in a quiescent region has no scale of its own
     for gs, os_ in pairs:
@@ -708,6 +730,13 @@ def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sp
         for k, v in e.items():
             worst[k] = max(worst.get(k, 0.0), v)
     assert max(worst.values()) <= tol, worst
+    if perts:
+        # scale = the largest perturbation over all windows (a window in the quiescent core has none of its own)
+        sc = [max(np.abs(op[k]).max() for _, op in perts) for k in (0, 1)]
+        pe = [max(np.abs(gp[k] - op[k]).max() for gp, op in perts) / sc[k] if sc[k] > 0 else 0.0 for k in (0, 1)]
+        print("perturbation-form parity, cfg %d windows after %d steps: rho' %.3g (scale %.3g), p' %.3g (scale %.3g)" % (cfg, steps, pe[0], sc[0], pe[1], sc[1]))
+        assert max(pe) <= PERT_TOL, (pe, sc)
+        worst["rho'"], worst["p'"] = pe
     return worst
 
 
