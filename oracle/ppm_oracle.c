@@ -466,12 +466,17 @@ void oracle_sweep_pencil(int n, int d, double dx, double dt, double gamma, doubl
  *   clamped to [0,1].  Everything else is the single-fluid scheme with gamma -> Gamma of the cell it belongs to:
  *   c_i = sqrt(Gamma_i p_i/rho_i) (H0, used by H4 and H6); the Riemann problem at a face takes Gamma of its left
  *   cell for the left state and of its right cell for the right state (H7: the contact separates them); the
- *   energy flux carries the enthalpy with Gamma of the upwind side the sampled state lies on (H8); and the new
- *   pressure is recovered from the conserved energy with beta of the NEW f, i.e. after this sweep's PPB remap
- *   (H9: p = (E - KE)/beta(f_new)).  Total energy sum(p beta(f) + KE) is conserved to round-off; a contact at
- *   rest in pressure equilibrium stays exactly so; with gamma1 = gamma2 the scheme is the single-fluid one.
- *   (Known limit of every conservative gamma-model: a MOVING contact between different gammas picks up a
- *   pressure ripple of first order in the gamma jump; quantified in tests/test_oracle_twofluid.py.)
+ *   energy flux carries the enthalpy (beta~ + 1) p^ of the gas that actually crosses the face: beta~ = beta(f~), f~ =
+ *   the mean FV of the slab of mass dM that the PPB remap donates through that face (H8) — so the energy flux and
+ *   the FV flux move the same gas; and the new pressure is recovered from the conserved energy with beta of the NEW
+ *   f, i.e. after this sweep's PPB remap (H9: p = (E - KE)/beta(f_new)).  Total energy sum(p beta(f) + KE) is
+ *   conserved to round-off; a contact at rest in pressure equilibrium stays exactly so; a contact carried by a
+ *   uniform flow of uniform density keeps its pressure to round-off (with the upwind CELL-MEAN Gamma in the
+ *   enthalpy instead, a two-gas shock tube grows an O(1) density spike at the contact and does not converge: tried,
+ *   measured, rejected); with gamma1 = gamma2 the scheme is the single-fluid one.
+ *   (Remaining limit: FV is remapped in the MASS coordinate (R11), beta is a VOLUME average; across a contact that is
+ *   also a density jump the two differ and a moving contact keeps a small pressure ripple, quantified in
+ *   tests/test_oracle_twofluid.py.)
  * ---------------------------------------------------------------------------------------- */
 double oracle_mix_beta(double f, double gamma1, double gamma2) {
     f = clamp01(f);
@@ -588,6 +593,12 @@ void oracle_sweep_pencil_2f(int n, int d, double dx, double dt, double gamma1, d
         oracle_h6_trace(a, b, ci, rho[j], c[j], dtdx, src, wl, wr);
         for (int k = 0; k < 5; ++k) { WL[k][j] = wl[k]; WR[k][j] = wr[k]; }
     }
+    /* P2 (ahead of H8, which needs the pre-limited polynomial of the donor cell) */
+    for (int j = 3; j <= nt - 4; ++j) {
+        double mm[10];
+        for (int k = 0; k < 10; ++k) mm[k] = m[k][j];
+        theta[j] = oracle_p2_theta(mm);
+    }
     /* H7, H8: face f lies between cells f-1 (Gamma_L) and f (Gamma_R) */
     for (int f = NG; f <= nt - NG; ++f) {
         double L[5], R[5], o[5], gh;
@@ -595,14 +606,28 @@ void oracle_sweep_pencil_2f(int n, int d, double dx, double dt, double gamma1, d
         L[4] = fmax(p0f[f] + WL[4][f - 1], p_floor);     R[4] = fmax(p0f[f] + WR[4][f], p_floor);
         for (int k = 1; k <= 3; ++k) { L[k] = WL[k][f - 1]; R[k] = WR[k][f]; }
         oracle_h7_riemann_2f(L, R, Gam[f - 1], Gam[f], rho_floor, p_floor, o, &gh, NULL, NULL);
+        (void)gh;            /* (Gamma of the sampled side: the sound speeds inside the solver have used it) */
         double Fm = o[0] * o[1];
         double pprime = o[4] - p0f[f];
         F[0][f] = Fm;
         F[1][f] = Fm * o[1] + pprime;
         F[2][f] = Fm * o[2];
         F[3][f] = Fm * o[3];
-        F[4][f] = o[1] * (gh / (gh - 1.0) * o[4] + 0.5 * o[0] * (o[1] * o[1] + o[2] * o[2] + o[3] * o[3]));
         dM[f] = dt * Fm;     /* P1 */
+        /* the enthalpy that crosses the face belongs to the gas that crosses it: beta of the mean FV of the slab of mass
+         * dM that the PPB remap takes out of the donor cell (its pre-limited polynomial along the sweep, P2/P4; the
+         * transverse families average to zero over the slab).  With this the internal-energy flux p^ u^ beta~ and the
+         * FV flux of the remap move the SAME gas, and a contact carried by a uniform flow of uniform density keeps
+         * its pressure exactly. */
+        {
+            const int jd = (dM[f] >= 0.0) ? f - 1 : f;                       /* donor cell */
+            const double sig = fmin(fabs(dM[f]) / (rho[jd] * dx), 1.0);      /* donated fraction of its mass */
+            const double sm = (dM[f] >= 0.0) ? 0.5 - 0.5 * sig : -0.5 + 0.5 * sig;   /* slab midpoint in the cell's mass coordinate */
+            const int i1 = PPB_FAM[d][0][2], i2 = PPB_FAM[d][0][3];
+            const double fs = m[0][jd] + theta[jd] * (m[i1][jd] * sm + m[i2][jd] * (sm * sm + sig * sig / 12.0 - 1.0 / 12.0));
+            const double bh = oracle_mix_beta(fs, gamma1, gamma2);
+            F[4][f] = o[1] * ((bh + 1.0) * o[4] + 0.5 * o[0] * (o[1] * o[1] + o[2] * o[2] + o[3] * o[3]));
+        }
     }
     /* H9, first part: density, momenta and the conserved energy (E0 with beta of the OLD f) */
     for (int j = NG; j < nt - NG; ++j) {
@@ -620,12 +645,6 @@ void oracle_sweep_pencil_2f(int n, int d, double dx, double dt, double gamma1, d
         const double u1 = mu1 / r1, v1 = mv1 / r1, w1 = mw1 / r1;
         KE1[j] = 0.5 * r1 * (u1 * u1 + v1 * v1 + w1 * w1);
         qn[0][i] = rp1; qn[1][i] = u1; qn[2][i] = v1; qn[3][i] = w1;
-    }
-    /* P2 */
-    for (int j = 3; j <= nt - 4; ++j) {
-        double mm[10];
-        for (int k = 0; k < 10; ++k) mm[k] = m[k][j];
-        theta[j] = oracle_p2_theta(mm);
     }
     /* P1, P3, P4 */
     for (int j = NG; j < nt - NG; ++j) {
