@@ -219,6 +219,8 @@ def _bench_grid(args, cfg, dev, lr, ws, barrier, K, reps, with_e2e):
         g.set_option(OPT_FLATTEN3D, 1)
     if args.sphere:
         g.set_sphere(0.5, (0.5, 0.5, 0.5))
+    if args.two_fluid:
+        g.set_two_fluid(1.4, w.gamma)        # the stable layer (FV = 1) is a gamma = 1.4 gas, the convection zone keeps 5/3
     _load_state(g, w, 8 if n >= 1024 else 32)
     dt = 0.7 * g.cfl_dt(w.cfl)       # fixed for the run: no host sync inside the timed region
     do_step = g.advect if args.advect else g.step
@@ -321,7 +323,7 @@ def run_gpu(args):
     r = _bench_grid(args, args.workload, dev, lr, ws, barrier, K, reps, not args.no_e2e)
     # second target grid in the same run: config 5 (1024^3, its 5 steps x 3 repetitions) when the headline is config 4
     also = None
-    want_also = (args.workload == 4 and not args.no_also and not args.advect and not args.direct
+    want_also = (args.workload == 4 and not args.no_also and not args.advect and not args.direct and not args.two_fluid
                  and torch.cuda.get_device_properties(dev).total_memory > 150e9)
     if want_also:
         try:
@@ -358,6 +360,7 @@ def run_gpu(args):
                    "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (15 * ncell * 4 / 1e9),
                    "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk,
                    "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)",
+                   "eos": "two-fluid: gamma 1.4 (tracked, FV) / 5/3 (ppm_set_two_fluid; reading R25)" if args.two_fluid else "one ideal gas",
                    "geometry": "star inside the confining sphere inscribed in the cube (ppm_set_sphere; PAPER.md L69): cell-updates count ALL cells of the cube, 52 % of which are fluid" if args.sphere else "reflecting cube",
                    "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step, CFL max-reduction fused into the last sweep)",
                    "timing": "median of %d repetitions of the %d-step region (CUDA events on the library's stream)" % (len(r["ms_reps"]), K)},
@@ -410,6 +413,7 @@ def main():
     ap.add_argument("--advect", action="store_true", help="time PPB-only steps (ppm_advect, SURVEY 8(f) NEXT-2) instead of full PPM+PPB steps")
     ap.add_argument("--flatten3d", action="store_true", help="fully 3-D shock-flattening mode (SURVEY 8(f) NEXT-1): one more light kernel per step")
     ap.add_argument("--sphere", action="store_true", help="the paper's run geometry (SURVEY 8(f) NEXT-3): confining sphere inscribed in the cube")
+    ap.add_argument("--two-fluid", action="store_true", help="two-fluid equation of state (SURVEY 8(f) NEXT-4): the tracked fluid has gamma = 1.4")
     ap.add_argument("--direct", action="store_true", help="direct global-memory sweep path instead of the bulk-staged one")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window (--impl reference)")

@@ -162,6 +162,17 @@ int ppm_set_option(ppm_ctx *ctx, int option, int value);
  * neither PPM_OPT_FLATTEN3D nor PPM_OPT_IO_PATH = 1 is set.  Host-side state only (no launch). */
 int ppm_set_sphere(ppm_ctx *ctx, double radius, const double center[3]);
 
+/* Two-fluid equation of state ("multifluid", L87 "fv ... gives the fraction of the volume of a
+ * cell that is occupied by a special, tracked multifluid constituent"; the paper prints no EOS: reading R25 in DESIGN.md).  The
+ * tracked fluid (volume fraction f = FV, the PPB cell mean m000 clamped to [0,1]) has adiabatic index gamma_tracked, the rest
+ * gamma_rest; both are ideal gases in pressure equilibrium inside a cell, so the internal energy per volume is e = p beta(f) with
+ * beta(f) = f/(gamma_tracked-1) + (1-f)/(gamma_rest-1), i.e. the cell is an ideal gas with Gamma(f) = 1 + 1/beta(f).  Each side of
+ * a face takes Gamma of its own cell, the enthalpy flux carries beta of the gas the PPB remap moves through the face, and the new
+ * pressure is recovered from the conserved energy with beta of the new f; ppm_cfl_dt and the energy of ppm_reduce_conserved use
+ * Gamma(f) too.  gamma of ppm_params is not used while the mode is on.  gamma_tracked <= 0 switches it off.
+ * PPM_EINVAL unless both indices are finite and > 1; not together with ppm_set_sphere or PPM_OPT_FLATTEN3D.  Host-side state only. */
+int ppm_set_two_fluid(ppm_ctx *ctx, double gamma_tracked, double gamma_rest);
+
 /* One increment of the rotation spin-up ("We treat the rotation by adding a solid body rotational flow
  * component to our simulation gradually over the first several thousand time steps"; reading R24): every fluid cell gets
  * du = domega e_z x (X - centre), i.e. du_x = -domega (Y - cy), du_y = +domega (X - cx), about the sphere's centre (the

@@ -22,7 +22,7 @@ GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
-           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_destroy",
+           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_set_two_fluid", "ppm_destroy",
            "ppm_last_error")
 OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED, OPT_STATE_FORM = 2, 3, 4, 5
 
@@ -71,6 +71,7 @@ def lib():
         L.ppm_measure_fp32_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.ppm_set_sphere.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.ppm_spin_up.argtypes = [C.c_void_p, C.c_double]
+        L.ppm_set_two_fluid.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.ppm_destroy.argtypes = [C.c_void_p]
         L.ppm_destroy.restype = None
         L.ppm_last_error.argtypes = [C.c_void_p]
@@ -282,6 +283,10 @@ class PPM:
         """NEXT-3: confining sphere; radius <= 0 switches it off"""
         cen = (C.c_double * 3)(*[float(v) for v in center])
         self._check(lib().ppm_set_sphere(self._h, float(radius), cen))
+
+    def set_two_fluid(self, gamma_tracked, gamma_rest=0.0):
+        """NEXT-4: two-fluid equation of state (reading R25); gamma_tracked <= 0 switches it off"""
+        self._check(lib().ppm_set_two_fluid(self._h, float(gamma_tracked), float(gamma_rest)))
 
     def spin_up(self, domega):
         """NEXT-3: one increment of the solid-body rotation ramp about z"""

@@ -278,6 +278,7 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (c->sphere && ((option == PPM_OPT_IO_PATH && value == 1) || (option == PPM_OPT_FLATTEN3D && value == 1))) {
         set_err(c, "ppm_set_option: not together with the confining sphere"); return PPM_EINVAL;
     }
+    if (c->twof && option == PPM_OPT_FLATTEN3D && value == 1) { set_err(c, "ppm_set_option: PPM_OPT_FLATTEN3D not together with the two-fluid equation of state"); return PPM_EINVAL; }
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
     if (option == PPM_OPT_STATE_FORM && (value == 0 || value == 1)) { c->pert_io = value; return PPM_OK; }
     if (option == PPM_OPT_CFL_FUSED && (value == 0 || value == 1)) { c->cfl_fused = value; c->cfl_valid = 0; return PPM_OK; }
@@ -303,9 +304,21 @@ extern "C" int ppm_set_sphere(ppm_ctx* c, double radius, const double center[3])
     if ((c->prm.nx | c->prm.ny | c->prm.nz) & 3) { set_err(c, "ppm_set_sphere: grid extents must be multiples of 4 (the sphere runs on the bulk-staged sweeps)"); return PPM_EINVAL; }
     if (c->prm.grav.kind == PPM_GRAV_CONST_Z) { set_err(c, "ppm_set_sphere: not with plane-parallel (CONST_Z) gravity"); return PPM_EINVAL; }
     if (c->flat3d) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_FLATTEN3D"); return PPM_EINVAL; }
+    if (c->twof) { set_err(c, "ppm_set_sphere: not together with the two-fluid equation of state"); return PPM_EINVAL; }
     if (c->io_path != 0) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_IO_PATH = 1"); return PPM_EINVAL; }
     c->sphere = 1; c->sph_r = radius;
     for (int d = 0; d < 3; ++d) c->sph_c[d] = center[d];
+    c->cfl_valid = 0;
+    return PPM_OK;
+}
+
+extern "C" int ppm_set_two_fluid(ppm_ctx* c, double gamma_tracked, double gamma_rest) {
+    if (!c) { set_err(nullptr, "ppm_set_two_fluid: ctx is NULL"); return PPM_EINVAL; }
+    if (!(gamma_tracked > 0.0)) { c->twof = 0; c->cfl_valid = 0; return PPM_OK; }
+    if (!(gamma_tracked > 1.0) || !(gamma_rest > 1.0) || !isfinite(gamma_tracked) || !isfinite(gamma_rest)) { set_err(c, "ppm_set_two_fluid: both adiabatic indices must be finite and > 1"); return PPM_EINVAL; }
+    if (c->sphere) { set_err(c, "ppm_set_two_fluid: not together with the confining sphere"); return PPM_EINVAL; }
+    if (c->flat3d) { set_err(c, "ppm_set_two_fluid: not together with PPM_OPT_FLATTEN3D"); return PPM_EINVAL; }
+    c->twof = 1; c->gam_tracked = gamma_tracked; c->gam_rest = gamma_rest;
     c->cfl_valid = 0;
     return PPM_OK;
 }

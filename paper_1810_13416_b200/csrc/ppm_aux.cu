@@ -16,6 +16,9 @@ struct AuxParams {
     const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
     float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
     int sphere;                         // NEXT-3: confining sphere on
+    int twof;                           // NEXT-4: two-fluid EOS, beta(f) = beta2 + f dbeta (reading R25)
+    double beta2, dbeta;
+    float beta2f, dbetaf;
     int pert_io;                        // PPM_OPT_STATE_FORM = 1: the boundary arrays carry rho', p' as stored (no base state added / removed)
     double sph_r2, sph_cx, sph_cy, sph_cz;
 };
@@ -142,11 +145,12 @@ __global__ void __launch_bounds__(256) cfl_kernel(const AuxParams A, const float
     bool bad = false;
     for (long long B = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; B < nbricks; B += nwarps) {
         const float* p = st + B * PPM_BRICK_FLOATS + lane;
-        float v[2][5];
+        float v[2][5], fv[2] = {0.f, 0.f};
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int f = 0; f < 5; ++f) v[h][f] = ld_stream(p + 32 * h + 64 * f);
+        if (A.twof) { fv[0] = ld_stream(p + 64 * 5); fv[1] = ld_stream(p + 32 + 64 * 5); }      // m000: the mixture's Gamma
         const unsigned q = (unsigned)B / (unsigned)A.nbx;
         const int bx = (int)((unsigned)B - q * (unsigned)A.nbx);
         const int bz = (int)(q / (unsigned)A.nby);
@@ -159,7 +163,8 @@ __global__ void __launch_bounds__(256) cfl_kernel(const AuxParams A, const float
             if (aux_is_solid(A, i, j, k)) continue;                        // outside the confining sphere: not part of the flow
             const float2 b0 = base32(A, i, j, k);                          // fp32 base state, as the sweeps evaluate it
             const float rho = b0.x + v[h][0], pr = b0.y + v[h][4];
-            const float xs = gam * pr * __fdividef(1.0f, rho);
+            const float gk = A.twof ? 1.0f + __fdividef(1.0f, fmaf(__saturatef(fv[h]), A.dbetaf, A.beta2f)) : gam;
+            const float xs = gk * pr * __fdividef(1.0f, rho);
             const float cs = xs * rsqrtf(fmaxf(xs, 1e-37f));
             const float sp = fmaxf(fabsf(v[h][1]), fmaxf(fabsf(v[h][2]), fabsf(v[h][3]))) + cs;
             bad |= !(sp == sp) || !(rho > 0.f) || !(pr > 0.f);
@@ -190,7 +195,9 @@ __global__ void __launch_bounds__(256) conserved_kernel(AuxParams A, const float
         const double rho = r0 + (double)st[o], p = p0 + (double)st[o + 4 * 64];
         const double u = st[o + 64], v = st[o + 2 * 64], w = st[o + 3 * 64];
         acc[0] += rho; acc[1] += rho * u; acc[2] += rho * v; acc[3] += rho * w;
-        acc[4] += p / (A.gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w);
+        const double f000 = st[o + 5 * 64];
+        const double beta = A.twof ? A.beta2 + fmin(fmax(f000, 0.0), 1.0) * A.dbeta : 1.0 / (A.gamma - 1.0);     // e = p beta(f)
+        acc[4] += (A.twof ? p * beta : p / (A.gamma - 1.0)) + 0.5 * rho * (u * u + v * v + w * w);
         acc[5] += rho * (double)st[o + 5 * 64];
     }
     __shared__ double sm[6][256];
@@ -375,6 +382,10 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
     A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
     A.pert_io = c->pert_io;
+    A.twof = c->twof;
+    A.beta2 = c->twof ? 1.0 / (c->gam_rest - 1.0) : 0.0;
+    A.dbeta = c->twof ? 1.0 / (c->gam_tracked - 1.0) - A.beta2 : 0.0;
+    A.beta2f = (float)A.beta2; A.dbetaf = (float)A.dbeta;
     A.sphere = c->sphere; A.sph_r2 = c->sph_r * c->sph_r; A.sph_cx = c->sph_c[0]; A.sph_cy = c->sph_c[1]; A.sph_cz = c->sph_c[2];
     return A;
 }

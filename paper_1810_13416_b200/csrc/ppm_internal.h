@@ -43,6 +43,9 @@ struct SweepParams {
     const float2* __restrict__ tabg; // {g_k, g_k+1 - g_k}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
     unsigned int* cflmax;           // non-NULL: fold max_d |u_d| + c of every finished cell into it (bit pattern of a float >= 0)
+    // two-fluid EOS (NEXT-4, reading R25): beta(f) = beta2 + f dbeta, beta2 = 1/(gamma_rest - 1), dbeta = 1/(gamma_tracked - 1) - beta2
+    int twof;
+    float beta2, dbeta;
     // confining sphere (NEXT-3): centre along the (sweep, a, b) axes, radius^2, cell size — fp64, the oracle's criterion
     int sphere;
     double sph_dx, sph_r2, sph_cd, sph_ca, sph_cb;
@@ -71,6 +74,8 @@ struct ppm_ctx {
     int flat3d;                     // PPM_OPT_FLATTEN3D
     int sphere;                     // ppm_set_sphere: confining sphere on (NEXT-3)
     double sph_r, sph_c[3];         // its radius and centre
+    int twof;                       // ppm_set_two_fluid: two-fluid equation of state on (NEXT-4)
+    double gam_tracked, gam_rest;   // adiabatic index of the tracked fluid (FV) and of the rest
     float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
     int sms;                        // multiprocessors of the device
     int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state

@@ -425,10 +425,17 @@ __device__ __forceinline__ int fold_face(const Segment& g, int f) {
 // state into vmax, so that the step's last sweep leaves the next step's CFL maximum behind and ppm_cfl_dt has no pass
 // of its own to make.
 // SPH: confining sphere (above); seg = this lane's fluid segment, gpen = the lane's pencil in the INPUT buffer (cell 0, field 0).
-template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH, class IO>
+// TWOF: two-fluid equation of state (reading R25): e = p beta(f), beta = beta2 + f dbeta with f the
+// PPB cell mean clamped to [0,1]; Gamma = 1 + 1/beta of its own cell on each side of a face, the enthalpy flux with beta of the
+// slab of gas the PPB remap donates through the face, the new pressure from the energy with beta of the NEW f.  mpen = the
+// lane's pencil of m000 in the INPUT buffer (cell 0): Gamma of cell n-2 is needed one iteration before the rings hand over that
+// cell's PPB coefficients, so m000 is read straight from global memory (an L2 hit: the bulk copy fetches the same lines), one
+// iteration ahead of its use.
+template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH, bool TWOF, class IO>
 __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a, const int b, const int c0, const int c1,
                                       const bool valid, const unsigned wmask, const float* __restrict__ pflat, float& vmax,
-                                      const Segment seg = Segment(), const float* __restrict__ gpen = nullptr) {
+                                      const Segment seg = Segment(), const float* __restrict__ gpen = nullptr,
+                                      const float* __restrict__ mpen = nullptr) {
     const float gam = P.gamma, gp = P.gp, gmg = P.gmg, g_gm1 = P.g_gm1;
     const float dtdx = P.dtdx, hdt = P.hdt;
 
@@ -460,6 +467,13 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         float sg;
         const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
         fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+    }
+    // two-fluid EOS: Gamma of cells n-4, n-3 (the cell n-2 joins them inside the iteration); m000 of cell n-2 in flight
+    float Gm4 = gam, Gm3 = gam, mpre = 0.f;
+    if (TWOF) {
+        float sg;
+        const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
+        mpre = __ldg(mpen + (long long)(jf >> 2) * P.SBd + ((jf & 3) << (2 * DIR)));
     }
     // One iteration of the pipeline.  phase = integral_constant<int, S>:
     //   S = -1   any iteration: the brick phase n & 3, the boundary images and the pipeline-fill tests are run-time
@@ -498,7 +512,14 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         // 1/rho is taken once per cell and carried (the tracing and the PPB masses need it again), and c and 1/c^2 come
         // from ONE reciprocal square root: c = x rsqrt(x), 1/c^2 = rsqrt(x)^2 with x = gamma p / rho
         gi[3] = mk(g_new, rcp(fw[2].x));
-        const float xc = gam * fw[2].y * gi[3].y;
+        float Gm2 = gam;                                             // adiabatic index of cell n-2
+        if (TWOF) {
+            Gm2 = 1.0f + rcp(fmaf(sat(mpre), P.dbeta, P.beta2));     // Gamma = 1 + 1/beta(f), f = m000 clamped to [0,1]
+            float sg;
+            const int jf = (S >= 0) ? n - 1 : image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (m000 is even under the mirror)
+            mpre = __ldg(mpen + (long long)(jf >> 2) * P.SBd + ((jf & 3) << (2 * DIR)));
+        }
+        const float xc = Gm2 * fw[2].y * gi[3].y;
         const float icn = rsqrtf(fmaxf(xc, 1e-37f));
         const float cn2 = xc * icn;                                  // c_{n-2}
         const float ic2n = icn * icn;
@@ -599,6 +620,44 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const V5 om = map3(num, den, den, [](float x, float y, float) { return sat(fmaf(fabsf(x) * rcp(y), 5.0f, -0.5f)); });   // H3
             parabola(q[2], Fcl, Fnl, Fc, Fn, om, pLn, pRn);
         }
+        // ---- K (first half): PPB coefficients of cell n-3, pre-limited (P2) ---------------------------
+        // (two-fluid mode takes them BEFORE the Riemann problem: its energy flux needs the donor cells' polynomials)
+        auto ppb_take = [&]() {
+        mv_ppb(mw[0], mw[1]); mv_ppb(mw[1], mw[2]);
+        if (S >= 0 || n - 3 >= c0 - 1) {
+            float m[10];
+            io.template ppb<S>(n - 3, m);
+            if (SPH && (n - 3 < seg.lo || n - 3 > seg.hi) && n - 3 >= seg.lo - PPM_NGHOST && n - 3 <= seg.hi + PPM_NGHOST) {
+                float sg;
+                const int j = fold_cell(seg, n - 3, sg);
+                const float* __restrict__ src = gpen + (long long)(j >> 2) * P.SBd + ((j & 3) << (2 * DIR));
+#pragma unroll
+                for (int k = 0; k < 10; ++k) m[k] = __ldg(src + 64 * (5 + PPB_PERM[DIR][k]));
+                m[1] *= sg; m[4] *= sg; m[6] *= sg;            // the coefficients odd in the normal direction
+            }
+            // bound B: first-order terms 1/2, pure second-order 1/6, mixed 1/4.
+            // local order: a1,b0,c0 are P1 terms; a2,d0,e0 are P2 terms; b1,c1,f0 are mixed P1P1 terms.
+            const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
+            const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
+            const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
+            // theta = min(1, max(0, min(m000, 1 - m000)) / B): 1 wherever the bound B already fits (the constraint is
+            // "almost never performed", PAPER.md L51) — then the coefficients are taken as they are
+            const float room = fmaxf(0.f, fminf(m[0], 1.0f - m[0]));
+            // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
+            if (IO::HAS_FAST) mw[2].a0 = m[0];
+            else asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
+            if ((PPM_UNIFORM_FAST & 8) && __all_sync(wmask, B <= room || !valid)) {
+                mw[2].a1 = m[1]; mw[2].a2 = m[2]; mw[2].f = m[9];
+                mw[2].bc0 = bc0; mw[2].bc1 = bc1; mw[2].de = de;
+            } else {
+                const float th = (B <= room) ? 1.0f : fdiv(room, fmaxf(B, PPM_TINY));
+                mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+                mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
+            }
+            io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
+        }
+        };
+        if (TWOF) ppb_take();
         // ---- I: Riemann problem at face (n-4)+1/2 : L = left state carried from cell n-4, R = right state of cell n-3
         float Frm, Frn, FrE;
         v2 FrB;
@@ -610,11 +669,14 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             r = mk(fmaxf(r.x, P.rho_floor), fmaxf(r.y, P.rho_floor));
             const v2 pp = mk(fmaxf(WLp, pfl), fmaxf(Wp.y, pfl));              // p' (floored)
             const v2 p = bc(p0f) + pp;
-            const v2 C2 = (p * gam) * r;
+            const v2 GK2 = mk(Gm4, Gm3);                                       // two-fluid: Gamma of the left cell n-4, of the right cell n-3
+            const v2 C2 = TWOF ? (p * GK2) * r : (p * gam) * r;
             const v2 C = C2 * mk(rsqrtf(fmaxf(C2.x, 1e-37f)), rsqrtf(fmaxf(C2.y, 1e-37f)));
             const float CLR = C.x * C.y;
             float pps = fmaxf(pfl, fdiv(hsum(swp(C) * pp) + CLR * (Zu.x - Zu.y), C.x + C.y));   // p*' acoustic guess
-            const v2 gpr = r * gp, gmr = C2 * gmg;
+            // W_K^2 = rho_K ((G+1)/2 p* + (G-1)/2 p_K) = gpr p* + gmr
+            const v2 gpr = TWOF ? r * fma2(GK2, bc(0.5f), bc(0.5f)) : r * gp;
+            const v2 gmr = TWOF ? (p * r) * fma2(GK2, bc(0.5f), bc(-0.5f)) : C2 * gmg;
             // Newton on p*' with the two-shock wave speeds W_K; at most 5 iterations (reading R7).  The loop
             // stops early only when EVERY lane's last update is below fp32 resolution of p* (warp-uniform
             // exit), i.e. when further iterations could not change the result beyond rounding.
@@ -663,6 +725,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const float rK = left ? r.x : r.y, uK = left ? Zu.x : Zu.y, pK = left ? p.x : p.y, ppK = left ? pp.x : pp.y;
             const float wk2 = left ? w2.x : w2.y, WK = left ? Ws.x : Ws.y;
             const v2 vw = mk(left ? WLv : Wv.y, left ? WLw : Ww.y);
+            const float GK = TWOF ? (left ? Gm4 : Gm3) : gam;                  // the gas on the upwind side of the contact
             float rs = fdiv(rK * wk2, wk2 - rK * (pps - ppK));                 // 1/(1/rK - (p*-pK)/WK^2)
             rs = fmaxf(rs, P.rho_floor);
             const float uKh = sg * uK, ush = sg * us;
@@ -671,11 +734,11 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // u_K - W_K/rho_K < 0, or a fan whose head u_K - c_K AND tail u* - c*_K are negative — every face of a
             // subsonic flow.  Written without the two sound speeds (u^2 rho < gamma p), and when it holds for every lane
             // of the warp the sampled state is the star state itself.
-            const bool star = shock ? (uKh * rK < WK) : ((uKh < 0.f || uKh * uKh * rK < gam * pK) && ush * ush * rs <= gam * ps);
+            const bool star = shock ? (uKh * rK < WK) : ((uKh < 0.f || uKh * uKh * rK < GK * pK) && ush * ush * rs <= GK * ps);
             float rh = rs, uh = us, pph = pps;
             if (!(PPM_UNIFORM_FAST & 4) || !__all_sync(wmask, star || !valid)) {
                 const float irK = rcp(rK);
-                const float cK = fsqrt(gam * pK * irK), cst = fsqrt(gam * ps * rcp(rs));
+                const float cK = fsqrt(GK * pK * irK), cst = fsqrt(GK * ps * rcp(rs));
                 const float lam_head = uKh - (shock ? WK * irK : cK);
                 const float lam_tail = shock ? lam_head : ush - cst;
                 const float th = (lam_head >= 0.f) ? 0.f : ((lam_tail <= 0.f) ? 1.f : fdiv(-lam_head, lam_tail - lam_head));
@@ -688,42 +751,20 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             Frm = Fm;
             Frn = fmaf(Fm, uh, pph);
             FrB = vw * Fm;
+            if (TWOF) {
+                // the enthalpy of the gas that crosses the face: beta of the mean FV of the slab of mass dt Fm that the PPB
+                // remap takes out of the donor cell (its pre-limited polynomial along the sweep; reading R25)
+                const bool fwd = Fm >= 0.f;
+                const float da0 = fwd ? mw[1].a0 : mw[2].a0, da1 = fwd ? mw[1].a1 : mw[2].a1, da2 = fwd ? mw[1].a2 : mw[2].a2;
+                const float sig = fminf(dtdx * fabsf(Fm) * (fwd ? gi[1].y : gi[2].y), 1.0f);       // donated fraction of the donor's mass
+                const float hs = fmaf(-0.5f, sig, 0.5f), sm = fwd ? hs : -hs;                       // slab midpoint in its mass coordinate
+                const float fs = fmaf(da2, fmaf(sm, sm, fmaf(sig * sig, 1.0f / 12.0f, -1.0f / 12.0f)), fmaf(da1, sm, da0));
+                const float bt1 = fmaf(sat(fs), P.dbeta, P.beta2) + 1.0f;
+                FrE = uh * fmaf(bt1, ph, 0.5f * rh * fmaf(uh, uh, hsum(vw * vw)));
+            } else
             FrE = uh * fmaf(g_gm1, ph, 0.5f * rh * fmaf(uh, uh, hsum(vw * vw)));
         }
-        // ---- K (first half): PPB coefficients of cell n-3, pre-limited (P2) ---------------------------
-        mv_ppb(mw[0], mw[1]); mv_ppb(mw[1], mw[2]);
-        if (S >= 0 || n - 3 >= c0 - 1) {
-            float m[10];
-            io.template ppb<S>(n - 3, m);
-            if (SPH && (n - 3 < seg.lo || n - 3 > seg.hi) && n - 3 >= seg.lo - PPM_NGHOST && n - 3 <= seg.hi + PPM_NGHOST) {
-                float sg;
-                const int j = fold_cell(seg, n - 3, sg);
-                const float* __restrict__ src = gpen + (long long)(j >> 2) * P.SBd + ((j & 3) << (2 * DIR));
-#pragma unroll
-                for (int k = 0; k < 10; ++k) m[k] = __ldg(src + 64 * (5 + PPB_PERM[DIR][k]));
-                m[1] *= sg; m[4] *= sg; m[6] *= sg;            // the coefficients odd in the normal direction
-            }
-            // bound B: first-order terms 1/2, pure second-order 1/6, mixed 1/4.
-            // local order: a1,b0,c0 are P1 terms; a2,d0,e0 are P2 terms; b1,c1,f0 are mixed P1P1 terms.
-            const v2 bc0 = mk(m[3], m[5]), bc1 = mk(m[4], m[6]), de = mk(m[7], m[8]);
-            const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
-            const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
-            // theta = min(1, max(0, min(m000, 1 - m000)) / B): 1 wherever the bound B already fits (the constraint is
-            // "almost never performed", PAPER.md L51) — then the coefficients are taken as they are
-            const float room = fmaxf(0.f, fminf(m[0], 1.0f - m[0]));
-            // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
-            if (IO::HAS_FAST) mw[2].a0 = m[0];
-            else asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
-            if ((PPM_UNIFORM_FAST & 8) && __all_sync(wmask, B <= room || !valid)) {
-                mw[2].a1 = m[1]; mw[2].a2 = m[2]; mw[2].f = m[9];
-                mw[2].bc0 = bc0; mw[2].bc1 = bc1; mw[2].de = de;
-            } else {
-                const float th = (B <= room) ? 1.0f : fdiv(room, fmaxf(B, PPM_TINY));
-                mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
-                mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
-            }
-            io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
-        }
+        if (!TWOF) ppb_take();
         // ---- J, K, L: finish cell n-4 ---------------------------------------------------------------------
         const int i = n - PPM_NGHOST;
         if (S >= 0 || i >= c0) {
@@ -755,18 +796,26 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const float u1 = mu1 * irn;
             const v2 vw1 = mB * irn;
             const float dKE = 0.5f * (r_new * fmaf(u1, u1, hsum(vw1 * vw1)) - r_old * fmaf(u0, u0, hsum(vw0 * vw0)));
-            float pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
+            float pp_new, Gnew = gam;
+            if (TWOF) {
+                // p beta is what the energy equation advances: p_new = (p_old beta_old + dE - dKE) / beta_new with beta of the
+                // NEW cell mean of FV, i.e. after this sweep's remap; in increment form on the perturbation
+                ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+                const float ibn = rcp(fmaf(sat(mo[0]), P.dbeta, P.beta2));
+                pp_new = pp_old + ((dE - dKE) - fw[0].y * (P.dbeta * (sat(mo[0]) - sat(mw[1].a0)))) * ibn;
+                Gnew = 1.0f + ibn;
+            } else pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
             const float p0c = fw[0].y - pp_old;
             if (!(p0c + pp_new > P.p_floor)) { pp_new = P.p_floor - p0c; bad = 1; }
             const bool fluid = !SPH || (i >= seg.lo && i <= seg.hi);
             if (bad && valid && fluid) atomicOr(P.flag, (r_new == r_new && pp_new == pp_new) ? 1 : 2);
             if (CFL && fluid) {                                         // C6 on the new state: c from the full rho, p
-                const float xs = gam * (p0c + pp_new) * irn;
+                const float xs = Gnew * (p0c + pp_new) * irn;
                 const float cnew = xs * rsqrtf(fmaxf(xs, 1e-37f));
                 vmax = fmaxf(vmax, fmaxf(fabsf(u1), fmaxf(fabsf(vw1.x), fabsf(vw1.y))) + cnew);
             }
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
-            ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+            if (!TWOF) ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
             io.template store<S>(i, ho, mo, fluid);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
@@ -775,6 +824,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
         Flm = Frm; Fln = Frn; FlE = FrE; FlB = MV2D(FrB);
         ft0 = ft1; ft1 = ftn; cs = cn2; b0fc = b0fn;
         ic2s = ic2n;
+        if (TWOF) { Gm4 = Gm3; Gm3 = Gm2; }
     };
     using std::integral_constant;
     if (IO::HAS_FAST) {
@@ -959,7 +1009,7 @@ struct IoDirect {
 
 // thread -> pencil: 16 lanes = the 4x4 transverse cells of one brick column; a CTA of 128 threads = 8 brick
 // columns adjacent along a.  (a, b) = the two transverse axes in increasing axis order.
-template <int DIR, int GRAV, bool FLAT>
+template <int DIR, int GRAV, bool FLAT, bool TWOF>
 __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
     const int t = threadIdx.x;
@@ -975,7 +1025,7 @@ __global__ void __maxnreg__(PPM_MAXREG) ppm_sweep_kernel(const SweepParams P) {
     IoDirect<DIR> io(P, tb, c0 - PPM_NGHOST, c0);
     const float* pflat = FLAT ? P.flat + ((long long)ba * P.FBa + (long long)bb * P.FBb + (((t & 3) << (2 * AXA)) + (((t >> 2) & 3) << (2 * AXB)))) : nullptr;
     float vmax = 0.f;
-    march<DIR, GRAV, FLAT, false, false>(P, io, a, b, c0, c1, true, wmask, pflat, vmax);
+    march<DIR, GRAV, FLAT, false, false, TWOF>(P, io, a, b, c0, c1, true, wmask, pflat, vmax, Segment(), nullptr, TWOF ? P.in + tb + 5 * 64 : nullptr);
 }
 
 // PPB-only sweep (NEXT-2), direct path
@@ -1326,7 +1376,7 @@ __device__ __forceinline__ unsigned bulk_copy_through(const SweepParams& P, floa
     return ph;
 }
 
-template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH>
+template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH, bool TWOF>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1373,11 +1423,15 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
     float vmax = 0.f;
     if (SPH) {
         const float* gpen = P.in + gcol + (long long)(lane >> 4) * P.SBa + (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)));
-        march<DIR, GRAV, FLAT, CFL, true>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax, seg, gpen);
+        march<DIR, GRAV, FLAT, CFL, true, false>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax, seg, gpen);
         bulk_copy_through<DIR>(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), lane, gcol, min(2, nba - ba0), c1, c1s, io.ph);
         (void)c0s;
-    } else
-    march<DIR, GRAV, FLAT, CFL, false>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax);
+    } else {
+        // two-fluid EOS: the lane's pencil of m000 in the input buffer (pad lanes of a ragged grid read their clamped column)
+        const float* mpen = TWOF ? P.in + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.SBa + (long long)bb * P.SBb + 5 * 64 +
+                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
+        march<DIR, GRAV, FLAT, CFL, false, TWOF>(P, io, a, b, c0, c1, valid, 0xffffffffu, pflat, vmax, Segment(), nullptr, mpen);
+    }
     if (CFL) {
         // warp max by one REDUX on the bit patterns (non-negative floats order like unsigned integers; a NaN has the
         // largest pattern and so survives: ppm_cfl_dt reports it), then one atomicMax per warp
@@ -1456,15 +1510,24 @@ cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_
 }
 template <int DIR, int GRAV, bool FLAT>
 cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ[4][MAX_DEV] = {};
+    static int occ[6][MAX_DEV] = {};
     if (P.sphere) {     // confining sphere (NEXT-3): no plane-parallel gravity, no 3-D flattening (ppm_set_sphere checks)
         if constexpr (GRAV != PPM_GRAV_CONST_Z && !FLAT) {
-            if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, true, true>, occ[3], P, sms, user_chunk, st);
-            return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, false, true>, occ[2], P, sms, user_chunk, st);
+            if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, true, true, false>, occ[3], P, sms, user_chunk, st);
+            return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, false, true, false>, occ[2], P, sms, user_chunk, st);
         } else return cudaErrorNotSupported;
     }
-    if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, true, false>, occ[1], P, sms, user_chunk, st);
-    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false, false>, occ[0], P, sms, user_chunk, st);
+    if (P.twof) {       // two-fluid EOS (NEXT-4): not with the 3-D flattening mode (ppm_set_two_fluid checks)
+#ifndef PPM_EXP_ONE
+        if constexpr (!FLAT) {
+            if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, true, false, true>, occ[5], P, sms, user_chunk, st);
+            return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, false, false, false, true>, occ[4], P, sms, user_chunk, st);
+        } else
+#endif
+        return cudaErrorNotSupported;
+    }
+    if (P.cflmax) return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, true, false, false>, occ[1], P, sms, user_chunk, st);
+    return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false, false, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
@@ -1493,15 +1556,19 @@ cudaError_t launch_dir(const SweepParams& P, int grav, dim3 grid, dim3 block, cu
     (void)fl; (void)grav; (void)grid; (void)block; (void)st; (void)P;
     return cudaErrorNotSupported;
 #else
+    if (P.twof && fl) return cudaErrorNotSupported;
     switch (grav) {
         case PPM_GRAV_NONE:
-            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_NONE, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_NONE, false><<<grid, block, 0, st>>>(P);
+            if (P.twof) ppm_sweep_kernel<DIR, PPM_GRAV_NONE, false, true><<<grid, block, 0, st>>>(P);
+            else if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_NONE, true, false><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_NONE, false, false><<<grid, block, 0, st>>>(P);
             break;
         case PPM_GRAV_CONST_Z:
-            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, false><<<grid, block, 0, st>>>(P);
+            if (P.twof) ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, false, true><<<grid, block, 0, st>>>(P);
+            else if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, true, false><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_CONST_Z, false, false><<<grid, block, 0, st>>>(P);
             break;
         default:
-            if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, true><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, false><<<grid, block, 0, st>>>(P);
+            if (P.twof) ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, false, true><<<grid, block, 0, st>>>(P);
+            else if (fl) ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, true, false><<<grid, block, 0, st>>>(P); else ppm_sweep_kernel<DIR, PPM_GRAV_RADIAL, false, false><<<grid, block, 0, st>>>(P);
             break;
     }
     return cudaGetLastError();
@@ -1543,6 +1610,9 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
     P.tab = c->tab; P.tabp = c->tabp; P.tabg = c->tabg;
     P.flag = c->flag;
+    P.twof = c->twof;
+    P.beta2 = (float)(1.0 / (c->twof ? c->gam_rest - 1.0 : p.gamma - 1.0));
+    P.dbeta = (float)(c->twof ? 1.0 / (c->gam_tracked - 1.0) - 1.0 / (c->gam_rest - 1.0) : 0.0);
     P.sphere = c->sphere;
     if (c->sphere) {
         P.sph_dx = p.dx; P.sph_r2 = c->sph_r * c->sph_r;

@@ -44,12 +44,17 @@ def _load(g, w, device="cuda", nzs=32):
         g.set_state(w.fields((0, 0, z0), (n, n, z1), device=device), z0=z0)
 
 
-def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False):
-    """steps on both sides with the GPU's dt; returns dict of results after step 1 and at the end."""
+def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False, twofluid=None, edit=None):
+    """steps on both sides with the GPU's dt; returns dict of results after step 1 and at the end.
+    twofluid = (gamma_tracked, gamma_rest): NEXT-4 on both sides; edit(f): in-place change of the input fields."""
     PPM = _gpu()
     from paper_1810_13416_b200.binding import OPT_FLATTEN3D, OPT_IO_PATH
     f = w.fields()
+    if edit is not None:
+        edit(f)
     o = _oracle(w)
+    if twofluid:
+        o.set_two_fluid(*twofluid)
     o.set_state(f.numpy())
     g = PPM.from_workload(w)
     if chunk:
@@ -59,6 +64,8 @@ def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False):
         o.set_flatten3d(True)
     if direct:
         g.set_option(OPT_IO_PATH, 1)
+    if twofluid:
+        g.set_two_fluid(*twofluid)
     g.set_state(f.cuda())
     out = {}
     c0g, c0o = g.reduce_conserved(), o.reduce_conserved()
@@ -674,6 +681,143 @@ def test_sphere_cfg4_full_512_windows_that_straddle_the_sphere():
     c = 256
     _window_check(4, 2, [((c + 248, c, c), 24), ((c + 178, c + 178, c), 24), ((c + 150, c + 140, c + 150), 24), ((c + 175, c, c), 24)],
                   sphere=(0.5, (0.5, 0.5, 0.5)))
+
+
+# ---------------------------------------------------------------- NEXT-4: two-fluid equation of state ------
+TWO_FLUID = (1.4, 5.0 / 3.0)        # tracked fluid (FV), the rest
+
+
+@pytest.mark.parametrize("direct", [False, True])
+def test_two_fluid_cfg1_matches_oracle(direct):
+    """config 1 (periodic, FV = tanh slab between 0.1 and 0.9: every cell is a mixture, Gamma varies between 1.43 and 1.63)
+    with the velocities raised to Mach 0.3 so that the energy equation really works; 20 steps, both data paths"""
+    w = W.make(1)
+
+    def edit(f):
+        f[1:4] *= 8.0
+    r = _run_pair(w, w.steps, twofluid=TWO_FLUID, direct=direct, edit=edit)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[w.steps][0].values()) <= MULTI_STEP, r[w.steps][0]
+    assert r["cons0"].max() <= CONS and r["cons1"].max() <= CONS
+    # the mixture's total energy sum(p beta(f) + KE) is conserved on the periodic box (fp32 round-off only)
+    c0, d = r["c0"], r["drift_gpu"]
+    assert d[0] <= 2e-6 * c0[0] and d[4] <= 2e-6 * c0[4] and d[5] <= 2e-6 * c0[5]
+    print("two-fluid cfg1 (%s path): after 1 step %s, after %d steps %s" % ("direct" if direct else "bulk", r[1][0], w.steps, r[w.steps][0]))
+
+
+def test_two_fluid_differs_from_single_fluid_and_equal_gammas_do_not():
+    """the mode really changes the flow (so the test above is not vacuous), and with gamma_tracked = gamma_rest it is the
+    single-fluid scheme to fp32 round-off"""
+    PPM = _gpu()
+    w = W.make(1)
+    f = w.fields()
+    f[1:4] *= 8.0
+    res = []
+    for tf in (None, (w.gamma, w.gamma), TWO_FLUID):
+        g = PPM.from_workload(w)
+        if tf:
+            g.set_two_fluid(*tf)
+        g.set_state(f.cuda())
+        for s in range(5):
+            g.step(0.004, s)
+        res.append(g.get_state().cpu().numpy().astype(np.float64))
+        g.close()
+    e_same = max_rel(res[1], res[0])
+    e_diff = max_rel(res[2], res[0])
+    assert max(e_same.values()) <= 2e-6, e_same
+    assert e_diff["p"] > 1e-3, e_diff
+
+
+def test_two_fluid_blast_through_a_gas_interface_L1():
+    """config 3 at 64^3 (Mach-3 blast, density contrast 1000) with the dense layer made of the OTHER gas (FV = the interface
+    tanh instead of 1e-5 of it): shocks, the limiter and the Newton iterations with one Gamma per side; 30 steps"""
+    w = W.make(3, n=64)
+
+    def edit(f):
+        f[5:] *= 1e5
+    r = _run_pair(w, 30, twofluid=TWO_FLUID, edit=edit)
+    assert max(r[1][1].values()) <= L1_SHOCK, r[1][1]
+    assert max(r[30][1].values()) <= L1_SHOCK, r[30][1]
+    assert r["cons1"].max() <= CONS
+    gs, os_ = r["final"]
+    assert np.abs(os_[1:4]).max() > 2.0 and os_[5].max() > 0.99
+    print("two-fluid blast: L1 after 1 step %s, after 30 steps %s" % (r[1][1], r[30][1]))
+
+
+def test_two_fluid_stratified_box_with_gravity():
+    """config 2 at 64^3 (constant gravity, reflecting z walls, FV = 1 above z = 0.6): the hydrostatic base state does not depend
+    on the gases' adiabatic indices, the perturbation equations do; 40 steps"""
+    w = W.make(2, n=64)
+    r = _run_pair(w, 40, twofluid=TWO_FLUID)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[40][0].values()) <= MULTI_STEP, r[40][0]
+    assert r["cons1"].max() <= CONS
+    assert r["pert"]["rho'"] <= PERT_TOL and r["pert"]["p'"] <= PERT_TOL, r["pert"]
+
+
+def test_two_fluid_radial_gravity_convection_zone():
+    """config 4 at 64^3 (radial gravity, FV = 1 outside r = 0.45): the stable layer is the other gas; 10 steps"""
+    w = W.make(4, n=64)
+    r = _run_pair(w, 10, twofluid=TWO_FLUID)
+    assert max(r[1][0].values()) <= ONE_STEP, r[1][0]
+    assert max(r[10][0].values()) <= MULTI_STEP, r[10][0]
+    assert r["cons1"].max() <= CONS
+    assert r["pert"]["rho'"] <= PERT_TOL and r["pert"]["p'"] <= PERT_TOL, r["pert"]
+
+
+def test_two_fluid_ragged_grid_mixed_boundaries():
+    """37 x 29 x 24: direct path along x and y (ragged), bulk along z; reflecting x, periodic y, reflecting z"""
+    PPM = _gpu()
+    from oracle import binding as ob
+    rng = np.random.default_rng(77)
+    nx, ny, nz = 37, 29, 24
+    dx = 1.0 / 40
+    bc = (1, 1, 0, 0, 1, 1)
+    f = torch.zeros((15, nz, ny, nx), dtype=torch.float32)
+    z, y, x = np.meshgrid((np.arange(nz) + 0.5) * dx, (np.arange(ny) + 0.5) * dx, (np.arange(nx) + 0.5) * dx, indexing="ij")
+    f[0] = torch.from_numpy(1.0 + 0.3 * np.sin(7 * x) * np.cos(5 * y) + 0.2 * np.sin(9 * z))
+    f[4] = torch.from_numpy(0.8 + 0.2 * np.cos(6 * x + 4 * z))
+    for k in (1, 2, 3):
+        f[k] = torch.from_numpy(0.3 * np.sin(5 * x + 3 * y + 4 * z + k))
+    f[5] = torch.from_numpy(0.5 + 0.45 * np.tanh((np.sin(6 * x) + np.cos(5 * y) + np.sin(4 * z)) / 0.3))
+    f[6:] = torch.from_numpy(0.01 * rng.standard_normal((9, nz, ny, nx)))
+    g = PPM(nx, ny, nz, dx, 5.0 / 3.0, bc)
+    g.set_two_fluid(*TWO_FLUID)
+    g.set_state(f.cuda())
+    o = ob.Oracle(nx, ny, nz, dx, 5.0 / 3.0, bc, None)
+    o.set_two_fluid(*TWO_FLUID)
+    o.set_state(f.numpy())
+    for s in range(6):
+        dt = g.cfl_dt(0.6)
+        assert abs(dt - o.cfl_dt(0.6)) <= DT_TOL * dt
+        g.step(dt, s)
+        o.step(dt, s)
+        if s == 0:
+            e1 = max_rel(g.get_state().cpu().numpy().astype(np.float64), o.get_state())
+            assert max(e1.values()) <= ONE_STEP, e1
+    e = max_rel(g.get_state().cpu().numpy().astype(np.float64), o.get_state())
+    assert max(e.values()) <= MULTI_STEP, e
+    assert conserved_rel(g.reduce_conserved(), o.reduce_conserved(), o.get_state(), dx, 5.0 / 3.0).max() <= CONS
+    g.close()
+
+
+def test_two_fluid_argument_checks():
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_FLATTEN3D
+    w = W.make(4, n=32)
+    g = PPM.from_workload(w)
+    with pytest.raises(Exception):
+        g.set_two_fluid(0.9, 1.4)                       # an adiabatic index <= 1
+    g.set_two_fluid(*TWO_FLUID)
+    with pytest.raises(Exception):
+        g.set_sphere(0.5, (0.5, 0.5, 0.5))              # the two NEXT modes are not combined
+    with pytest.raises(Exception):
+        g.set_option(OPT_FLATTEN3D, 1)
+    g.set_two_fluid(0.0)                                # off again
+    g.set_sphere(0.5, (0.5, 0.5, 0.5))
+    with pytest.raises(Exception):
+        g.set_two_fluid(*TWO_FLUID)
+    g.close()
 
 
 # ---------------------------------------------------------------- full-size configs on windows --------
