@@ -38,7 +38,8 @@ extern "C" {
 typedef struct ppm_ctx ppm_ctx; /* opaque; owns only small device scratch (tables, reduction cells) */
 
 enum { PPM_OK = 0, PPM_EINVAL = 1, PPM_ENOMEM = 2, PPM_ECUDA = 3, PPM_ESTATE = 4 };
-enum { PPM_BC_PERIODIC = 0, PPM_BC_REFLECT = 1 }; /* per face: xlo,xhi,ylo,yhi,zlo,zhi; periodic must pair up */
+enum { PPM_BC_PERIODIC = 0, PPM_BC_REFLECT = 1, PPM_BC_HALO = 2 }; /* per face: xlo,xhi,ylo,yhi,zlo,zhi; periodic must pair up;
+                                                     HALO: the cells beyond the face belong to a neighbouring sub-domain (see ppm_set_halo) */
 enum { PPM_GRAV_NONE = 0, PPM_GRAV_CONST_Z = 1, PPM_GRAV_RADIAL = 2 };
 #define PPM_NFIELDS 15
 #define PPM_NGHOST 4 /* stencil reach per sweep */
@@ -161,6 +162,40 @@ int ppm_set_option(ppm_ctx *ctx, int option, int value);
  * PPM_EINVAL unless all six faces are PPM_BC_REFLECT, the extents are multiples of 4, gravity is NONE or RADIAL, and
  * neither PPM_OPT_FLATTEN3D nor PPM_OPT_IO_PATH = 1 is set.  Host-side state only (no launch). */
 int ppm_set_sphere(ppm_ctx *ctx, double radius, const double center[3]);
+
+/* ---- Brick decomposition over several GPUs ("each MPI rank ... a grid brick ... must
+ * exchange ... a halo one briquette thick").  One context per sub-domain (one process per GPU); a face shared with a neighbouring
+ * sub-domain has the boundary type PPM_BC_HALO.  A 1-D sweep along an axis only ever needs ghost cells ALONG that axis, 4 deep = one
+ * brick layer, so before each sweep a sub-domain packs its first and last brick layer along the sweep axis (ppm_pack_halo), the
+ * layers travel to the two neighbours (NCCL send/recv or a peer copy — the caller's plumbing), and the sweep reads the received
+ * layer as its ghost brick (ppm_set_halo).  No edge or corner data is ever exchanged and no ghost cell is updated redundantly.
+ * The results are bit for bit those of the undivided grid (ppm_set_origin makes the base state be evaluated at the global
+ * positions).  A grid with a HALO face advances with ppm_sweep / ppm_sweep_cfl (ppm_step returns PPM_EINVAL: an exchange is due
+ * between its sweeps); the extent along an axis with a HALO face must be a multiple of 4 and >= 8.  Not combined with
+ * PPM_OPT_FLATTEN3D, PPM_OPT_IO_PATH = 1, ppm_set_sphere, ppm_set_two_fluid or ppm_advect. */
+
+/* Floats in one brick layer normal to `axis` of an nx x ny x nz grid (= the size of a halo buffer): 960 * ceil(n_a/4) * ceil(n_b/4)
+ * with a, b the two other axes.  0 for bad arguments.  Pure host arithmetic. */
+size_t ppm_halo_floats(int nx, int ny, int nz, int axis);
+
+/* Gathers the first (side = 0: cells 0..3) or last (side = 1) brick layer along `axis` of the current state into dev_dst [device,
+ * ppm_halo_floats() floats, 16-byte aligned]: whole brick records, ordered [bricks along b][bricks along a] with a < b the two other
+ * axes.  Only enqueues work (1 copy kernel). */
+int ppm_pack_halo(ppm_ctx *ctx, int axis, int side, float *dev_dst);
+
+/* Registers the brick layer of the neighbour beyond the low (side = 0) or high (side = 1) face of `axis` — a buffer filled by the
+ * NEIGHBOUR's ppm_pack_halo(axis, 1 - side) — as the ghost brick of the sweeps along `axis`.  dev_layer: [device], borrowed until
+ * replaced or the context is destroyed; its contents are read by every later ppm_sweep along that axis (stream-ordered: refill it
+ * before each).  PPM_EINVAL unless that face is PPM_BC_HALO.  Host-side state only. */
+int ppm_set_halo(ppm_ctx *ctx, int axis, int side, const float *dev_layer);
+
+/* Global cell index of this grid's cell (0,0,0) [host, 3 ints >= 0]: positions (the radial distance of the gravity profile, the
+ * spin-up axis) are then taken at the global cell centres, with the arithmetic of the undivided grid.  Host-side state only. */
+int ppm_set_origin(ppm_ctx *ctx, const int org[3]);
+
+/* ppm_sweep that also reduces the CFL maximum of the state it writes (S10 fused, as the last sweep of ppm_step does), so that
+ * the next ppm_cfl_dt reads 4 bytes back: the last sweep of a step driven sweep by sweep. */
+int ppm_sweep_cfl(ppm_ctx *ctx, double dt, int axis);
 
 /* Two-fluid equation of state ("multifluid", L87 "fv ... gives the fraction of the volume of a
  * cell that is occupied by a special, tracked multifluid constituent"; the paper prints no EOS: reading R25 in DESIGN.md).  The

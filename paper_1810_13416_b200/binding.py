@@ -17,12 +17,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("PPM_B200_LIB") or os.path.join(HERE, "libppm_b200.so")
 
 PPM_OK, PPM_EINVAL, PPM_ENOMEM, PPM_ECUDA, PPM_ESTATE = 0, 1, 2, 3, 4
-BC_PERIODIC, BC_REFLECT = 0, 1
+BC_PERIODIC, BC_REFLECT, BC_HALO = 0, 1, 2
 GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
            "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
-           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_set_two_fluid", "ppm_destroy",
+           "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_set_two_fluid", "ppm_halo_floats", "ppm_pack_halo", "ppm_set_halo",
+           "ppm_set_origin", "ppm_sweep_cfl", "ppm_destroy",
            "ppm_last_error")
 OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED, OPT_STATE_FORM = 2, 3, 4, 5
 
@@ -72,6 +73,12 @@ def lib():
         L.ppm_set_sphere.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.ppm_spin_up.argtypes = [C.c_void_p, C.c_double]
         L.ppm_set_two_fluid.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.ppm_halo_floats.restype = C.c_size_t
+        L.ppm_halo_floats.argtypes = [C.c_int] * 4
+        L.ppm_pack_halo.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.ppm_set_halo.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.ppm_set_origin.argtypes = [C.c_void_p, C.POINTER(C.c_int)]
+        L.ppm_sweep_cfl.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.ppm_destroy.argtypes = [C.c_void_p]
         L.ppm_destroy.restype = None
         L.ppm_last_error.argtypes = [C.c_void_p]
@@ -283,6 +290,28 @@ class PPM:
         """NEXT-3: confining sphere; radius <= 0 switches it off"""
         cen = (C.c_double * 3)(*[float(v) for v in center])
         self._check(lib().ppm_set_sphere(self._h, float(radius), cen))
+
+    # ---- NEXT-4: brick decomposition (the exchange itself lives in paper_1810_13416_b200/decomposition.py) ----
+    def halo_floats(self, axis):
+        return int(lib().ppm_halo_floats(self.n[0], self.n[1], self.n[2], int(axis)))
+
+    def pack_halo(self, axis, side, dst):
+        """the first (side 0) / last (side 1) brick layer along `axis` -> dst (device float32 tensor of halo_floats(axis))"""
+        assert dst.is_cuda and dst.dtype == torch.float32 and dst.is_contiguous() and dst.numel() >= self.halo_floats(axis)
+        self._check(lib().ppm_pack_halo(self._h, int(axis), int(side), C.c_void_p(dst.data_ptr())))
+
+    def set_halo(self, axis, side, layer):
+        """registers the neighbour's brick layer (device tensor, kept alive by this object) as the ghost brick beyond that face"""
+        assert layer.is_cuda and layer.dtype == torch.float32 and layer.is_contiguous() and layer.numel() >= self.halo_floats(axis)
+        self._halos = getattr(self, "_halos", {})
+        self._halos[(axis, side)] = layer
+        self._check(lib().ppm_set_halo(self._h, int(axis), int(side), C.c_void_p(layer.data_ptr())))
+
+    def set_origin(self, org):
+        self._check(lib().ppm_set_origin(self._h, (C.c_int * 3)(*[int(v) for v in org])))
+
+    def sweep_cfl(self, dt, axis):
+        self._check(lib().ppm_sweep_cfl(self._h, float(dt), int(axis)))
 
     def set_two_fluid(self, gamma_tracked, gamma_rest=0.0):
         """NEXT-4: two-fluid equation of state (reading R25); gamma_tracked <= 0 switches it off"""

@@ -60,10 +60,13 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     const int ext[3] = {prm->nx, prm->ny, prm->nz};
     for (int d = 0; d < 3; ++d) {
         const int lo = prm->bc[2 * d], hi = prm->bc[2 * d + 1];
-        if ((lo != PPM_BC_PERIODIC && lo != PPM_BC_REFLECT) || (hi != PPM_BC_PERIODIC && hi != PPM_BC_REFLECT)) {
+        if ((lo != PPM_BC_PERIODIC && lo != PPM_BC_REFLECT && lo != PPM_BC_HALO) || (hi != PPM_BC_PERIODIC && hi != PPM_BC_REFLECT && hi != PPM_BC_HALO)) {
             set_err(c, "ppm_create: unknown boundary type on axis %d", d); return PPM_EINVAL;
         }
         if ((lo == PPM_BC_PERIODIC) != (hi == PPM_BC_PERIODIC)) { set_err(c, "ppm_create: periodic faces must pair up (axis %d)", d); return PPM_EINVAL; }
+        if ((lo == PPM_BC_HALO || hi == PPM_BC_HALO) && (ext[d] % 4 != 0 || ext[d] < 8)) {
+            set_err(c, "ppm_create: an axis with a PPM_BC_HALO face needs an extent that is a multiple of 4 and >= 8 (axis %d)", d); return PPM_EINVAL;
+        }
         if (lo == PPM_BC_REFLECT && ext[d] < PPM_NGHOST) { set_err(c, "ppm_create: reflecting axis %d needs >= %d cells", d, PPM_NGHOST); return PPM_EINVAL; }
     }
     const ppm_gravity& g = prm->grav;
@@ -197,20 +200,44 @@ extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z
     return dst_is_device ? PPM_OK : read_flag(c);
 }
 
-extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) {
-    if (!c) { set_err(nullptr, "ppm_sweep: ctx is NULL"); return PPM_EINVAL; }
-    DevGuard guard(c);
-    if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "ppm_sweep: need finite dt > 0 and axis in 0..2"); return PPM_EINVAL; }
-    if (c->flat3d) CU(ppm_launch_flatten3d(c));     // the detector field of the state this sweep starts from
-    c->cfl_valid = 0;
-    CU(ppm_launch_sweep(c, axis, dt));
+// PPM_BC_HALO faces: the sweep along `axis` reads the neighbour's brick layer — it must have been handed over, and only the
+// bulk-staged sweeps of the plain scheme know how to
+static int halo_ready(ppm_ctx* c, int axis, const char* who) {
+    const bool lo = c->prm.bc[2 * axis] == PPM_BC_HALO, hi = c->prm.bc[2 * axis + 1] == PPM_BC_HALO;
+    if (!lo && !hi) return PPM_OK;
+    if ((lo && !c->halo[axis][0]) || (hi && !c->halo[axis][1])) { set_err(c, "%s: axis %d has a PPM_BC_HALO face without a halo layer (ppm_set_halo)", who, axis); return PPM_EINVAL; }
+    if (!ppm_axis_is_bulk(c, axis)) { set_err(c, "%s: PPM_BC_HALO faces need the bulk-staged path (PPM_OPT_IO_PATH = 0)", who); return PPM_EINVAL; }
+    if (c->flat3d || c->twof || c->sphere) { set_err(c, "%s: PPM_BC_HALO faces are not combined with PPM_OPT_FLATTEN3D, the two-fluid EOS or the sphere", who); return PPM_EINVAL; }
     return PPM_OK;
 }
+static bool has_halo(const ppm_ctx* c) {
+    for (int k = 0; k < 6; ++k) if (c->prm.bc[k] == PPM_BC_HALO) return true;
+    return false;
+}
+
+static int sweep_impl(ppm_ctx* c, double dt, int axis, bool with_cfl, const char* who) {
+    if (!c) { set_err(nullptr, "%s: ctx is NULL", who); return PPM_EINVAL; }
+    DevGuard guard(c);
+    if (!(dt > 0.0) || !isfinite(dt) || axis < 0 || axis > 2) { set_err(c, "%s: need finite dt > 0 and axis in 0..2", who); return PPM_EINVAL; }
+    int rc = halo_ready(c, axis, who);
+    if (rc) return rc;
+    if (c->flat3d) CU(ppm_launch_flatten3d(c));     // the detector field of the state this sweep starts from
+    c->cfl_valid = 0;
+    const bool fuse = with_cfl && c->cfl_fused && ppm_axis_is_bulk(c, axis);
+    if (fuse) CU(cudaMemsetAsync(c->cflmax, 0, sizeof(unsigned int), c->stream));
+    CU(ppm_launch_sweep(c, axis, dt, false, fuse));
+    if (fuse) c->cfl_valid = 1;
+    return PPM_OK;
+}
+
+extern "C" int ppm_sweep(ppm_ctx* c, double dt, int axis) { return sweep_impl(c, dt, axis, false, "ppm_sweep"); }
+extern "C" int ppm_sweep_cfl(ppm_ctx* c, double dt, int axis) { return sweep_impl(c, dt, axis, true, "ppm_sweep_cfl"); }
 
 extern "C" int ppm_step(ppm_ctx* c, double dt, int sweep_order) {
     if (!c) { set_err(nullptr, "ppm_step: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_step: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
+    if (has_halo(c)) { set_err(c, "ppm_step: a grid with PPM_BC_HALO faces advances sweep by sweep (ppm_sweep / ppm_sweep_cfl), the halo layers exchanged before each"); return PPM_EINVAL; }
     if (c->flat3d) CU(ppm_launch_flatten3d(c));     // once per step, on the step's starting state
     c->cfl_valid = 0;
     for (int s = 0; s < 3; ++s) {
@@ -229,6 +256,7 @@ extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
     DevGuard guard(c);
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_advect: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
     if (c->sphere) { set_err(c, "ppm_advect: the PPB-only mode has no confining sphere"); return PPM_EINVAL; }
+    if (has_halo(c)) { set_err(c, "ppm_advect: not on a grid with PPM_BC_HALO faces"); return PPM_EINVAL; }
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt, true));
     return PPM_OK;
 }
@@ -304,10 +332,51 @@ extern "C" int ppm_set_sphere(ppm_ctx* c, double radius, const double center[3])
     if ((c->prm.nx | c->prm.ny | c->prm.nz) & 3) { set_err(c, "ppm_set_sphere: grid extents must be multiples of 4 (the sphere runs on the bulk-staged sweeps)"); return PPM_EINVAL; }
     if (c->prm.grav.kind == PPM_GRAV_CONST_Z) { set_err(c, "ppm_set_sphere: not with plane-parallel (CONST_Z) gravity"); return PPM_EINVAL; }
     if (c->flat3d) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_FLATTEN3D"); return PPM_EINVAL; }
+    if (c->org[0] | c->org[1] | c->org[2]) { set_err(c, "ppm_set_sphere: not on a sub-domain (ppm_set_origin)"); return PPM_EINVAL; }
     if (c->twof) { set_err(c, "ppm_set_sphere: not together with the two-fluid equation of state"); return PPM_EINVAL; }
     if (c->io_path != 0) { set_err(c, "ppm_set_sphere: not together with PPM_OPT_IO_PATH = 1"); return PPM_EINVAL; }
     c->sphere = 1; c->sph_r = radius;
     for (int d = 0; d < 3; ++d) c->sph_c[d] = center[d];
+    c->cfl_valid = 0;
+    return PPM_OK;
+}
+
+// ---- NEXT-4: brick decomposition -----------------------------------------------------
+extern "C" size_t ppm_halo_floats(int nx, int ny, int nz, int axis) {
+    if (nx < 1 || ny < 1 || nz < 1 || axis < 0 || axis > 2) return 0;
+    const size_t nb[3] = {(size_t)(nx + 3) / 4, (size_t)(ny + 3) / 4, (size_t)(nz + 3) / 4};
+    return (size_t)PPM_BRICK_FLOATS * nb[(axis + 1) % 3] * nb[(axis + 2) % 3];
+}
+
+static int halo_args(ppm_ctx* c, int axis, int side, const void* p, const char* who) {
+    if (!c) { set_err(nullptr, "%s: ctx is NULL", who); return PPM_EINVAL; }
+    if (axis < 0 || axis > 2 || side < 0 || side > 1 || !p) { set_err(c, "%s: need axis in 0..2, side in 0..1 and a device buffer", who); return PPM_EINVAL; }
+    if (((uintptr_t)p & 15) != 0) { set_err(c, "%s: the buffer must be 16-byte aligned", who); return PPM_EINVAL; }
+    return PPM_OK;
+}
+
+extern "C" int ppm_pack_halo(ppm_ctx* c, int axis, int side, float* dev_dst) {
+    int rc = halo_args(c, axis, side, dev_dst, "ppm_pack_halo");
+    if (rc) return rc;
+    DevGuard guard(c);
+    CU(ppm_launch_pack_halo(c, axis, side, dev_dst));
+    return PPM_OK;
+}
+
+extern "C" int ppm_set_halo(ppm_ctx* c, int axis, int side, const float* dev_layer) {
+    int rc = halo_args(c, axis, side, dev_layer, "ppm_set_halo");
+    if (rc) return rc;
+    if (c->prm.bc[2 * axis + side] != PPM_BC_HALO) { set_err(c, "ppm_set_halo: face %d of axis %d is not PPM_BC_HALO", side, axis); return PPM_EINVAL; }
+    c->halo[axis][side] = dev_layer;
+    return PPM_OK;
+}
+
+extern "C" int ppm_set_origin(ppm_ctx* c, const int org[3]) {
+    if (!c) { set_err(nullptr, "ppm_set_origin: ctx is NULL"); return PPM_EINVAL; }
+    if (!org || org[0] < 0 || org[1] < 0 || org[2] < 0) { set_err(c, "ppm_set_origin: need three non-negative cell indices"); return PPM_EINVAL; }
+    if (c->prm.grav.kind == PPM_GRAV_CONST_Z && org[2] != 0) { set_err(c, "ppm_set_origin: a grid with plane-parallel (CONST_Z) gravity cannot be cut along z"); return PPM_EINVAL; }
+    if (c->sphere) { set_err(c, "ppm_set_origin: not together with the confining sphere"); return PPM_EINVAL; }
+    for (int d = 0; d < 3; ++d) c->org[d] = org[d];
     c->cfl_valid = 0;
     return PPM_OK;
 }

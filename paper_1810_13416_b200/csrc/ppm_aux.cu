@@ -16,6 +16,7 @@ struct AuxParams {
     const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
     float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
     int sphere;                         // NEXT-3: confining sphere on
+    int ox, oy, oz;                     // ppm_set_origin: global index of cell (0,0,0) (brick decomposition), else 0
     int twof;                           // NEXT-4: two-fluid EOS, beta(f) = beta2 + f dbeta (reading R25)
     double beta2, dbeta;
     float beta2f, dbetaf;
@@ -57,7 +58,7 @@ __device__ __forceinline__ void base64(const AuxParams& A, int i, int j, int k, 
         const double* t = A.tab64 + 3 * (2 * k + 2 * PPM_NGHOST + 1);
         r0 = t[1]; p0 = t[2];
     } else if (A.grav_kind == PPM_GRAV_RADIAL) {
-        const double x = (i + 0.5) * A.dx - A.cx, y = (j + 0.5) * A.dx - A.cy, z = (k + 0.5) * A.dx - A.cz;
+        const double x = (i + A.ox + 0.5) * A.dx - A.cx, y = (j + A.oy + 0.5) * A.dx - A.cy, z = (k + A.oz + 0.5) * A.dx - A.cz;
         const double r = sqrt(x * x + y * y + z * z);
         double t = (r - A.s0) / A.ds;
         int kk = (int)floor(t);
@@ -117,7 +118,7 @@ __device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k
     }
     if (A.grav_kind == PPM_GRAV_RADIAL) {
         const float dx = A.dxf;
-        const float x = ((float)i + 0.5f) * dx - A.cxf, y = ((float)j + 0.5f) * dx - A.cyf, z = ((float)k + 0.5f) * dx - A.czf;
+        const float x = ((float)(i + A.ox) + 0.5f) * dx - A.cxf, y = ((float)(j + A.oy) + 0.5f) * dx - A.cyf, z = ((float)(k + A.oz) + 0.5f) * dx - A.czf;
         const float r2 = fmaf(x, x, fmaf(y, y, z * z));
         const float r = r2 * rsqrtf(fmaxf(r2, 1e-30f));
         const float t = (r - A.s0f) * A.inv_dsf;
@@ -343,9 +344,25 @@ __global__ void __launch_bounds__(256) spin_up_kernel(const AuxParams A, float* 
         int i, j, k;
         long long o;
         if (!cell_of(A, t, i, j, k, o) || aux_is_solid(A, i, j, k)) continue;
-        const double x = ((double)i + 0.5) * A.dx - cx, y = ((double)j + 0.5) * A.dx - cy;
+        const double x = ((double)(i + A.ox) + 0.5) * A.dx - cx, y = ((double)(j + A.oy) + 0.5) * A.dx - cy;
         st[o + 64] = (float)((double)st[o + 64] - domega * y);
         st[o + 2 * 64] = (float)((double)st[o + 2 * 64] + domega * x);
+    }
+}
+
+// NEXT-4 (bricks with a halo one briquette thick): one brick layer of the state — the bricks
+// with index kb along `axis` — gathered into a contiguous buffer [bricks along b][bricks along a] of whole brick records (a < b the
+// two other axes), the layout the sweeps read a PPM_BC_HALO ghost brick from.  Pure copy: one float4 per thread and trip.
+__global__ void __launch_bounds__(256) pack_halo_kernel(const float4* __restrict__ st, float4* __restrict__ dst, int nbx, int nby, int nbz, int axis, int kb) {
+    constexpr int R4 = PPM_BRICK_FLOATS / 4;                       // float4 per brick record
+    const int na = (axis == 0) ? nby : nbx, nb = (axis == 2) ? nby : nbz;
+    const long long tot = (long long)na * nb * R4;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+        const int e = (int)(t % R4);
+        const long long br = t / R4;
+        const int a = (int)(br % na), b = (int)(br / na);
+        const int bx = (axis == 0) ? kb : a, by = (axis == 1) ? kb : (axis == 0 ? a : b), bz = (axis == 2) ? kb : b;
+        dst[t] = st[((long long)(bz * nby + by) * nbx + bx) * R4 + e];
     }
 }
 
@@ -382,6 +399,7 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
     A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
     A.pert_io = c->pert_io;
+    A.ox = c->org[0]; A.oy = c->org[1]; A.oz = c->org[2];
     A.twof = c->twof;
     A.beta2 = c->twof ? 1.0 / (c->gam_rest - 1.0) : 0.0;
     A.dbeta = c->twof ? 1.0 / (c->gam_tracked - 1.0) - A.beta2 : 0.0;
@@ -433,6 +451,16 @@ cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega) {
     const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
     const double cx = c->sphere ? c->sph_c[0] : c->prm.grav.center[0], cy = c->sphere ? c->sph_c[1] : c->prm.grav.center[1];
     spin_up_kernel<<<grid_for(n, c->sms * 16), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], domega, cx, cy);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t ppm_launch_pack_halo(ppm_ctx* c, int axis, int side, float* dst) {
+    const int nbd = (axis == 0) ? c->nbx : (axis == 1 ? c->nby : c->nbz);
+    const int na = (axis == 0) ? c->nby : c->nbx, nb = (axis == 2) ? c->nby : c->nbz;
+    const long long tot = (long long)na * nb * (PPM_BRICK_FLOATS / 4);
+    pack_halo_kernel<<<grid_for(tot, c->sms * 8), 256, 0, c->stream>>>(reinterpret_cast<const float4*>(c->buf[c->cur]), reinterpret_cast<float4*>(dst),
+                                                                     c->nbx, c->nby, c->nbz, axis, side ? nbd - 1 : 0);
     c->launches += 1;
     return cudaGetLastError();
 }

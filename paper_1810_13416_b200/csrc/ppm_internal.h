@@ -43,6 +43,12 @@ struct SweepParams {
     const float2* __restrict__ tabg; // {g_k, g_k+1 - g_k}
     int* flag;                      // sticky state flag (bit 0: floor hit, bit 1: NaN)
     unsigned int* cflmax;           // non-NULL: fold max_d |u_d| + c of every finished cell into it (bit pattern of a float >= 0)
+    // brick decomposition (NEXT-4): global index of cell 0 along the (sweep, a, b) axes, and the brick layers received
+    // from the two neighbours along the sweep axis (PPM_BC_HALO faces): [bricks along b][bricks along a] records, strides HBa, HBb
+    int org_d, org_a, org_b;
+    const float* halo_lo;
+    const float* halo_hi;
+    long long HBa, HBb;
     // two-fluid EOS (NEXT-4, reading R25): beta(f) = beta2 + f dbeta, beta2 = 1/(gamma_rest - 1), dbeta = 1/(gamma_tracked - 1) - beta2
     int twof;
     float beta2, dbeta;
@@ -74,6 +80,8 @@ struct ppm_ctx {
     int flat3d;                     // PPM_OPT_FLATTEN3D
     int sphere;                     // ppm_set_sphere: confining sphere on (NEXT-3)
     double sph_r, sph_c[3];         // its radius and centre
+    int org[3];                     // ppm_set_origin: global index of cell (0,0,0) (a sub-domain of a brick decomposition; else 0)
+    const float* halo[3][2];        // ppm_set_halo: per axis, low / high side: the neighbour's brick layer (borrowed device memory)
     int twof;                       // ppm_set_two_fluid: two-fluid equation of state on (NEXT-4)
     double gam_tracked, gam_rest;   // adiabatic index of the tracked fluid (FV) and of the rest
     float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
@@ -97,3 +105,4 @@ cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
 cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);
 cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega);
+cudaError_t ppm_launch_pack_halo(ppm_ctx* c, int axis, int side, float* dst);

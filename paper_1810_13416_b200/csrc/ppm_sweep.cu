@@ -171,6 +171,7 @@ __device__ __forceinline__ int image_face(int f, int n, int bc_lo, int bc_hi) {
     if ((unsigned)f < (unsigned)n) return f;
     if (f == n) return (bc_hi == PPM_BC_PERIODIC) ? 0 : f;
     const int bcx = (f < 0) ? bc_lo : bc_hi;
+    if (bcx == PPM_BC_HALO) return f;                                 // a neighbour's cells: the face is where it is
     if (bcx == PPM_BC_PERIODIC) {
         f += (f < 0) ? n : -n;
         if ((unsigned)f >= (unsigned)n) f = ((f % n) + n) % n;
@@ -217,7 +218,9 @@ template <int DIR, int GRAV> struct Geo {
     __device__ __forceinline__ void init(const SweepParams& P, int a, int b) {
         t2 = 0.f; cst.rp = bc(0.f); cst.g = 0.f;
         if (GRAV == PPM_GRAV_RADIAL) {
-            float xa = ((float)a + 0.5f) * P.dx - P.cen_a, xb = ((float)b + 0.5f) * P.dx - P.cen_b;
+            // (org: global index of the grid's cell 0 — a sub-domain of a brick decomposition evaluates the base state at the
+            //  same global positions, with the same arithmetic, as the undivided grid; 0 otherwise)
+            float xa = ((float)(a + P.org_a) + 0.5f) * P.dx - P.cen_a, xb = ((float)(b + P.org_b) + 0.5f) * P.dx - P.cen_b;
             t2 = xa * xa + xb * xb;
         } else if (GRAV == PPM_GRAV_CONST_Z && DIR != 2) {
             float4 v = __ldg(P.tab + 2 * b + 2 * PPM_NGHOST + 1);   // b is the z index for x- and y-sweeps
@@ -231,7 +234,7 @@ template <int DIR, int GRAV> struct Geo {
             if (DIR == 2) { float4 v = __ldg(P.tab + 2 * j + 2 * PPM_NGHOST + 1); o.g = sgn * v.z; o.rp = mk(v.x, v.y); }
             else o = cst;
         } else if (GRAV == PPM_GRAV_RADIAL) {
-            float xd = ((float)j + 0.5f) * P.dx - P.cen_d;
+            float xd = ((float)(j + P.org_d) + 0.5f) * P.dx - P.cen_d;
             float r2 = fmaf(xd, xd, t2);
             float ir = rsqrtf(fmaxf(r2, 1e-30f));
             o = table_at(P, r2 * ir);
@@ -246,7 +249,7 @@ template <int DIR, int GRAV> struct Geo {
             if (DIR == 2) { float4 v = __ldg(P.tab + 2 * f + 2 * PPM_NGHOST); o = mk(v.x, v.y); }
             else o = cst.rp;
         } else if (GRAV == PPM_GRAV_RADIAL) {
-            float xd = (float)f * P.dx - P.cen_d;
+            float xd = (float)(f + P.org_d) * P.dx - P.cen_d;
             float r2 = fmaf(xd, xd, t2);
             o = table_rp(P, fsqrt(r2));
         }
@@ -1113,6 +1116,7 @@ struct IoBulk {
     uint64_t* const bar;         // [0..NH) hydro slots, [NH..NH+NP) PPB slots
     const int lane;
     const long long gcol;        // float offset of the warp's first brick column (brick 0 along the sweep axis)
+    const long long hcol;        // the same column inside a halo layer (PPM_BC_HALO: one brick layer of a neighbouring sub-domain)
     const int ncol;              // brick columns of this warp that exist (1 or 2)
     const int k0, kend;          // first / last brick index along the sweep axis this pencil segment touches (ghosts included)
     // per-brick state, refreshed when a new brick comes up (once per 4 iterations); everything is warp-uniform
@@ -1123,11 +1127,12 @@ struct IoBulk {
     int hrev, prev;              // 3 if the brick being read is a mirror image (cells taken in reverse, odd fields negated), else 0
     int jb;                      // image index of the hydro brick's cell 0
 
-    __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, unsigned ph_, int lane_, long long gcol_, int ncol_, int c0, int c1)
+    __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, unsigned ph_, int lane_, long long gcol_, int ncol_, int c0, int c1,
+                                      long long hcol_ = 0)
         : P(P_),
           hyd(wsm + (lane_ >> 4) * (G::HB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
           ppr(wsm + G::NH * G::HSLOT + (lane_ >> 4) * (G::PB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
-          hyd0(wsm), ppr0(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_), gcol(gcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4),
+          hyd0(wsm), ppr0(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_), gcol(gcol_), hcol(hcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4),
           ph(ph_), hs(0), ps(0), hcur(0), hprv(0), pcur(0), pst(0), hrev(0), prev(0), jb(0) {
         if (lane == 0) {
 #pragma unroll
@@ -1141,23 +1146,31 @@ struct IoBulk {
         rev = 0;
         const int nk = P.nbrick_d;
         if ((unsigned)k < (unsigned)nk) return k;
-        if (k < 0) { if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = 3; return 0; }
+        if (k < 0) { if (P.bc_lo == PPM_BC_HALO) return k; if (P.bc_lo == PPM_BC_PERIODIC) return nk - 1; rev = 3; return 0; }
+        if (P.bc_hi == PPM_BC_HALO) return k;                  // (a halo brick keeps its own index: its cells sit where they are)
         if (P.bc_hi == PPM_BC_PERIODIC) return 0;
         rev = 3; return nk - 1;
     }
-    __device__ __forceinline__ void issue_hydro(int k, int slot) {       // lane 0 only
+    // record of chunk k in the warp's first brick column, and the stride to its second column: the state buffer, or — for the
+    // one ghost chunk beyond a PPM_BC_HALO face — the halo layer received from the neighbouring sub-domain
+    __device__ __forceinline__ const float* brick_src(int k, long long& stride2) const {
+        if (k < 0 && P.bc_lo == PPM_BC_HALO) { stride2 = P.HBa; return P.halo_lo + hcol; }
+        if (k >= P.nbrick_d && P.bc_hi == PPM_BC_HALO) { stride2 = P.HBa; return P.halo_hi + hcol; }
         int rev; const int bd = chunk_brick(k, rev);
-        const float* src = P.in + gcol + (long long)bd * P.SBd;
+        stride2 = P.SBa;
+        return P.in + gcol + (long long)bd * P.SBd;
+    }
+    __device__ __forceinline__ void issue_hydro(int k, int slot) {       // lane 0 only
+        long long st2; const float* src = brick_src(k, st2);
         mbar_expect_tx(bar + slot, ncol * G::HB * 4);
         bulk_g2s(hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
-        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + P.SBa, G::HB * 4, bar + slot);
+        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + st2, G::HB * 4, bar + slot);
     }
     __device__ __forceinline__ void issue_ppb(int k, int slot) {         // lane 0 only
-        int rev; const int bd = chunk_brick(k, rev);
-        const float* src = P.in + gcol + (long long)bd * P.SBd + G::HB;
+        long long st2; const float* src = brick_src(k, st2) + G::HB;
         mbar_expect_tx(bar + G::NH + slot, ncol * G::PB * 4);
         bulk_g2s(ppr0 + slot * G::PSLOT, src, G::PB * 4, bar + G::NH + slot);
-        if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + P.SBa, G::PB * 4, bar + G::NH + slot);
+        if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + st2, G::PB * 4, bar + G::NH + slot);
     }
     __device__ __forceinline__ void wait_slot(int j) {        // whole warp
         mbar_wait(bar + j, (ph >> j) & 1);
@@ -1415,7 +1428,8 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
         ph0 = bulk_copy_through<DIR>(P, wsm, wbar, lane, gcol, min(2, nba - ba0), c0, c0w, 0u);
         c0 = c0w; c1 = c1w;
     }
-    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), ph0, lane, gcol, min(2, nba - ba0), c0, c1);
+    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), ph0, lane, gcol, min(2, nba - ba0), c0, c1,
+                   (long long)ba0 * P.HBa + (long long)bb * P.HBb);
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
     const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
@@ -1610,6 +1624,9 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
     P.cen_d = (float)p.grav.center[axis]; P.cen_a = (float)p.grav.center[ia]; P.cen_b = (float)p.grav.center[ib];
     P.tab = c->tab; P.tabp = c->tabp; P.tabg = c->tabg;
     P.flag = c->flag;
+    P.org_d = c->org[axis]; P.org_a = c->org[ia]; P.org_b = c->org[ib];
+    P.halo_lo = c->halo[axis][0]; P.halo_hi = c->halo[axis][1];
+    P.HBa = PPM_BRICK_FLOATS; P.HBb = (long long)PPM_BRICK_FLOATS * ((ext[ia] + 3) / 4);    // a halo layer: [bricks along b][bricks along a] records
     P.twof = c->twof;
     P.beta2 = (float)(1.0 / (c->twof ? c->gam_rest - 1.0 : p.gamma - 1.0));
     P.dbeta = (float)(c->twof ? 1.0 / (c->gam_tracked - 1.0) - 1.0 / (c->gam_rest - 1.0) : 0.0);

@@ -820,6 +820,65 @@ def test_two_fluid_argument_checks():
     g.close()
 
 
+# ---------------------------------------------------------------- NEXT-4: brick decomposition -------------
+@pytest.mark.parametrize("cfg,n,procs,steps", [(4, 64, (2, 2, 2), 6), (1, 32, (2, 1, 2), 6), (2, 64, (2, 2, 1), 6), (4, 64, (1, 4, 1), 3)])
+def test_brick_decomposition_equals_the_undivided_grid_bitwise(cfg, n, procs, steps):
+    """the grid cut into sub-domains with PPM_BC_HALO faces, one brick layer exchanged
+    with the two face neighbours before every sweep (all sub-domains in this process on this GPU, device copies for the
+    messages) gives the SAME BITS as the undivided grid: radial gravity with walls (2x2x2 = the 8-GPU layout, and 4 slabs),
+    the periodic cube (wrap-around neighbours, both neighbours the same sub-domain), plane-parallel gravity cut across x, y"""
+    PPM = _gpu()
+    from paper_1810_13416_b200.decomposition import BrickDecomposition, LocalCluster
+    w = W.make(cfg, n=n)
+    f = w.fields()
+    mono = PPM.from_workload(w)
+    mono.set_state(f.cuda())
+    d = BrickDecomposition((n, n, n), procs, w.bc)
+    cl = LocalCluster(d, w.dx, w.gamma, w.grav, w.rho_floor, w.p_floor)
+    cl.set_state(f)
+    assert torch.equal(cl.get_state(), mono.get_state())
+    for s in range(steps):
+        dt = mono.cfl_dt(w.cfl)
+        assert cl.cfl_dt(w.cfl) == dt                       # the fused / standalone maxima of the parts bracket the same cells
+        order = (0, 5, 2, 3)[s % 4]
+        mono.step(dt, order)
+        cl.step(dt, order)
+    a, b = mono.get_state(), cl.get_state()
+    assert torch.equal(a, b), float((a - b).abs().max())
+    ca, cb = mono.reduce_conserved(), cl.reduce_conserved()
+    assert np.allclose(ca, cb, rtol=1e-12, atol=1e-14 * np.abs(ca).max())
+    # what travelled: per step, every cut axis sends 2 layers per interior face pair; nothing else
+    sent = sum(p.halo_bytes for p in cl.parts)
+    faces = sum(1 for r in range(d.size) for ax in range(3) for sd in (0, 1) if d.neighbour(r, ax, sd) is not None and True)
+    per_step = sum(d.halo_cells(ax) * 15 * 4 for r in range(d.size) for ax in range(3) for sd in (0, 1) if d.neighbour(r, ax, sd) is not None)
+    assert sent == steps * per_step and faces > 0
+    mono.close()
+    cl.close()
+
+
+def test_brick_decomposition_argument_checks():
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import BC_HALO, OPT_FLATTEN3D, PPMError
+    g = PPM(32, 32, 32, 1.0 / 32, 5.0 / 3.0, (1, BC_HALO, 1, 1, 1, 1))
+    g.set_state(torch.ones((15, 32, 32, 32), dtype=torch.float32).cuda())
+    with pytest.raises(PPMError):
+        g.step(1e-3, 0)                                     # an exchange is due between the sweeps
+    with pytest.raises(PPMError):
+        g.sweep(1e-3, 0)                                    # no halo layer handed over yet
+    g.sweep(1e-3, 1)                                        # axes without a HALO face sweep as ever
+    lay = torch.empty(g.halo_floats(0), dtype=torch.float32, device="cuda")
+    assert g.halo_floats(0) == 15 * 64 * 8 * 8
+    with pytest.raises(PPMError):
+        g.set_halo(0, 0, lay)                               # that face is a wall
+    g.pack_halo(0, 0, lay)
+    g.set_halo(0, 1, lay)
+    g.sweep(1e-3, 0)
+    g.sync()
+    with pytest.raises(PPMError):
+        PPM(30, 32, 32, 1.0 / 32, 5.0 / 3.0, (1, BC_HALO, 1, 1, 1, 1))      # not whole bricks along a HALO axis
+    g.close()
+
+
 # ---------------------------------------------------------------- full-size configs on windows --------
 def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sphere=None):
     PPM = _gpu()
