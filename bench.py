@@ -121,6 +121,12 @@ class _Clocks:
         return out
 
 
+def _geometry(w):
+    walls = "periodic" if all(b == 0 for b in w.bc) else ("reflecting walls" if all(b == 1 for b in w.bc) else "periodic x,y + reflecting z walls")
+    grav = {None: "no gravity", 1: "plane-parallel gravity", 2: "radial gravity"}[None if not w.grav else int(w.grav["kind"])]
+    return walls + " + " + grav
+
+
 def _load_state(g, w, nzs):
     n = w.n
     for z0 in range(0, n, nzs):
@@ -356,7 +362,7 @@ def run_gpu(args):
         "metric": METRIC, "value": aggregate_value(ncell, K, ms, ws), "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": r["warmup"],
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "%s %d^3, %s, dt fixed at 0.7*CFL dt, sweep order xyz/zyx alternating" % (w.name, n, "reflecting walls + radial gravity" if w.grav else "periodic"),
+        "config": {"workload": "%s %d^3, %s, dt fixed at 0.7*CFL dt, sweep order xyz/zyx alternating" % (w.name, n, _geometry(w)),
                    "cells_per_gpu": ncell, "l2": "inputs (%.1f GB state) larger than the 126 MB L2" % (15 * ncell * 4 / 1e9),
                    "parallelism": "replicas only (1 grid per GPU)", "chunk": args.chunk,
                    "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)",
@@ -401,6 +407,86 @@ def run_gpu(args):
     return 0
 
 
+def run_decomposed(args):
+    """--decompose px,py,pz: ONE global grid (the workload) cut into px*py*pz sub-domains, a brick layer
+    exchanged with the face neighbours before every sweep.  Under torchrun with px*py*pz ranks: one sub-domain per GPU, NCCL
+    send/recv over NVLink ("strong" scaling: the total work is fixed).  In a single process: all sub-domains on this GPU
+    (LocalCluster, device copies) — what the decomposition itself costs (packing, copies, shorter pencils), measured where only
+    one GPU is to be had."""
+    from paper_1810_13416_b200.decomposition import BrickDecomposition, DecomposedPPM, LocalCluster
+    ws, rank, lr = _dist()
+    procs = tuple(int(v) for v in args.decompose.split(","))
+    torch.cuda.set_device(lr)
+    dev = torch.device("cuda", lr)
+    w = W.make(args.workload)
+    n = w.n
+    d = BrickDecomposition((n, n, n), procs, w.bc)
+    if ws > 1:
+        import torch.distributed as dist
+        assert ws == d.size, "--decompose %s needs %d ranks" % (args.decompose, d.size)
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if ws > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    if ws > 1:
+        g = DecomposedPPM(d, rank, w.dx, w.gamma, w.grav, w.rho_floor, w.p_floor, dev)
+        parts = [g]
+    else:
+        g = LocalCluster(d, w.dx, w.gamma, w.grav, w.rho_floor, w.p_floor, dev)
+        parts = g.parts
+    for p in parts:                                   # every sub-domain generates its own box of the synthetic input
+        o, ln = p.org, d.local_n()
+        for z0 in range(0, ln[2], 32):
+            z1 = min(ln[2], z0 + 32)
+            p.ppm.set_state(w.fields((o[0], o[1], o[2] + z0), (o[0] + ln[0], o[1] + ln[1], o[2] + z1), device=dev), z0=z0)
+    dt = 0.7 * g.cfl_dt(w.cfl)
+    K, Wm = args.steps, max(args.warmup, 3)
+    for s in range(Wm):
+        g.step(dt, 0 if s % 2 == 0 else 5)
+    barrier()
+    clk = _Clocks(lr)
+    reps = args.reps if args.reps else 5
+    ms_reps = []
+    b0 = sum(p.halo_bytes for p in parts)
+    for r in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(parts[0].ppm.stream)
+        for s in range(K):
+            g.step(dt, 0 if s % 2 == 0 else 5)
+        e1.record(parts[0].ppm.stream)
+        barrier()
+        ms_reps.append(e0.elapsed_time(e1))
+    halo = (sum(p.halo_bytes for p in parts) - b0) / (reps * K)
+    clocks = clk.stop()
+    for p in parts:
+        p.ppm.sync()
+    ms = float(np.median(ms_reps))
+    vals = max_over_ranks([ms, halo], ws, dev) if ws > 1 else [ms, halo]
+    if rank == 0:
+        peak, peak_kind = _peaks()
+        line = {"metric": METRIC, "value": n ** 3 * K / (vals[0] * 1e-3), "unit": UNIT, "n_gpus": ws, "steps": K, "warmup": Wm,
+                "ms_per_step": vals[0] / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "%s %d^3 as ONE grid cut into %s sub-domains of %s cells" % (w.name, n, "x".join(map(str, procs)), "x".join(map(str, d.local_n()))),
+                           "parallelism": ("brick decomposition, one sub-domain per GPU, NCCL send/recv of one brick layer per face before each sweep" if ws > 1 else
+                                           "brick decomposition, all %d sub-domains on ONE GPU (device copies for the messages)" % d.size),
+                           "halo_bytes_per_step_per_rank_max": vals[1],
+                           "timing": "median of %d repetitions of the %d-step region (CUDA events)" % (reps, K)},
+                "repetitions_ms_per_step": [x / K for x in ms_reps], "clocks": clocks,
+                "roofline": {"bound": "hbm", "achieved": BYTES_PER_CELL_SWEEP * n ** 3 * 3 * K / (vals[0] * 1e-3) / 1e9 / ws, "peak": peak, "unit": "GB/s",
+                             "frac": BYTES_PER_CELL_SWEEP * n ** 3 * 3 * K / (vals[0] * 1e-3) / 1e9 / ws / peak, "traffic": None, "peak_kind": "of " + peak_kind,
+                             "note": "per GPU: sweeps + packing + exchange"},
+                "gpu_launches": int(sum(p.ppm.launch_count() for p in parts))}
+        print(json.dumps(line))
+    g.close()
+    if ws > 1:
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -414,6 +500,7 @@ def main():
     ap.add_argument("--flatten3d", action="store_true", help="fully 3-D shock-flattening mode (SURVEY 8(f) NEXT-1): one more light kernel per step")
     ap.add_argument("--sphere", action="store_true", help="the paper's run geometry (SURVEY 8(f) NEXT-3): confining sphere inscribed in the cube")
     ap.add_argument("--two-fluid", action="store_true", help="two-fluid equation of state (SURVEY 8(f) NEXT-4): the tracked fluid has gamma = 1.4")
+    ap.add_argument("--decompose", default="", help="px,py,pz: the workload as ONE grid cut into sub-domains with halo exchange (SURVEY 8(f) NEXT-4); under torchrun with px*py*pz ranks one sub-domain per GPU, else all on this GPU")
     ap.add_argument("--direct", action="store_true", help="direct global-memory sweep path instead of the bulk-staged one")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--ref-side", type=int, default=128, help="side of the oracle's sample window (--impl reference)")
@@ -423,6 +510,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.decompose:
+        return run_decomposed(args)
     return run_gpu(args)
 
 

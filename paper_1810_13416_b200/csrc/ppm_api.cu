@@ -147,7 +147,7 @@ extern "C" void ppm_destroy(ppm_ctx* c) {
     if (!c) return;
     DevGuard guard(c);
     cudaFree(c->flag); cudaFree(c->cflmax); cudaFree(c->partial); cudaFree(c->result);
-    cudaFree(c->tab); cudaFree(c->tabp); cudaFree(c->tabg); cudaFree(c->tab64); cudaFree(c->F3);
+    cudaFree(c->tab); cudaFree(c->tabp); cudaFree(c->tabg); cudaFree(c->tab64); cudaFree(c->F3); cudaFree(c->R0c); cudaFree(c->P0c);
     free(c);
 }
 
@@ -315,6 +315,14 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
             const size_t n = (size_t)c->nbx * c->nby * c->nbz * 64;
             cudaError_t e = cudaMalloc(&c->F3, n * sizeof(float));
             if (e != cudaSuccess) { c->F3 = nullptr; cudaGetLastError(); set_err(c, "ppm_set_option: cannot allocate the %zu-byte detector field", n * sizeof(float)); return PPM_ENOMEM; }
+        }
+        if (value && c->prm.grav.kind == PPM_GRAV_RADIAL && !c->P0c) {
+            // the detector kernel stages 2.5 points per cell: with a radial profile their base state comes from two per-cell
+            // arrays (8 more bytes per cell, filled once) instead of a table lookup each
+            const size_t n = (size_t)c->nbx * c->nby * c->nbz * 64;
+            if (cudaMalloc(&c->R0c, n * sizeof(float)) != cudaSuccess || cudaMalloc(&c->P0c, n * sizeof(float)) != cudaSuccess) {
+                cudaGetLastError(); cudaFree(c->R0c); c->R0c = c->P0c = nullptr;      // fall back to the lookups
+            } else CU(ppm_launch_base_fill(c));
         }
         c->flat3d = value;
         return PPM_OK;

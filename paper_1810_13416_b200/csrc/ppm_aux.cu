@@ -16,6 +16,8 @@ struct AuxParams {
     const float4* __restrict__ tab32;   // node k: {rho0, p0, g, 0} (the sweeps' fp32 table)
     float dxf, cxf, cyf, czf, s0f, inv_dsf, gamf;   // fp32 copies for the fp32 kernels (no fp64 conversions in their loops)
     int sphere;                         // NEXT-3: confining sphere on
+    const float* __restrict__ R0c;      // 3-D flattening mode with RADIAL gravity: rho0, p0 at every cell centre as the sweeps evaluate them
+    const float* __restrict__ P0c;      // ([brick][4z][4y][4x], filled once when the option is set), else NULL
     int ox, oy, oz;                     // ppm_set_origin: global index of cell (0,0,0) (brick decomposition), else 0
     int twof;                           // NEXT-4: two-fluid EOS, beta(f) = beta2 + f dbeta (reading R25)
     double beta2, dbeta;
@@ -270,8 +272,11 @@ __device__ __forceinline__ void f3_point(const AuxParams& A, const float* __rest
         if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
         if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
     }
-    const long long o = cell_offset(A, gx, gy, gz);
-    const float2 b0 = base32(A, gx, gy, gz);
+    // brick index and cell in brick -> float offset of field 0 in the state, slot in a one-field array
+    const int br = ((gz >> 2) * A.nby + (gy >> 2)) * A.nbx + (gx >> 2), cb = (gz & 3) << 4 | (gy & 3) << 2 | (gx & 3);
+    const long long o = (long long)br * PPM_BRICK_FLOATS + cb;
+    // base state: from the per-cell arrays where they exist (RADIAL: spares a table lookup per staged point), else evaluated
+    const float2 b0 = A.P0c ? make_float2(d < 0 ? __ldg(A.R0c + br * 64LL + cb) : 0.f, __ldg(A.P0c + br * 64LL + cb)) : base32(A, gx, gy, gz);
     sP[si] = b0.y + st[o + 4 * 64];
     if (d < 0) {
         rc = b0.x + st[o];
@@ -337,6 +342,17 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
     F3[brick * 64 + c] = F;
 }
 
+// rho0, p0 of every storage slot (pad cells included: harmless values), fp32 exactly as base32 gives them
+__global__ void __launch_bounds__(256) base_fill_kernel(const AuxParams A, float* __restrict__ R0c, float* __restrict__ P0c) {
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < A.nslots; t += (long long)gridDim.x * blockDim.x) {
+        int i, j, k;
+        long long o;
+        cell_of(A, t, i, j, k, o);
+        const float2 b = base32(A, i, j, k);
+        R0c[t] = b.x; P0c[t] = b.y;
+    }
+}
+
 // NEXT-3 ("adding a solid body rotational flow component ... gradually over the first several thousand
 // time steps"; reading R24): one increment of the ramp, du = domega e_z x (X - centre) on every fluid cell.
 __global__ void __launch_bounds__(256) spin_up_kernel(const AuxParams A, float* __restrict__ st, double domega, double cx, double cy) {
@@ -399,6 +415,7 @@ AuxParams make_aux(const ppm_ctx* c) {
     A.dxf = (float)A.dx; A.cxf = (float)A.cx; A.cyf = (float)A.cy; A.czf = (float)A.cz;
     A.s0f = (float)A.s0; A.inv_dsf = (float)(A.grav_kind != PPM_GRAV_NONE ? 1.0 / A.ds : 0.0); A.gamf = (float)A.gamma;
     A.pert_io = c->pert_io;
+    A.R0c = c->R0c; A.P0c = c->P0c;
     A.ox = c->org[0]; A.oy = c->org[1]; A.oz = c->org[2];
     A.twof = c->twof;
     A.beta2 = c->twof ? 1.0 / (c->gam_rest - 1.0) : 0.0;
@@ -434,6 +451,14 @@ cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c) {
     const dim3 grid((c->nbx + 1) / 2, (c->nby + 1) / 2, (c->nbz + 1) / 2);
     flatten3d_kernel<<<grid, 512, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->F3);
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
+cudaError_t ppm_launch_base_fill(ppm_ctx* c) {
+    AuxParams A = make_aux(c);
+    A.R0c = A.P0c = nullptr;
+    base_fill_kernel<<<grid_for(A.nslots, c->sms * 16), 256, 0, c->stream>>>(A, c->R0c, c->P0c);
     c->launches += 1;
     return cudaGetLastError();
 }

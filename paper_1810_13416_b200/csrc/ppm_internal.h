@@ -84,6 +84,8 @@ struct ppm_ctx {
     const float* halo[3][2];        // ppm_set_halo: per axis, low / high side: the neighbour's brick layer (borrowed device memory)
     int twof;                       // ppm_set_two_fluid: two-fluid equation of state on (NEXT-4)
     double gam_tracked, gam_rest;   // adiabatic index of the tracked fluid (FV) and of the rest
+    float* R0c;                     // device: rho0 / p0 at every cell centre (3-D flattening mode with RADIAL gravity; library-owned), else NULL
+    float* P0c;
     float* F3;                      // device: 3-D shock detector field (library-owned, allocated when the option is set)
     int sms;                        // multiprocessors of the device
     int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state
@@ -102,6 +104,7 @@ cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, floa
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs);
 cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
+cudaError_t ppm_launch_base_fill(ppm_ctx* c);    // fills R0c, P0c
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
 cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);
 cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega);

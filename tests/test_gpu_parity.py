@@ -89,6 +89,10 @@ def _run_pair(w, steps, chunk=0, check_each=(), flat3d=False, direct=False, twof
     g.set_option(OPT_STATE_FORM, 0)
     out["pert"] = pert_rel((gp[0], gp[4]), (o.raw_field(0), o.raw_field(4)))
     print("perturbation-form parity after %d steps (%s %d^3): %s" % (steps, w.name, w.n, {k: float("%.3g" % v) for k, v in out["pert"].items()}))
+    fmt = lambda e: {k: float("%.2e" % v) for k, v in e.items()}
+    print("parity %s %d^3%s: max-rel after 1 step %s; after %d steps max-rel %s, L1 %s; conserved totals %.1e" % (
+        w.name, w.n, " (two-fluid)" if twofluid else (" (3-D flattening)" if flat3d else ""), fmt(out[1][0]), steps, fmt(out[steps][0]),
+        fmt(out[steps][1]), float(out["cons1"].max())))
     out["drift_gpu"] = np.abs(g.reduce_conserved() - c0g)
     out["c0"] = c0g
     out["final"] = (gs, os_)
@@ -932,6 +936,7 @@ def _window_check(cfg, steps, windows, nzs_load=16, tol=ONE_STEP, norm="max", sp
         e = max_rel(gs, os_, scale) if norm == "max" else l1_rel(gs, os_)
         for k, v in e.items():
             worst[k] = max(worst.get(k, 0.0), v)
+    print("parity cfg %d at full size (%d^3), %d windows, %d steps, %s norm: %s" % (cfg, n, len(windows), steps, norm, {k: float("%.2e" % v) for k, v in worst.items()}))
     assert max(worst.values()) <= tol, worst
     if perts:
         # scale = the largest perturbation over all windows (a window in the quiescent core has none of its own)
