@@ -324,22 +324,30 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
     const int b = tid >> 6, c = tid & 63;
     const int lx = (b & 1) * 4 + (c & 3), ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3), lz = (b >> 2) * 4 + (c >> 4);
     const int g[3] = {org[0] + lx, org[1] + ly, org[2] + lz};
-    if (g[0] >= A.nx || g[1] >= A.ny || g[2] >= A.nz) return;
+    const bool valid = g[0] < A.nx && g[1] < A.ny && g[2] < A.nz;          // (a tile may overhang a ragged grid)
     const int s0 = f3_idx(lx, ly, lz);
-    const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
     float F = 0.f;
     const int stride[3] = {1, F3_W, F3_W * F3_W};
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const int sd = stride[d];
-        const float d1 = sP[s0 + sd] - sP[s0 - sd], d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
-        const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
-        const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), fminf(sP[s0 + sd], sP[s0 - sd])) - 1.0f);
-        const float conv = __saturatef((sU[d][s0 - sd] - sU[d][s0 + sd]) * ics);
-        F = fmaxf(F, steep * jump * conv);
+        const float pp = sP[s0 + sd], pm = sP[s0 - sd];
+        const float d1 = pp - pm, pmin = fminf(pp, pm);
+        // the jump ramp clamp(3|d1|/min(p) - 1) is zero unless the pressure changes by a third over two cells: when no cell of
+        // the warp is that near a shock along d the coefficient is the same zero without the three divisions
+        if (__any_sync(0xffffffffu, valid && 3.0f * fabsf(d1) > pmin)) {
+            const float d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
+            const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
+            const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
+            const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), pmin) - 1.0f);
+            const float conv = __saturatef((sU[d][s0 - sd] - sU[d][s0 + sd]) * ics);
+            F = fmaxf(F, steep * jump * conv);
+        }
     }
-    const long long brick = ((long long)(g[2] >> 2) * A.nby + (g[1] >> 2)) * A.nbx + (g[0] >> 2);
-    F3[brick * 64 + c] = F;
+    if (valid) {
+        const long long brick = ((long long)(g[2] >> 2) * A.nby + (g[1] >> 2)) * A.nbx + (g[0] >> 2);
+        F3[brick * 64 + c] = F;
+    }
 }
 
 // rho0, p0 of every storage slot (pad cells included: harmless values), fp32 exactly as base32 gives them

@@ -90,6 +90,12 @@ __device__ constexpr int PPB_PERM[3][10] = {
 __device__ __forceinline__ float sat(float x) { return __saturatef(x); }
 // streaming read that leaves the (small: L1 is carved out as shared memory) L1 to the gravity-table lines
 __device__ __forceinline__ float ld_noalloc(const float* p) { float v; asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v; }
+// the detector field F~ (3-D flattening mode): a brick's 256 bytes are read in four iterations, 64 bytes (z sweep: one row) or 16
+// scattered 4-byte pieces of every sector (x, y sweeps) at a time — with L1 allocation the sectors are fetched once per brick
+#ifndef PPM_FLAT_L1
+#define PPM_FLAT_L1 1
+#endif
+__device__ __forceinline__ float ld_flat(const float* p) { return PPM_FLAT_L1 ? __ldg(p) : ld_noalloc(p); }
 __device__ __forceinline__ float med3(float a, float b, float c) { return fmaxf(fminf(a, b), fminf(fmaxf(a, b), c)); }
 __device__ __forceinline__ float rcp(float x) { return __fdividef(1.0f, x); }
 __device__ __forceinline__ float fdiv(float a, float b) { return __fdividef(a, b); }
@@ -469,7 +475,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
     if (FLAT) {
         float sg;
         const int jf = image_cell(c0 - PPM_NGHOST - 2, P.n, P.bc_lo, P.bc_hi, sg);
-        fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+        fpre = ld_flat(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
     }
     // two-fluid EOS: Gamma of cells n-4, n-3 (the cell n-2 joins them inside the iteration); m000 of cell n-2 in flight
     float Gm4 = gam, Gm3 = gam, mpre = 0.f;
@@ -531,7 +537,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             ftn = fpre;                                              // F~_{n-2}, in flight since the last iteration
             float sg;
             const int jf = (S >= 0) ? n - 1 : image_cell(n - 1, P.n, P.bc_lo, P.bc_hi, sg);     // (the detector is mirror-invariant)
-            fpre = ld_noalloc(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
+            fpre = ld_flat(pflat + (long long)(jf >> 2) * P.FBd + ((jf & 3) << (2 * DIR)));
         } else {
             // The jump ramp clamp(3|d1|/min(p) - 1) is zero wherever the pressure changes by less than a third over two
             // cells: everywhere but in strong shocks.  When no lane of the warp is near one, f~ = 0 without the three
