@@ -67,6 +67,10 @@
 #endif
 // direct path: whole brick records this many bricks ahead along the pencil are pulled into L2 with one bulk
 // prefetch per half warp (0 = off)
+// bulk path: warps per CTA (1, 2, 3, 4, 6 or 12: 12 warps stay resident per SM)
+#ifndef PPM_BULK_WARPS
+#define PPM_BULK_WARPS 4
+#endif
 #ifndef PPM_PREFETCH_BRICKS
 #define PPM_PREFETCH_BRICKS 1
 #endif
@@ -1098,7 +1102,8 @@ template <int DIR> struct BulkGeom {
     static constexpr int HSLOT = 2 * HB + PAD, PSLOT = 2 * PB + PAD;
     static constexpr int NH = 3, NP = 2;                        // ring depths
     static constexpr int WARP_FLOATS = NH * HSLOT + NP * PSLOT;
-    static constexpr int WARPS = 4;
+    static constexpr int WARPS = PPM_BULK_WARPS;                // warps per CTA (build knob; 12 warps are resident per SM)
+    static constexpr int CTAS = 12 / PPM_BULK_WARPS;            // resident CTAs per SM the launch bounds ask for
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * 4 + WARPS * (NH + NP) * sizeof(uint64_t);
 };
 
@@ -1166,18 +1171,19 @@ struct IoBulk {
         stride2 = P.SBa;
         return P.in + gcol + (long long)bd * P.SBd;
     }
-    __device__ __forceinline__ void issue_hydro(int k, int slot) {       // lane 0 only
-        long long st2; const float* src = brick_src(k, st2);
+    // src = the record of the wanted brick in the warp's first column, st2 = stride to its second column
+    __device__ __forceinline__ void issue_hydro_at(const float* src, long long st2, int slot) {       // lane 0 only
         mbar_expect_tx(bar + slot, ncol * G::HB * 4);
         bulk_g2s(hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
         if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + st2, G::HB * 4, bar + slot);
     }
-    __device__ __forceinline__ void issue_ppb(int k, int slot) {         // lane 0 only
-        long long st2; const float* src = brick_src(k, st2) + G::HB;
+    __device__ __forceinline__ void issue_ppb_at(const float* src, long long st2, int slot) {         // lane 0 only
         mbar_expect_tx(bar + G::NH + slot, ncol * G::PB * 4);
-        bulk_g2s(ppr0 + slot * G::PSLOT, src, G::PB * 4, bar + G::NH + slot);
-        if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + st2, G::PB * 4, bar + G::NH + slot);
+        bulk_g2s(ppr0 + slot * G::PSLOT, src + G::HB, G::PB * 4, bar + G::NH + slot);
+        if (ncol > 1) bulk_g2s(ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + G::HB + st2, G::PB * 4, bar + G::NH + slot);
     }
+    __device__ __forceinline__ void issue_hydro(int k, int slot) { long long st2; const float* src = brick_src(k, st2); issue_hydro_at(src, st2, slot); }
+    __device__ __forceinline__ void issue_ppb(int k, int slot) { long long st2; const float* src = brick_src(k, st2); issue_ppb_at(src, st2, slot); }
     __device__ __forceinline__ void wait_slot(int j) {        // whole warp
         mbar_wait(bar + j, (ph >> j) & 1);
         ph ^= 1u << j;
@@ -1226,8 +1232,17 @@ struct IoBulk {
 #endif
                 if (lane == 0) {
                     tma_wait_read0();
-                    if (S >= 0 || (k + 1 >= k0 + G::NH && k + 1 <= kend)) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
-                    if (S >= 0 || (k >= k0 + G::NP && k <= kend)) issue_ppb(k, ps ^ 1);
+                    if (S >= 0) {
+                        // steady state: brick k is an interior brick of the state buffer — no image, no halo layer; only brick
+                        // k + 1 can be the ghost brick beyond the high end
+                        const float* rec = P.in + gcol + (long long)k * P.SBd;
+                        if (k + 1 < P.nbrick_d) issue_hydro_at(rec + P.SBd, P.SBa, hs == G::NH - 1 ? 0 : hs + 1);
+                        else issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
+                        issue_ppb_at(rec, P.SBa, ps ^ 1);
+                    } else {
+                        if (k + 1 >= k0 + G::NH && k + 1 <= kend) issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
+                        if (k >= k0 + G::NP && k <= kend) issue_ppb(k, ps ^ 1);
+                    }
                 }
             }
         } else if (s == 3) {                                   // PPB cell c = n - 3 is the first of brick c >> 2
@@ -1396,7 +1411,7 @@ __device__ __forceinline__ unsigned bulk_copy_through(const SweepParams& P, floa
 }
 
 template <int DIR, int GRAV, bool FLAT, bool CFL, bool SPH, bool TWOF>
-__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_kernel(const SweepParams P) {
+__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS) ppm_sweep_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sm = reinterpret_cast<float*>(smem_raw);
@@ -1462,7 +1477,7 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_sweep_bulk_k
 
 // PPB-only sweep (NEXT-2), bulk-staged path: same rings; the hydro slots travel through unchanged
 template <int DIR>
-__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, 3) ppm_advect_bulk_kernel(const SweepParams P) {
+__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS) ppm_advect_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sm = reinterpret_cast<float*>(smem_raw);
@@ -1648,7 +1663,7 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
     const int nba = (P.na + 3) / 4, nbb = (P.nb + 3) / 4;
     cudaError_t e;
     if (use_bulk) {
-        P.ntiles = ((nba + 7) / 8) * nbb;                                     // CTA tile = 4 warps x 2 brick columns along a
+        P.ntiles = ((nba + 2 * PPM_BULK_WARPS - 1) / (2 * PPM_BULK_WARPS)) * nbb;   // CTA tile = WARPS warps x 2 brick columns along a
         const int uc = c->chunk > 0 ? chunk : 0;                              // 0: whole pencils, the last wave cut to finish together
 #ifndef PPM_EXP_ONE
         if (advect) {
