@@ -49,6 +49,7 @@ struct SweepParams {
     const float* halo_lo;
     const float* halo_hi;
     long long HBa, HBb;
+    unsigned long long k10;         // the packed f32x2 constant (1.0f, 0.0f)
     // two-fluid EOS (NEXT-4, reading R25): beta(f) = beta2 + f dbeta, beta2 = 1/(gamma_rest - 1), dbeta = 1/(gamma_tracked - 1) - beta2
     int twof;
     float beta2, dbeta;

@@ -36,6 +36,7 @@
 // cancel out all large contributions", L35): the Newton iteration runs on p*' = p* - p0f, the update
 // adds increments to rho', p' instead of rebuilding them from E.
 #include <stdlib.h>
+#include <string.h>
 
 #include <type_traits>
 
@@ -70,6 +71,9 @@
 // bulk path: warps per CTA (1, 2, 3, 4, 6 or 12: 12 warps stay resident per SM)
 #ifndef PPM_BULK_WARPS
 #define PPM_BULK_WARPS 4
+#endif
+#ifndef PPM_K10_PARAM
+#define PPM_K10_PARAM 1
 #endif
 #ifndef PPM_PREFETCH_BRICKS
 #define PPM_PREFETCH_BRICKS 1
@@ -606,7 +610,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             const v2 beta = fma2(np(du), bc(rc), dp) * ic2h;
             const v2 al0 = fma2(Ep - Ap, bc(-ic2), Er - Ar);
             // W = (qR, qL) + (-,+) * (...)
-            const v2 K10 = mk(1.0f, 0.0f);
+            const v2 K10 = PPM_K10_PARAM ? up(P.k10) : mk(1.0f, 0.0f);      // (1, 0): as a 64-bit kernel argument it sits in a uniform register pair
             const v2 Br = fma2(bc(dq.A.x), K10, bc(L.A.x)), Bu = fma2(bc(dq.u), K10, bc(L.u)), Bp = fma2(bc(dq.A.y), K10, bc(L.A.y));
             const v2 Bv = fma2(bc(dq.B.x), K10, bc(L.B.x)), Bw = fma2(bc(dq.B.y), K10, bc(L.B.y));
             Wr = Br + np((Ar + beta) + al0);
@@ -1648,6 +1652,7 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
     P.org_d = c->org[axis]; P.org_a = c->org[ia]; P.org_b = c->org[ib];
     P.halo_lo = c->halo[axis][0]; P.halo_hi = c->halo[axis][1];
     P.HBa = PPM_BRICK_FLOATS; P.HBb = (long long)PPM_BRICK_FLOATS * ((ext[ia] + 3) / 4);    // a halo layer: [bricks along b][bricks along a] records
+    { const float one = 1.0f; unsigned int b; memcpy(&b, &one, 4); P.k10 = (unsigned long long)b; }      // the f32x2 constant (1, 0)
     P.twof = c->twof;
     P.beta2 = (float)(1.0 / (c->twof ? c->gam_rest - 1.0 : p.gamma - 1.0));
     P.dbeta = (float)(c->twof ? 1.0 / (c->gam_tracked - 1.0) - 1.0 / (c->gam_rest - 1.0) : 0.0);
