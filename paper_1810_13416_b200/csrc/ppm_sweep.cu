@@ -75,6 +75,10 @@
 #ifndef PPM_K10_PARAM
 #define PPM_K10_PARAM 1
 #endif
+// steady-state body: bulk copies issued by the whole warp under a leader predicate instead of inside `if (lane == 0)` (A/B knob)
+#ifndef PPM_PRED_COPIES
+#define PPM_PRED_COPIES 1
+#endif
 #ifndef PPM_PREFETCH_BRICKS
 #define PPM_PREFETCH_BRICKS 1
 #endif
@@ -1119,6 +1123,28 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes) : "memory");
 }
 
+// The same operations predicated on `lead` inside the asm (lead = lane 0).  The statement is executed by the whole, converged
+// warp with warp-uniform operands, so ptxas issues the bulk copy once under a predicate instead of wrapping it, inside an
+// `if (lane == 0)` region, into a lane-election loop of its own (five more instructions per copy).
+__device__ __forceinline__ void mbar_expect_tx_p(bool lead, uint64_t* bar, uint32_t bytes) {
+    asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %2, 0;\nand.pred q, q, e;\n@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n}\n"
+                 ::"r"(smem_u32(bar)), "r"(bytes), "r"((int)lead) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s_p(bool lead, void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %4, 0;\nand.pred q, q, e;\n@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n}\n"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "r"((int)lead) : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_p(bool lead, void* dst, const void* src, uint32_t bytes) {
+    asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %3, 0;\nand.pred q, q, e;\n@q cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n}\n"
+                 ::"l"(dst), "r"(smem_u32(src)), "r"(bytes), "r"((int)lead) : "memory");
+}
+__device__ __forceinline__ void tma_commit_p(bool lead) {
+    asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %0, 0;\nand.pred q, q, e;\n@q cp.async.bulk.commit_group;\n}\n" ::"r"((int)lead) : "memory");
+}
+__device__ __forceinline__ void tma_wait_read0_p(bool lead) {
+    asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %0, 0;\nand.pred q, q, e;\n@q cp.async.bulk.wait_group.read 0;\n}\n" ::"r"((int)lead) : "memory");
+}
+
 template <int DIR>
 struct IoBulk {
     using G = BulkGeom<DIR>;
@@ -1174,6 +1200,17 @@ struct IoBulk {
         int rev; const int bd = chunk_brick(k, rev);
         stride2 = P.SBa;
         return P.in + gcol + (long long)bd * P.SBd;
+    }
+    // steady state, whole warp: the same two issues with the leader predicate inside the asm
+    __device__ __forceinline__ void issue_hydro_w(bool lead, const float* src, long long st2, int slot) {
+        mbar_expect_tx_p(lead, bar + slot, ncol * G::HB * 4);
+        bulk_g2s_p(lead, hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
+        bulk_g2s_p(lead && ncol > 1, hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + st2, G::HB * 4, bar + slot);
+    }
+    __device__ __forceinline__ void issue_ppb_w(bool lead, const float* src, long long st2, int slot) {
+        mbar_expect_tx_p(lead, bar + G::NH + slot, ncol * G::PB * 4);
+        bulk_g2s_p(lead, ppr0 + slot * G::PSLOT, src + G::HB, G::PB * 4, bar + G::NH + slot);
+        bulk_g2s_p(lead && ncol > 1, ppr0 + slot * G::PSLOT + G::PB + G::PAD, src + G::HB + st2, G::PB * 4, bar + G::NH + slot);
     }
     // src = the record of the wanted brick in the warp's first column, st2 = stride to its second column
     __device__ __forceinline__ void issue_hydro_at(const float* src, long long st2, int slot) {       // lane 0 only
@@ -1234,11 +1271,20 @@ struct IoBulk {
                     __syncwarp();
                 }
 #endif
-                if (lane == 0) {
+                if (S >= 0 && PPM_PRED_COPIES) {
+                    // steady state: brick k is an interior brick of the state buffer — no image, no halo layer; only brick
+                    // k + 1 can be the ghost brick beyond the high end (its record comes from brick_src then)
+                    const bool lead = true;            // (the leader is elected inside the asm; `lead` carries the warp-uniform condition)
+                    tma_wait_read0_p(lead);
+                    const float* rec = P.in + gcol + (long long)k * P.SBd;
+                    long long st2 = P.SBa;
+                    const float* nxt = rec + P.SBd;
+                    if (k + 1 >= P.nbrick_d) nxt = brick_src(k + 1, st2);
+                    issue_hydro_w(lead, nxt, st2, hs == G::NH - 1 ? 0 : hs + 1);
+                    issue_ppb_w(lead, rec, P.SBa, ps ^ 1);
+                } else if (lane == 0) {
                     tma_wait_read0();
                     if (S >= 0) {
-                        // steady state: brick k is an interior brick of the state buffer — no image, no halo layer; only brick
-                        // k + 1 can be the ghost brick beyond the high end
                         const float* rec = P.in + gcol + (long long)k * P.SBd;
                         if (k + 1 < P.nbrick_d) issue_hydro_at(rec + P.SBd, P.SBa, hs == G::NH - 1 ? 0 : hs + 1);
                         else issue_hydro(k + 1, hs == G::NH - 1 ? 0 : hs + 1);
@@ -1326,7 +1372,17 @@ struct IoBulk {
         if (s == 3) {                                          // brick i >> 2 is complete: ship it
             fence_async_smem();                                // generic-proxy writes -> visible to the async proxy
             __syncwarp();
-            if (lane == 0) {
+            if (S >= 0 && PPM_PRED_COPIES) {
+                const bool lead = true;
+                float* dst = P.out + gcol + (long long)(i >> 2) * P.SBd;
+                const float* sh = hyd0 + hprv;
+                const float* sp = ppr0 + pst;
+                bulk_s2g_p(lead, dst, sh, G::HB * 4);
+                bulk_s2g_p(lead, dst + G::HB, sp, G::PB * 4);
+                bulk_s2g_p(lead && ncol > 1, dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
+                bulk_s2g_p(lead && ncol > 1, dst + P.SBa + G::HB, sp + G::PB + G::PAD, G::PB * 4);
+                tma_commit_p(lead);
+            } else if (lane == 0) {
                 float* dst = P.out + gcol + (long long)(i >> 2) * P.SBd;
                 const float* sh = hyd0 + hprv;
                 const float* sp = ppr0 + pst;
@@ -1455,6 +1511,14 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS
     }
     IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), ph0, lane, gcol, min(2, nba - ba0), c0, c1,
                    (long long)ba0 * P.HBa + (long long)bb * P.HBb);
+    if (PPM_PRED_COPIES) {
+        // The steady-state body issues its bulk copies from the lane elect.sync picks, the generic body from lane 0, and bulk
+        // async-groups belong to the thread that committed them: the two must be the same lane (they are: the lowest one).
+        // Checked once per warp; a mismatch raises the state flag (PPM_ESTATE) instead of racing silently.
+        unsigned e;
+        asm volatile("{\n.reg .pred q;\nelect.sync _|q, 0xffffffff;\nselp.u32 %0, 1, 0, q;\n}\n" : "=r"(e));
+        if ((e != 0) != (lane == 0)) atomicOr(P.flag, 2);
+    }
     // pad pencils of a ragged grid (and the lanes of a missing second brick column) compute garbage that is never read
     const float* pflat = FLAT ? P.flat + ((long long)min(ba0 + (lane >> 4), nba - 1) * P.FBa + (long long)bb * P.FBb +
                                           (((lane & 3) << (2 * G::AXA)) + (((lane >> 2) & 3) << (2 * G::AXB)))) : nullptr;
