@@ -64,7 +64,7 @@ typedef struct {
     int nx, ny, nz;     /* cells; each >= 1 */
     double dx;          /* cubic cells; cell (i,j,k) is centred at ((i+.5)dx, (j+.5)dx, (k+.5)dx) */
     double gamma;       /* ideal-gas adiabatic index, > 1 */
-    double rho_floor, p_floor; /* > 0 */
+    double rho_floor, p_floor; /* p_floor > 0; rho_floor > 1e-30 (the PPB remap divides by the new mass of a cell) */
     ppm_gravity grav;
     int bc[6];
     void *stream; /* cudaStream_t the library enqueues on (0 = default stream) */

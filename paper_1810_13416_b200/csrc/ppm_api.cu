@@ -53,7 +53,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     if (prm->struct_size != sizeof(ppm_params)) { set_err(c, "ppm_create: struct_size %zu != %zu", prm->struct_size, sizeof(ppm_params)); return PPM_EINVAL; }
     if (prm->nx < 1 || prm->ny < 1 || prm->nz < 1) { set_err(c, "ppm_create: grid dims must be >= 1"); return PPM_EINVAL; }
     if ((long long)prm->nx * prm->ny * prm->nz >= (1LL << 31)) { set_err(c, "ppm_create: more than 2^31 - 1 cells (2 x 15 such fields would not fit one GPU anyway)"); return PPM_EINVAL; }
-    if (!(prm->dx > 0.0) || !(prm->gamma > 1.0) || !(prm->rho_floor > 0.0) || !(prm->p_floor > 0.0)) {
+    if (!(prm->dx > 0.0) || !(prm->gamma > 1.0) || !((float)prm->rho_floor > PPM_TINY) || !(prm->p_floor > 0.0)) {     // (rho_floor > 1e-30: the PPB remap divides by the new mass)
         set_err(c, "ppm_create: need dx > 0, gamma > 1, floors > 0"); return PPM_EINVAL;
     }
     if (((uintptr_t)dev_buf_a | (uintptr_t)dev_buf_b) & 127) { set_err(c, "ppm_create: device buffers must be 128-byte aligned"); return PPM_EINVAL; }

@@ -52,7 +52,7 @@
 // warp-uniform shortcuts past work whose outcome is known for every lane (no shock near, star state at the face,
 // Newton converged, PPB polynomial inside its bounds); a bit mask, 0 = always the general code (A/B knob)
 #ifndef PPM_NEWTON_NESTED
-#define PPM_NEWTON_NESTED 0
+#define PPM_NEWTON_NESTED 1     // Newton iterations 2..5 as nested ifs instead of a loop (round 2: -1.6 %, profiles/r2_experiments.md)
 #endif
 #ifndef PPM_UNIFORM_FAST
 #define PPM_UNIFORM_FAST 2      // bits: 1 flattening, 2 converged W_K, 4 star state, 8 PPB theta
@@ -78,6 +78,9 @@
 // steady-state body: bulk copies issued by the whole warp under a leader predicate instead of inside `if (lane == 0)` (A/B knob)
 #ifndef PPM_PRED_COPIES
 #define PPM_PRED_COPIES 1
+#endif
+#ifndef PPM_PPB_PAIRS
+#define PPM_PPB_PAIRS 0      // 1: shift the (a0,a1), (a2,f0) pairs with packed FMA-pipe copies too (measured slower: 12.87 vs 12.83 ms)
 #endif
 #ifndef PPM_PREFETCH_BRICKS
 #define PPM_PREFETCH_BRICKS 1
@@ -300,16 +303,19 @@ __device__ __forceinline__ void parabola(const V5& q0, const V5& Lc, const V5& R
 
 // ---- P4: exact projection of up to three pieces onto the Legendre basis ---------------------------
 // pre-limited coefficients of one cell in local family order, stored as the pairs the remap uses
-struct PpbCell { float a0, a1, a2; v2 bc0, bc1, de; float f; };   // bc0 = (b0, c0), bc1 = (b1, c1), de = (d0, e0)
-__device__ __forceinline__ void mv_ppb(PpbCell& d, const PpbCell& s) { d.a0 = s.a0; d.a1 = s.a1; d.a2 = s.a2; d.f = s.f; d.bc0 = mv2(s.bc0); d.bc1 = mv2(s.bc1); d.de = mv2(s.de); }
+struct PpbCell { v2 a01, a2f; v2 bc0, bc1, de; };   // a01 = (a0, a1), a2f = (a2, f0), bc0 = (b0, c0), bc1 = (b1, c1), de = (d0, e0): all pairs, shifted as such
+__device__ __forceinline__ void mv_ppb(PpbCell& d, const PpbCell& s) { d.a01 = PPM_PPB_PAIRS ? mv2(s.a01) : s.a01; d.a2f = PPM_PPB_PAIRS ? mv2(s.a2f) : s.a2f; d.bc0 = mv2(s.bc0); d.bc1 = mv2(s.bc1); d.de = mv2(s.de); }
 
 // S[0..2]: cells i-1, i, i+1 (masses per dx rm, r0, rp); dl, dr = mass per dx through the left / right
 // face (positive rightward).  The two donor pieces (from i-1 and from i+1) run as one packed computation for
 // the degree-2 family; the (b,c) and (d,e) families are packed inside every piece.
 // irm, ir0, irp: reciprocals of the three masses; rn, irn: the cell's new mass per dx (= r0 - dr + dl; the caller has it
 // as the updated density) and its reciprocal.
+// CHECK: the new mass may vanish (PPB-only sweeps: rn = 1 - dt du/dx), the cell then keeps its coefficients; the full step needs
+// no test: its new density is never below rho_floor, which ppm_create keeps above PPM_TINY.
+template <bool CHECK>
 __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, float ir0, float irp, float rn, float irn, float dl, float dr, float (&out)[10]) {
-    const bool ok = rn > PPM_TINY;
+    const bool ok = !CHECK || rn > PPM_TINY;
     const float dln = fmaxf(-dl, 0.f), drp = fmaxf(dr, 0.f);
     const v2 dD = mk(fmaxf(dl, 0.f), fmaxf(-dr, 0.f));      // donated mass: from the left cell, from the right cell
     const v2 irD = mk(irm, irp);
@@ -326,17 +332,17 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
     const float x21 = fmaf(x1, x1, -1.0f / 12.0f), s21 = fmaf(s1, s1, -1.0f / 12.0f);
     // reference constants (own cell's degree-0 coefficients): projecting a constant is exact, so only
     // deviations from it are integrated (keeps fp32 round-off at the size of the variation)
-    const float refA = S[1].a0;
+    const float refA = S[1].a01.x;
     const v2 refBC = S[1].bc0;
     // ---- degree-2 family: donors packed (x = from i-1, y = from i+1), own piece scalar
     float a0, a1, a2;
     {
-        const v2 c0 = mk(S[0].a0, S[2].a0), c1 = mk(S[0].a1, S[2].a1), c2 = mk(S[0].a2, S[2].a2);
+        const v2 c0 = mk(S[0].a01.x, S[2].a01.x), c1 = mk(S[0].a01.y, S[2].a01.y), c2 = mk(S[0].a2f.x, S[2].a2f.x);
         const v2 E2 = (c2 * bD) * bD, E1 = bD * fma2(c2 + c2, sD, c1);
         const v2 E0 = (c0 - bc(refA)) + fma2(c1, sD, c2 * s2D);
         const v2 J0 = fma2(w2D, E2, wD * E0), J1 = w2D * E1, J2 = fma2(w4D, E2, w2D * E0);
         const v2 A1 = fma2(xD, J0, J1), A2 = fma2(x2D, J0, fma2(xD + xD, J1, J2));
-        const float d1 = S[1].a1, d2 = S[1].a2;
+        const float d1 = S[1].a01.y, d2 = S[1].a2f.x;
         const float e2 = d2 * b1 * b1, e1 = b1 * fmaf(2.0f * d2, s1, d1);
         const float e0 = fmaf(d1, s1, d2 * s21);
         const float j0 = fmaf(w21, e2, w1 * e0), j1 = w21 * e1, j2 = fmaf(w41, e2, w21 * e0);
@@ -358,18 +364,18 @@ __device__ __forceinline__ void ppb_remap(const PpbCell (&S)[3], float irm, floa
         g0 = (J0m + J0o) + J0p;
         g1 = (fma2(bc(xD.x), J0m, J1m) + fma2(bc(x1), J0o, J1o)) + fma2(bc(xD.y), J0p, J1p);
         de = fma2(bc(wD.x), S[0].de, fma2(bc(w1), S[1].de, S[2].de * bc(wD.y)));
-        f0 = fmaf(wD.x, S[0].f, fmaf(w1, S[1].f, wD.y * S[2].f));
+        f0 = fmaf(wD.x, S[0].a2f.y, fmaf(w1, S[1].a2f.y, wD.y * S[2].a2f.y));
     }
-    out[0] = ok ? refA + a0 : S[1].a0;
-    out[1] = ok ? 12.0f * a1 : S[1].a1;
-    out[2] = ok ? 180.0f * a2 : S[1].a2;
+    out[0] = ok ? refA + a0 : S[1].a01.x;
+    out[1] = ok ? 12.0f * a1 : S[1].a01.y;
+    out[2] = ok ? 180.0f * a2 : S[1].a2f.x;
     out[3] = ok ? refBC.x + g0.x : S[1].bc0.x;
     out[4] = ok ? 12.0f * g1.x : S[1].bc1.x;
     out[5] = ok ? refBC.y + g0.y : S[1].bc0.y;
     out[6] = ok ? 12.0f * g1.y : S[1].bc1.y;
     out[7] = ok ? de.x : S[1].de.x;
     out[8] = ok ? de.y : S[1].de.y;
-    out[9] = ok ? f0 : S[1].f;
+    out[9] = ok ? f0 : S[1].a2f.y;
 }
 
 // =====================================================================================================
@@ -481,7 +487,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
     v2 b0fc = bc(0.f);                                                  // (rho0, p0) at the face being solved
     PpbCell mw[3];
 #pragma unroll
-    for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
+    for (int s = 0; s < 3; ++s) { mw[s].a01.x = mw[s].a01.y = mw[s].a2f.x = mw[s].a2f.y = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
 
     float fpre = 0.f;
     if (FLAT) {
@@ -665,14 +671,14 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             // "almost never performed") — then the coefficients are taken as they are
             const float room = fmaxf(0.f, fminf(m[0], 1.0f - m[0]));
             // (a real copy: the register m[0] arrived in is about to be reloaded by the prefetch below)
-            if (IO::HAS_FAST) mw[2].a0 = m[0];
-            else asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
+            if (IO::HAS_FAST) mw[2].a01.x = m[0];
+            else asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a01.x) : "f"(m[0]));
             if ((PPM_UNIFORM_FAST & 8) && __all_sync(wmask, B <= room || !valid)) {
-                mw[2].a1 = m[1]; mw[2].a2 = m[2]; mw[2].f = m[9];
+                mw[2].a01.y = m[1]; mw[2].a2f.x = m[2]; mw[2].a2f.y = m[9];
                 mw[2].bc0 = bc0; mw[2].bc1 = bc1; mw[2].de = de;
             } else {
                 const float th = (B <= room) ? 1.0f : fdiv(room, fmaxf(B, PPM_TINY));
-                mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+                mw[2].a01.y = m[1] * th; mw[2].a2f.x = m[2] * th; mw[2].a2f.y = m[9] * th;
                 mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
             }
             io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
@@ -776,7 +782,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 // the enthalpy of the gas that crosses the face: beta of the mean FV of the slab of mass dt Fm that the PPB
                 // remap takes out of the donor cell (its pre-limited polynomial along the sweep; reading R25)
                 const bool fwd = Fm >= 0.f;
-                const float da0 = fwd ? mw[1].a0 : mw[2].a0, da1 = fwd ? mw[1].a1 : mw[2].a1, da2 = fwd ? mw[1].a2 : mw[2].a2;
+                const float da0 = fwd ? mw[1].a01.x : mw[2].a01.x, da1 = fwd ? mw[1].a01.y : mw[2].a01.y, da2 = fwd ? mw[1].a2f.x : mw[2].a2f.x;
                 const float sig = fminf(dtdx * fabsf(Fm) * (fwd ? gi[1].y : gi[2].y), 1.0f);       // donated fraction of the donor's mass
                 const float hs = fmaf(-0.5f, sig, 0.5f), sm = fwd ? hs : -hs;                       // slab midpoint in its mass coordinate
                 const float fs = fmaf(da2, fmaf(sm, sm, fmaf(sig * sig, 1.0f / 12.0f, -1.0f / 12.0f)), fmaf(da1, sm, da0));
@@ -821,9 +827,9 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (TWOF) {
                 // p beta is what the energy equation advances: p_new = (p_old beta_old + dE - dKE) / beta_new with beta of the
                 // NEW cell mean of FV, i.e. after this sweep's remap; in increment form on the perturbation
-                ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+                ppb_remap<false>(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
                 const float ibn = rcp(fmaf(sat(mo[0]), P.dbeta, P.beta2));
-                pp_new = pp_old + ((dE - dKE) - fw[0].y * (P.dbeta * (sat(mo[0]) - sat(mw[1].a0)))) * ibn;
+                pp_new = pp_old + ((dE - dKE) - fw[0].y * (P.dbeta * (sat(mo[0]) - sat(mw[1].a01.x)))) * ibn;
                 Gnew = 1.0f + ibn;
             } else pp_new = pp_old + (gam - 1.0f) * (dE - dKE);
             const float p0c = fw[0].y - pp_old;
@@ -836,7 +842,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 vmax = fmaxf(vmax, fmaxf(fabsf(u1), fmaxf(fabsf(vw1.x), fabsf(vw1.y))) + cnew);
             }
             ho[0] = rp_new; ho[1] = u1; ho[2] = vw1.x; ho[3] = vw1.y; ho[4] = pp_new;
-            if (!TWOF) ppb_remap(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+            if (!TWOF) ppb_remap<false>(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
             io.template store<S>(i, ho, mo, fluid);
         }
         // ---- rotate the carried pipeline registers ----------------------------------------------------
@@ -900,7 +906,7 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
     float Flm = 0.f;                                        // u at the left face of cell n-4
     PpbCell mw[3];
 #pragma unroll
-    for (int s = 0; s < 3; ++s) { mw[s].a0 = mw[s].a1 = mw[s].a2 = mw[s].f = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
+    for (int s = 0; s < 3; ++s) { mw[s].a01.x = mw[s].a01.y = mw[s].a2f.x = mw[s].a2f.y = 0.f; mw[s].bc0 = mw[s].bc1 = mw[s].de = bc(0.f); }
 #pragma unroll 1
     for (int n = c0 - PPM_NGHOST; n < c1 + PPM_NGHOST; ++n) {
         io.template begin<-1>(n);
@@ -921,8 +927,8 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
             const v2 Bp = fma2(abs2(bc1), bc(0.25f), fma2(abs2(de), bc(1.0f / 6.0f), abs2(bc0) * 0.5f));
             const float B = fmaf(fabsf(m[9]), 0.25f, fmaf(fabsf(m[2]), 1.0f / 6.0f, fmaf(fabsf(m[1]), 0.5f, hsum(Bp))));
             const float th = fminf(1.0f, fdiv(fmaxf(0.f, fminf(m[0], 1.0f - m[0])), fmaxf(B, PPM_TINY)));
-            asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a0) : "f"(m[0]));
-            mw[2].a1 = m[1] * th; mw[2].a2 = m[2] * th; mw[2].f = m[9] * th;
+            asm volatile("mov.f32 %0, %1;" : "=f"(mw[2].a01.x) : "f"(m[0]));
+            mw[2].a01.y = m[1] * th; mw[2].a2f.x = m[2] * th; mw[2].a2f.y = m[9] * th;
             mw[2].bc0 = bc0 * th; mw[2].bc1 = bc1 * th; mw[2].de = de * th;
             io.ppb_prefetch(n - 2, mw[2]);
         }
@@ -930,7 +936,7 @@ __device__ __forceinline__ void march_ppb(const SweepParams& P, IO& io, const in
         if (i >= c0) {
             float mo[10];
             const float rn = 1.0f - dtdx * (Frm - Flm);
-            ppb_remap(mw, 1.0f, 1.0f, 1.0f, rn, rcp(fmaxf(rn, PPM_TINY)), dtdx * Flm, dtdx * Frm, mo);
+            ppb_remap<true>(mw, 1.0f, 1.0f, 1.0f, rn, rcp(fmaxf(rn, PPM_TINY)), dtdx * Flm, dtdx * Frm, mo);
             io.template store_ppb<-1>(i, mo);
         }
         Flm = Frm;
@@ -1000,7 +1006,7 @@ struct IoDirect {
     __device__ __forceinline__ void ppb_prefetch(int c, const PpbCell& used) {
         const int j = image_cell(c, P.n, P.bc_lo, P.bc_hi, snm);
         const float* p = pin + off(j);
-        asm volatile("" : "+l"(p) : "f"(used.a0), "f"(used.a1), "f"(used.a2), "f"(used.f), "f"(used.bc0.x), "f"(used.bc0.y),
+        asm volatile("" : "+l"(p) : "f"(used.a01.x), "f"(used.a01.y), "f"(used.a2f.x), "f"(used.a2f.y), "f"(used.bc0.x), "f"(used.bc0.y),
                      "f"(used.bc1.x), "f"(used.bc1.y), "f"(used.de.x), "f"(used.de.y));
 #pragma unroll
         for (int k = 0; k < 10; ++k) nm[k] = __ldg(p + 64 * (5 + PPB_PERM[DIR][k]));
