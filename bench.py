@@ -252,6 +252,14 @@ def _bench_grid(args, cfg, dev, lr, ws, barrier, K, reps, with_e2e):
         e3.record(g.stream)
         barrier()
         ms_cfl.append(e2.elapsed_time(e3))
+    # the same K steps with the uniform-FV shortcut switched off (PPM_OPT_FV_SHORTCUT = 0): every cell runs the PPB remap
+    ms_noskip = []
+    if not args.advect:
+        from paper_1810_13416_b200.binding import OPT_FV_SHORTCUT
+        g.set_option(OPT_FV_SHORTCUT, 0)
+        do_step(dt, 0); do_step(dt, 5)
+        ms_noskip = _time_steps(g, do_step, dt, K, min(reps, 3), barrier)
+        g.set_option(OPT_FV_SHORTCUT, 1)
     fp32 = None
     try:
         fp32 = g.measure_fp32_peak()
@@ -266,7 +274,7 @@ def _bench_grid(args, cfg, dev, lr, ws, barrier, K, reps, with_e2e):
     g.close()
     del g
     torch.cuda.empty_cache()
-    return {"w": w, "n": n, "ms_reps": ms_reps, "ms_cfl": ms_cfl, "launches": launches, "clocks": clocks, "fp32": fp32,
+    return {"w": w, "n": n, "ms_reps": ms_reps, "ms_cfl": ms_cfl, "ms_noskip": ms_noskip, "launches": launches, "clocks": clocks, "fp32": fp32,
             "e2e": e2e, "warmup": Wm}
 
 
@@ -369,10 +377,15 @@ def run_gpu(args):
                    "eos": "two-fluid: gamma 1.4 (tracked, FV) / 5/3 (ppm_set_two_fluid; reading R25)" if args.two_fluid else "one ideal gas",
                    "geometry": "star inside the confining sphere inscribed in the cube (ppm_set_sphere; PAPER.md L69): cell-updates count ALL cells of the cube, 52 % of which are fluid" if args.sphere else "reflecting cube",
                    "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step, CFL max-reduction fused into the last sweep)",
+                   "fv_shortcut": "on (library default): the PPB remap is skipped where FV is uniform under a whole warp — same values; 'without_fv_shortcut' is the same run with it off",
                    "timing": "median of %d repetitions of the %d-step region (CUDA events on the library's stream)" % (len(r["ms_reps"]), K)},
         "repetitions_ms_per_step": [x / K for x in r["ms_reps"]],
         "roofline": _roofline(n, ms / K, args.advect, peak, peak_kind, fp32_peak, fp32_kind),
         "clocks": r["clocks"], "gpu_launches": int(r["launches"]),
+        "without_fv_shortcut": ({"value": aggregate_value(ncell, K, med(r["ms_noskip"]), ws), "unit": UNIT, "ms_per_step": med(r["ms_noskip"]) / K,
+                                 "roofline_frac": BYTES_PER_CELL_SWEEP * ncell * 3 * K / (med(r["ms_noskip"]) * 1e-3) / 1e9 / peak,
+                                 "note": "PPM_OPT_FV_SHORTCUT = 0: the PPB remap runs in every cell, also where FV is uniform under a whole warp (this rank's time); same values"}
+                                if r["ms_noskip"] else None),
         "with_cfl_dt": {"value": aggregate_value(ncell, K, ms_cfl, ws), "unit": UNIT, "ms_per_step": ms_cfl / K,
                         "note": "ppm_cfl_dt before every step: the maximum is reduced inside the previous step's last sweep, so this is a 4-byte read + host sync"},
     }
@@ -396,7 +409,8 @@ def run_gpu(args):
                         "repetitions_ms_per_step": [x / 5 for x in also["ms_reps"]],
                         "roofline": _roofline(n5, ms_also / 5, False, peak, peak_kind, fp5[0], fp5[1]),
                         "clocks": also["clocks"], "gpu_launches": int(also["launches"]),
-                        "with_cfl_dt_ms_per_step": med(also["ms_cfl"]) / 5}
+                        "with_cfl_dt_ms_per_step": med(also["ms_cfl"]) / 5,
+                        "without_fv_shortcut_ms_per_step": (med(also["ms_noskip"]) / 5 if also["ms_noskip"] else None)}
     elif also:
         line["also"] = also
     if ws == 1 and not args.no_cpu_baseline:

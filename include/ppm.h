@@ -137,6 +137,11 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    only reads 4 bytes back; 0 = ppm_cfl_dt always runs its own reduction pass over the state.  The
  *                    two agree to fp32 rounding of c (bit for bit without a base state).  Whatever else changes the
  *                    state (ppm_set_state, ppm_sweep, a sweep on the direct path) makes ppm_cfl_dt fall back to the pass.
+ *  PPM_OPT_FV_SHORTCUT : 1 (default) = where FV is uniform under a whole warp — the three cells the PPB remap of a cell draws from have
+ *                    the same mean and no higher coefficient, in all 32 pencils of the warp — the remap is skipped: it would return
+ *                    that mean and nine zeros whatever mass moves (the tracked gas differs from its surroundings
+ *                    only near the boundary of the convection zone).  The values are the same (a denormal is a zero either way:
+ *                    the arithmetic is flush-to-zero); 0 = always run the remap (bench.py reports both timings).
  *  PPM_OPT_STATE_FORM : 0 (default) = ppm_set_state / ppm_get_state exchange the FULL rho and p; 1 = they exchange the
  *                    perturbations rho' = rho - rho0, p' = p - p0 exactly as the library stores and evolves them (PAPER.md L35:
  *                    "perturbations to a base, hydrostatic state"), so that no digit of a small perturbation is lost to the
@@ -150,7 +155,7 @@ int ppm_set_chunk(ppm_ctx *ctx, int chunk_cells);
  *                    (ppm_sweep: on the state that sweep starts from) and spread over i-1..i+1 along the sweep.
  *                    Setting it allocates one library-owned device array of ppm_state_floats()/15 floats
  *                    (PPM_ENOMEM if that fails) and adds one light kernel launch per step. */
-enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4, PPM_OPT_STATE_FORM = 5 };
+enum { PPM_OPT_IO_PATH = 2, PPM_OPT_FLATTEN3D = 3, PPM_OPT_CFL_FUSED = 4, PPM_OPT_STATE_FORM = 5, PPM_OPT_FV_SHORTCUT = 6 };
 int ppm_set_option(ppm_ctx *ctx, int option, int value);
 /* Confining sphere ("our star is enclosed in an impenetrable and immovable sphere that
  * is inscribed in the cubical domain of our uniform Cartesian grid ... a very simple boundary condition at the sphere";

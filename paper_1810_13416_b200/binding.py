@@ -25,7 +25,7 @@ EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_swee
            "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_set_two_fluid", "ppm_halo_floats", "ppm_pack_halo", "ppm_set_halo",
            "ppm_set_origin", "ppm_sweep_cfl", "ppm_destroy",
            "ppm_last_error")
-OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED, OPT_STATE_FORM = 2, 3, 4, 5
+OPT_IO_PATH, OPT_FLATTEN3D, OPT_CFL_FUSED, OPT_STATE_FORM, OPT_FV_SHORTCUT = 2, 3, 4, 5, 6
 
 
 class ppm_gravity(C.Structure):

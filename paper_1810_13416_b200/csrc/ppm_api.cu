@@ -103,6 +103,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     if (cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sms < 1) c->sms = 148;
     c->chunk = 0;
     c->cfl_fused = 1; c->cfl_valid = 0;
+    c->fv_shortcut = 1;
     c->err[0] = 0;
     // brick records of 4x4x4 cells x 15 fields; extents are rounded up to whole bricks (ppm_state_floats)
     c->nbx = (prm->nx + 3) / 4; c->nby = (prm->ny + 3) / 4; c->nbz = (prm->nz + 3) / 4;
@@ -309,6 +310,7 @@ extern "C" int ppm_set_option(ppm_ctx* c, int option, int value) {
     if (c->twof && option == PPM_OPT_FLATTEN3D && value == 1) { set_err(c, "ppm_set_option: PPM_OPT_FLATTEN3D not together with the two-fluid equation of state"); return PPM_EINVAL; }
     if (option == PPM_OPT_IO_PATH && (value == 0 || value == 1)) { c->io_path = value; return PPM_OK; }
     if (option == PPM_OPT_STATE_FORM && (value == 0 || value == 1)) { c->pert_io = value; return PPM_OK; }
+    if (option == PPM_OPT_FV_SHORTCUT && (value == 0 || value == 1)) { c->fv_shortcut = value; return PPM_OK; }
     if (option == PPM_OPT_CFL_FUSED && (value == 0 || value == 1)) { c->cfl_fused = value; c->cfl_valid = 0; return PPM_OK; }
     if (option == PPM_OPT_FLATTEN3D && (value == 0 || value == 1)) {
         if (value && !c->F3) {

@@ -50,6 +50,7 @@ struct SweepParams {
     const float* halo_hi;
     long long HBa, HBb;
     unsigned long long k10;         // the packed f32x2 constant (1.0f, 0.0f)
+    int fv_shortcut;                // PPM_OPT_FV_SHORTCUT: skip the PPB remap where FV is uniform under a whole warp (same values)
     // two-fluid EOS (NEXT-4, reading R25): beta(f) = beta2 + f dbeta, beta2 = 1/(gamma_rest - 1), dbeta = 1/(gamma_tracked - 1) - beta2
     int twof;
     float beta2, dbeta;
@@ -92,6 +93,7 @@ struct ppm_ctx {
     int cfl_fused;                  // PPM_OPT_CFL_FUSED (default 1): the last sweep of ppm_step also reduces the CFL maximum of the new state
     int cfl_valid;                  // cflmax holds the maximum of the CURRENT state (set by a fused step, cleared by anything else that changes the state)
     int io_path;                    // PPM_OPT_IO_PATH: 0 = bulk-staged where the sweep-axis extent is whole bricks, 1 = direct everywhere
+    int fv_shortcut;                // PPM_OPT_FV_SHORTCUT (default 1)
     int pert_io;                    // PPM_OPT_STATE_FORM: 1 = ppm_set_state / ppm_get_state exchange rho', p' (perturbation form, as stored)
     long long launches;
     char err[512];

@@ -195,6 +195,31 @@ def test_cfl_reduction_fused_into_the_last_sweep_equals_the_standalone_pass():
         assert len(set(a)) == len(a)                       # the maximum really changes from step to step
 
 
+def test_uniform_fv_shortcut_gives_the_same_values():
+    """PPM_OPT_FV_SHORTCUT: where FV is uniform under a whole warp the PPB remap is skipped; the values must be those of the
+    full remap (bit for bit, up to the sign of a zero), on a state where the shortcut fires in most places (config 4: FV = 0 / 1
+    away from r = 0.45), on one where it fires almost nowhere (config 1) and on a constructed one with exactly uniform slabs."""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_FV_SHORTCUT
+    for cfg, n, steps in ((4, 64, 8), (1, 32, 6)):
+        w = W.make(cfg, n=n)
+        f = w.fields()
+        if cfg == 4:
+            f[5:, :, :, :20] = 0.0                      # an exactly uniform slab next to the varying field
+            f[5, :, :, :20] = 0.25
+        res = []
+        for on in (1, 0):
+            g = PPM.from_workload(w)
+            g.set_option(OPT_FV_SHORTCUT, on)
+            g.set_state(f.cuda())
+            for s in range(steps):
+                g.step(g.cfl_dt(w.cfl), s % 6)
+            res.append(g.get_state())
+            g.close()
+        assert torch.equal(res[0], res[1]), float((res[0] - res[1]).abs().max())
+        assert float(res[0][6:].abs().max()) > 0.0
+
+
 # ---------------------------------------------------------------- reduced-size, full step counts ------
 def test_cfg2_stratified_reduced_64_100_steps():
     w = W.make(2, n=64)
