@@ -834,7 +834,13 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             if (TWOF) {
                 // p beta is what the energy equation advances: p_new = (p_old beta_old + dE - dKE) / beta_new with beta of the
                 // NEW cell mean of FV, i.e. after this sweep's remap; in increment form on the perturbation
-                ppb_remap<false>(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
+                // (the uniform-FV shortcut, see below: the remap returns the cell's own mean and nine zeros)
+                const bool fvu2 = PPM_FV_SKIP && P.fv_shortcut && __all_sync(wmask, (zw == 7 && mw[0].a01.x == mw[1].a01.x && mw[1].a01.x == mw[2].a01.x) || !valid);
+                if (fvu2) {
+                    mo[0] = mw[1].a01.x;
+#pragma unroll
+                    for (int k = 1; k < 10; ++k) mo[k] = 0.f;
+                } else ppb_remap<false>(mw, gi[0].y, gi[1].y, gi[2].y, r_new, irn, dtdx * Flm, dtdx * Frm, mo);
                 const float ibn = rcp(fmaf(sat(mo[0]), P.dbeta, P.beta2));
                 pp_new = pp_old + ((dE - dKE) - fw[0].y * (P.dbeta * (sat(mo[0]) - sat(mw[1].a01.x)))) * ibn;
                 Gnew = 1.0f + ibn;

@@ -201,7 +201,7 @@ def test_uniform_fv_shortcut_gives_the_same_values():
     away from r = 0.45), on one where it fires almost nowhere (config 1) and on a constructed one with exactly uniform slabs."""
     PPM = _gpu()
     from paper_1810_13416_b200.binding import OPT_FV_SHORTCUT
-    for cfg, n, steps in ((4, 64, 8), (1, 32, 6)):
+    for cfg, n, steps, tf in ((4, 64, 8, None), (1, 32, 6, None), (4, 64, 6, TWO_FLUID)):
         w = W.make(cfg, n=n)
         f = w.fields()
         if cfg == 4:
@@ -210,6 +210,8 @@ def test_uniform_fv_shortcut_gives_the_same_values():
         res = []
         for on in (1, 0):
             g = PPM.from_workload(w)
+            if tf:
+                g.set_two_fluid(*tf)                    # (the two-fluid sweeps take the shortcut too)
             g.set_option(OPT_FV_SHORTCUT, on)
             g.set_state(f.cuda())
             for s in range(steps):
