@@ -55,7 +55,7 @@
 #define PPM_NEWTON_NESTED 1     // Newton iterations 2..5 as nested ifs instead of a loop (round 2: -1.6 %, profiles/r2_experiments.md)
 #endif
 #ifndef PPM_UNIFORM_FAST
-#define PPM_UNIFORM_FAST 2      // bits: 1 flattening, 2 converged W_K, 4 star state, 8 PPB theta
+#define PPM_UNIFORM_FAST 3      // bits: 1 flattening, 2 converged W_K, 4 star state, 8 PPB theta  (3: -0.8 % against 2 on the final code)
 #endif
 // direct-path CTA shape (build knobs): threads per CTA (a multiple of 16 = one brick column; the kernel uses no
 // shared memory and no block-wide sync, so the CTA size only sets the granularity of occupancy) and the register
@@ -688,7 +688,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
             }
             io.ppb_prefetch(n - 2, mw[2]);   // one cell ahead of its use (overshoots by one at the end: still a valid image cell)
             // bit s of zw: the nine higher coefficients of cell n-5+s all vanish (B is a positive combination of their moduli)
-            if (PPM_FV_SKIP) zw = ((zw << 1) | (B == 0.f ? 1 : 0)) & 7;
+            if (PPM_FV_SKIP) zw = ((zw << 1) | ((B == 0.f && P.fv_shortcut) ? 1 : 0)) & 7;       // (the run-time switch is folded in here: no branch of its own)
         } else if (PPM_FV_SKIP) zw = (zw << 1) & 7;
         };
         if (TWOF) ppb_take();
@@ -835,7 +835,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 // p beta is what the energy equation advances: p_new = (p_old beta_old + dE - dKE) / beta_new with beta of the
                 // NEW cell mean of FV, i.e. after this sweep's remap; in increment form on the perturbation
                 // (the uniform-FV shortcut, see below: the remap returns the cell's own mean and nine zeros)
-                const bool fvu2 = PPM_FV_SKIP && P.fv_shortcut && __all_sync(wmask, (zw == 7 && mw[0].a01.x == mw[1].a01.x && mw[1].a01.x == mw[2].a01.x) || !valid);
+                const bool fvu2 = PPM_FV_SKIP && __all_sync(wmask, (zw == 7 && mw[0].a01.x == mw[1].a01.x && mw[1].a01.x == mw[2].a01.x) || !valid);
                 if (fvu2) {
                     mo[0] = mw[1].a01.x;
 #pragma unroll
@@ -860,7 +860,7 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
                 // pencil of the warp — the remap returns that mean and nine zeros whatever mass moves (every piece integrates a
                 // deviation from the own cell's constant that is identically zero): the same values, without the ~120 instructions.
                 // (Most of a star: the tracked gas differs from its surroundings only near the boundary of the convection zone.)
-                const bool fvu = PPM_FV_SKIP && P.fv_shortcut && __all_sync(wmask, (zw == 7 && mw[0].a01.x == mw[1].a01.x && mw[1].a01.x == mw[2].a01.x) || !valid);
+                const bool fvu = PPM_FV_SKIP && __all_sync(wmask, (zw == 7 && mw[0].a01.x == mw[1].a01.x && mw[1].a01.x == mw[2].a01.x) || !valid);
                 if (fvu) {
                     mo[0] = mw[1].a01.x;
 #pragma unroll
