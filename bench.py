@@ -39,7 +39,7 @@ FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, 
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md); fallback only
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` captures, keyed by
 # cells per side: (bytes, the profiles/ file it comes from).  A size with no capture reports null.
-NCU_TRAFFIC = {512: (16.096e9, "profiles/r2d_sweeps_ncu_full.md (ncu --set full, 512^3)"),
+NCU_TRAFFIC = {512: (16.096e9, "profiles/r2e_final_sweeps_ncu.md (ncu --set full, 512^3)"),
                1024: (128.85e9, "profiles/r2d_sweeps_1024_ncu.md (ncu, 1024^3)")}
 
 
