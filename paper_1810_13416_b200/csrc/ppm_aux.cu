@@ -112,6 +112,45 @@ __global__ void __launch_bounds__(256) to_full_kernel(AuxParams A, const float* 
     }
 }
 
+// The same two conversions for grids whose x extent is a multiple of 4 (every bulk-staged grid): pure permutes moved as float4.
+// A warp takes one field of two x-adjacent bricks: lane = (brick of the pair, z layer, y row) reads the 4 x-cells of its row from
+// the dense slab (the two bricks' rows are 32 contiguous bytes: whole sectors) and writes them into the brick record, where the
+// 16 rows of a field are 256 contiguous bytes.  TO_PERT: dense full values -> brick records in perturbation form; else the reverse.
+template <bool TO_PERT>
+__global__ void __launch_bounds__(256) convert4_kernel(AuxParams A, const float* __restrict__ from, float* __restrict__ to, int z0, int nzs) {
+    // one CTA per row of bricks along x (blockIdx.x = by, blockIdx.y = brick layer of the slab); its 8 warps share out the brick pairs
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, sub = lane >> 4, zz = (lane >> 2) & 3, yy = lane & 3;
+    const int nbxp = (A.nbx + 1) >> 1;
+    const int by = blockIdx.x, bz = (z0 >> 2) + blockIdx.y;
+    const int y = by * 4 + yy, z = bz * 4 + zz;
+    if (y >= A.ny || z < z0 || z >= z0 + nzs) return;
+    const long long plane = (long long)nzs * A.ny * A.nx;                              // one field of the dense slab
+    const long long drow = ((long long)(z - z0) * A.ny + y) * A.nx;                    // this lane's row in it
+    const long long brow = (long long)(bz * A.nby + by) * A.nbx * PPM_BRICK_FLOATS + zz * 16 + yy * 4;
+    const bool based = !A.pert_io && A.grav_kind != PPM_GRAV_NONE;
+    for (int bxp = warp; bxp < nbxp; bxp += 8) {
+        const int bx = 2 * bxp + sub;
+        if (bx >= A.nbx) continue;
+        const float* fd = from + (TO_PERT ? drow + bx * 4 : brow + (long long)bx * PPM_BRICK_FLOATS);
+        float* td = to + (TO_PERT ? brow + (long long)bx * PPM_BRICK_FLOATS : drow + bx * 4);
+        float4 v[PPM_NFIELDS];
+#pragma unroll
+        for (int f = 0; f < PPM_NFIELDS; ++f) v[f] = *reinterpret_cast<const float4*>(fd + (TO_PERT ? f * plane : (long long)f * 64));
+        if (based) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                double r0, p0;
+                base64(A, bx * 4 + e, y, z, r0, p0);
+                float* c0 = &v[0].x; float* c4 = &v[4].x;
+                c0[e] = TO_PERT ? (float)((double)c0[e] - r0) : (float)((double)c0[e] + r0);
+                c4[e] = TO_PERT ? (float)((double)c4[e] - p0) : (float)((double)c4[e] + p0);
+            }
+        }
+#pragma unroll
+        for (int f = 0; f < PPM_NFIELDS; ++f) *reinterpret_cast<float4*>(td + (TO_PERT ? (long long)f * 64 : f * plane)) = v[f];
+    }
+}
+
 // fp32 base state (rho0, p0) at a cell centre, as the sweeps evaluate it
 __device__ __forceinline__ float2 base32(const AuxParams& A, int i, int j, int k) {
     if (A.grav_kind == PPM_GRAV_CONST_Z) {
@@ -442,7 +481,16 @@ int grid_for(long long n, int cap) {
 
 }  // namespace
 
+// float4 path: x extent a multiple of 4 (rows and brick rows are then 16-byte aligned: the slab sits at the start of a buffer)
+static bool convert4_ok(const ppm_ctx* c) { return (c->prm.nx & 3) == 0; }
+static dim3 convert4_grid(const ppm_ctx* c, int z0, int nzs) { return dim3(c->nby, ((z0 + nzs - 1) >> 2) - (z0 >> 2) + 1, 1); }
+
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs) {
+    if (convert4_ok(c)) {
+        convert4_kernel<true><<<convert4_grid(c, z0, nzs), 256, 0, c->stream>>>(make_aux(c), dense_slab, state, z0, nzs);
+        c->launches += 1;
+        return cudaGetLastError();
+    }
     const long long tot = (long long)c->prm.nx * c->prm.ny * nzs;
     to_perturbation_kernel<<<grid_for(tot, 148 * 16), 256, 0, c->stream>>>(make_aux(c), dense_slab, state, z0, nzs);
     c->launches += 1;
@@ -450,6 +498,11 @@ cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, floa
 }
 
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs) {
+    if (convert4_ok(c)) {
+        convert4_kernel<false><<<convert4_grid(c, z0, nzs), 256, 0, c->stream>>>(make_aux(c), state, dst, z0, nzs);
+        c->launches += 1;
+        return cudaGetLastError();
+    }
     const long long tot = (long long)c->prm.nx * c->prm.ny * nzs;
     to_full_kernel<<<grid_for(tot, 148 * 16), 256, 0, c->stream>>>(make_aux(c), state, dst, z0, nzs);
     c->launches += 1;
