@@ -186,14 +186,14 @@ class PPM:
         self._check(lib().ppm_get_state(self._h, self._ptrs(out), int(z0), int(nzs), int(out.is_cuda)))
         return out
 
-    def step_host_pipelined(self, host_ins, host_outs, dt, orders, slab=32, step=None):
+    def step_host_pipelined(self, host_ins, host_outs, dt, orders, slab=32, step=None, wait=True):
         """End-to-end helper for host-resident grids (argument marshalling and stream plumbing only: every byte is moved
         by cudaMemcpyAsync or by the library's conversion kernels).  For s = 0, 1, ...: upload host_ins[s], advance it one
         step (order orders[s]), download the result into host_outs[s].  All host tensors are pinned [15, nz, ny, nx]
         float32.  The grids are independent of one another, so the upload of grid s+1 (copy stream `up`, z-slabs through
         two device staging slabs, ppm_set_state from device memory) runs while grid s is downloaded (ppm_get_state into
         two more staging slabs, copy stream `down`): PCIe carries both directions at once.  Returns after the last
-        download has finished."""
+        download has finished (wait=False: returns once everything is enqueued; finish_host_pipelined() waits)."""
         nx, ny, nz = self.n
         step = step or self.step
         dev, main = self.device, self.stream
@@ -250,8 +250,18 @@ class PPM:
                     if s + 1 < K:                      # slab k of the state is free again: the next grid's slab k moves in
                         convert_upload(s + 1, k)
                         enqueue_upload()
-            down.synchronize()
-            main.synchronize()
+            if wait:
+                down.synchronize()
+                main.synchronize()
+        if wait:
+            self.sync()
+
+    def finish_host_pipelined(self):
+        """waits for a step_host_pipelined(..., wait=False) of this context (two contexts on two streams, each fed with every
+        other grid, keep both directions of the link busy while either one computes) and reports the state flag"""
+        if getattr(self, "_pipe", None) is not None:
+            self._pipe[4].synchronize()
+        self.stream.synchronize()
         self.sync()
 
     def step(self, dt, order=0):

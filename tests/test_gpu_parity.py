@@ -614,6 +614,16 @@ def test_host_pipelined_exchange_equals_serial_set_step_get():
     for r, o in zip(ref, outs):
         assert np.array_equal(r, o.numpy())
     assert not np.array_equal(ref[0], ref[1])
+    # two contexts on two streams, every other grid each, nothing waited for until both are enqueued (bench.py's e2e leg)
+    g2 = PPM.from_workload(w, stream=torch.cuda.Stream())
+    outs2 = [torch.zeros_like(fi).pin_memory() for fi in ins]
+    g.step_host_pipelined(ins[0::2], outs2[0::2], dt, [0, 2], slab=16, wait=False)
+    g2.step_host_pipelined(ins[1::2], outs2[1::2], dt, [1], slab=16, wait=False)
+    g.finish_host_pipelined()
+    g2.finish_host_pipelined()
+    for r, o in zip(ref, outs2):
+        assert np.array_equal(r, o.numpy())
+    g2.close()
     g.close()
 
 
