@@ -121,6 +121,22 @@ int ppm_cfl_dt(ppm_ctx *ctx, double cfl, double *dt_out);
  * fp64 accumulation in a fixed order (deterministic).  Synchronises the stream. */
 int ppm_reduce_conserved(ppm_ctx *ctx, double out[6]);
 
+/* The same six sums for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the per-block partial sums of the first pass live in a file-scope device array of
+ * the library instead of memory ppm_create allocated.  The call allocates and frees nothing, does not synchronise and
+ * does not read the state flag: it enqueues two kernels on the context's stream.
+ *   nblocks : blocks of the first pass, 1..PPM_STATIC_RED_BLOCKS; 0 = the count ppm_reduce_conserved uses (592) — the
+ *             sums are then bit for bit those of ppm_reduce_conserved; another count changes the order of the fp64
+ *             additions (differences at the 1e-15 level).  More than PPM_STATIC_RED_BLOCKS -> PPM_EINVAL, nothing runs.
+ *   dev_out : [device] 6 doubles, written by the second kernel (valid once the stream has reached it).
+ * The array (6 * PPM_STATIC_RED_BLOCKS doubles = 48 KB) is held by every GPU that loads the library until the process
+ * exits and is SHARED by every call on that GPU, whatever the context: calls that may overlap on the GPU (different
+ * streams) race on it — order them.  It keeps the last call's contents; nothing in it has to start at zero (every slot
+ * that is read was written by the same call).  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress; no allocation by this library). */
+#define PPM_STATIC_RED_BLOCKS 1024
+int ppm_reduce_conserved_static(ppm_ctx *ctx, int nblocks, double *dev_out);
+
 /* Waits for the stream and reports the sticky state flag (PPM_OK / PPM_ESTATE / PPM_ECUDA). */
 int ppm_sync(ppm_ctx *ctx);
 

@@ -17,11 +17,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("PPM_B200_LIB") or os.path.join(HERE, "libppm_b200.so")
 
 PPM_OK, PPM_EINVAL, PPM_ENOMEM, PPM_ECUDA, PPM_ESTATE = 0, 1, 2, 3, 4
+STATIC_RED_BLOCKS = 1024      # PPM_STATIC_RED_BLOCKS: first-pass blocks the static scratch array of ppm_reduce_conserved_static holds
 BC_PERIODIC, BC_REFLECT, BC_HALO = 0, 1, 2
 GRAV_NONE, GRAV_CONST_Z, GRAV_RADIAL = 0, 1, 2
 NF = 15
 EXPORTS = ("ppm_create", "ppm_set_state", "ppm_get_state", "ppm_step", "ppm_sweep", "ppm_advect", "ppm_cfl_dt",
-           "ppm_reduce_conserved", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
+           "ppm_reduce_conserved", "ppm_reduce_conserved_static", "ppm_sync", "ppm_set_chunk", "ppm_set_option", "ppm_axis_path", "ppm_launch_count",
            "ppm_state_floats", "ppm_plan_tail_chunk", "ppm_measure_fp32_peak", "ppm_set_sphere", "ppm_spin_up", "ppm_set_two_fluid", "ppm_halo_floats", "ppm_pack_halo", "ppm_set_halo",
            "ppm_set_origin", "ppm_sweep_cfl", "ppm_destroy",
            "ppm_last_error")
@@ -62,6 +63,7 @@ def lib():
         L.ppm_advect.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.ppm_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.ppm_reduce_conserved.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.ppm_reduce_conserved_static.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
         L.ppm_sync.argtypes = [C.c_void_p]
         L.ppm_set_chunk.argtypes = [C.c_void_p, C.c_int]
         L.ppm_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
@@ -283,6 +285,14 @@ class PPM:
         out = (C.c_double * 6)()
         self._check(lib().ppm_reduce_conserved(self._h, out))
         return np.array(list(out))
+
+    def reduce_conserved_static(self, out, nblocks=0):
+        """ppm_reduce_conserved_static: the six sums into `out` (a float64 CUDA tensor of 6 elements the caller owns); the
+        partial sums live in the library's static device array — no allocation, no synchronisation (enqueue only)"""
+        if not (out.is_cuda and out.dtype == torch.float64 and out.numel() == 6 and out.is_contiguous()):
+            raise ValueError("out: a contiguous float64 CUDA tensor of 6 elements")
+        self._check(lib().ppm_reduce_conserved_static(self._h, int(nblocks), C.c_void_p(out.data_ptr())))
+        return out
 
     def sync(self):
         self._check(lib().ppm_sync(self._h))

@@ -288,6 +288,21 @@ extern "C" int ppm_reduce_conserved(ppm_ctx* c, double out[6]) {
     return read_flag(c);
 }
 
+extern "C" int ppm_reduce_conserved_static(ppm_ctx* c, int nblocks, double* dev_out) {
+    if (!c) { set_err(nullptr, "ppm_reduce_conserved_static: ctx is NULL"); return PPM_EINVAL; }
+    if (!dev_out) { set_err(c, "ppm_reduce_conserved_static: dev_out is NULL"); return PPM_EINVAL; }
+    if (nblocks < 0) { set_err(c, "ppm_reduce_conserved_static: nblocks must be >= 0"); return PPM_EINVAL; }
+    const int nb = nblocks ? nblocks : c->nblocks_red;
+    if (nb > PPM_STATIC_RED_BLOCKS) {
+        set_err(c, "ppm_reduce_conserved_static: %d first-pass blocks need %zu bytes of partial sums; the static scratch array holds %d blocks (%zu bytes)",
+                nb, sizeof(double) * 6 * (size_t)nb, PPM_STATIC_RED_BLOCKS, sizeof(double) * 6 * (size_t)PPM_STATIC_RED_BLOCKS);
+        return PPM_EINVAL;
+    }
+    DevGuard guard(c);
+    CU(ppm_launch_conserved_static(c, nb, dev_out));
+    return PPM_OK;
+}
+
 extern "C" int ppm_sync(ppm_ctx* c) {
     if (!c) { set_err(nullptr, "ppm_sync: ctx is NULL"); return PPM_EINVAL; }
     DevGuard guard(c);

@@ -585,3 +585,46 @@ cudaError_t ppm_launch_conserved(ppm_ctx* c) {
     c->launches += 2;
     return cudaGetLastError();
 }
+
+// ---- conserved sums without any allocation (ppm_reduce_conserved_static) ---------------------------------------------
+// The first pass of the reduction needs 6 partial sums per CTA.  ppm_reduce_conserved keeps them in an array ppm_create
+// allocated; this variant keeps them in a file-scope device array, so the call works where cudaMalloc cannot be called
+// (graph capture, serving loops).  Every GPU that loads the library holds the 48 KB until the process exits; every call
+// on a device shares them.  Each first-pass CTA b < nb overwrites its six slots [q * nb + b] before the second pass reads
+// exactly those, so nothing has to start at zero and a previous call's contents (another nb, another grid) are never read.
+// In host code `g_static_partial` is a host-side stand-in, not a device address: the launch below gets the address
+// cudaGetSymbolAddress reports, looked up once per device with that device current.
+static __device__ __align__(256) double g_static_partial[6 * PPM_STATIC_RED_BLOCKS];
+
+static double* g_static_partial_dev[64] = {};      // device ordinal -> address of g_static_partial on that device
+
+// address of the array on the current device (no allocation; the first call per device asks the runtime)
+static cudaError_t static_partial_ptr(double** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    double* p = g_static_partial_dev[dev];
+    if (!p) {
+        e = cudaGetSymbolAddress((void**)&p, g_static_partial);
+        if (e != cudaSuccess) return e;
+        g_static_partial_dev[dev] = p;             // (two threads racing here store the same value)
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+// same two kernels, same assignment of cells to threads and the same reduction trees as ppm_launch_conserved: with
+// nb = c->nblocks_red the six sums come out bit for bit the same.  The caller made c's device current.
+cudaError_t ppm_launch_conserved_static(ppm_ctx* c, int nb, double* dev_out) {
+    double* partial = nullptr;
+    cudaError_t e = static_partial_ptr(&partial);
+    if (e != cudaSuccess) return e;
+    conserved_kernel<<<nb, 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], partial);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const double dv = c->prm.dx * c->prm.dx * c->prm.dx;
+    conserved_final_kernel<<<1, 32, 0, c->stream>>>(partial, nb, dv, dev_out);
+    c->launches += 2;
+    return cudaGetLastError();
+}

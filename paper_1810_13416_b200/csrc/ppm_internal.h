@@ -109,6 +109,7 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_base_fill(ppm_ctx* c);    // fills R0c, P0c
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
+cudaError_t ppm_launch_conserved_static(ppm_ctx* c, int nblocks, double* dev_out);   // partial sums in a file-scope device array
 cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);
 cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega);
 cudaError_t ppm_launch_pack_halo(ppm_ctx* c, int axis, int side, float* dst);
