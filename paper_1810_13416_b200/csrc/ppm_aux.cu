@@ -280,93 +280,98 @@ __device__ __forceinline__ int aux_image(int i, int n, int bc_lo, int bc_hi, flo
     return min(max(s, 0), n - 1);
 }
 
-// CTA = a tile of 2x2x2 bricks (8x8x8 cells), one thread per cell.  Phase 1 puts the full pressure of the tile and of
-// its two-cell arms along the three axes (the detector needs no corners) and the velocity components into shared
-// memory: 2.5 base-state evaluations per cell instead of 13.  Phase 2 evaluates the three 1-D detectors from there.
+// CTA = a tile of 2x2x2 bricks (8x8x8 cells), one thread per cell; shared memory holds the full pressure of the tile and
+// of its two-cell arms along the three axes (the detector needs no corners): 2.5 staged points per cell instead of 13.
 constexpr int F3_T = 8, F3_H = 2, F3_W = F3_T + 2 * F3_H, F3_N = F3_W * F3_W * F3_W;
 __device__ __forceinline__ int f3_idx(int lx, int ly, int lz) { return ((lz + F3_H) * F3_W + (ly + F3_H)) * F3_W + (lx + F3_H); }
 
-// one point of the tile (d < 0) or of its arms (d = axis of the arm) -> shared memory.  INSIDE: the tile and its arms
-// lie wholly inside the grid (all but the boundary tiles): no image logic at all.
-template <bool INSIDE>
-__device__ __forceinline__ void f3_point(const AuxParams& A, const float* __restrict__ st, float* sP, float (*sU)[F3_N],
-                                         int ox0, int oy0, int oz0, int lx, int ly, int lz, int d, float& rc) {
+// Full pressure of one point of a BOUNDARY tile (the tile itself: d < 0; its arms: d = axis of the arm) -> shared memory,
+// with the boundary images of the grid faces.
+__device__ __forceinline__ void f3_point_edge(const AuxParams& A, const float* __restrict__ st, float* sP,
+                                              int ox0, int oy0, int oz0, int lx, int ly, int lz, int d) {
     int gx = ox0 + lx, gy = oy0 + ly, gz = oz0 + lz;
     const int si = f3_idx(lx, ly, lz);
-    float sgn = 1.f;
-    bool ox = false, oy = false, oz = false;
-    if (!INSIDE) {
-        // A point outside the grid along ONE axis is the boundary image of a cell along that axis (an arm point
-        // by construction, a tile point when the tile overhangs a ragged grid); outside along two axes it is
-        // never anybody's neighbour.
-        ox = (unsigned)gx >= (unsigned)A.nx; oy = (unsigned)gy >= (unsigned)A.ny; oz = (unsigned)gz >= (unsigned)A.nz;
-        const int nout = (int)ox + (int)oy + (int)oz;
-        const int dout = ox ? 0 : (oy ? 1 : (oz ? 2 : d));
-        if (nout > 1 || (d >= 0 && nout == 1 && dout != d)) {
-            sP[si] = 1.f;
-            sU[0][si] = sU[1][si] = sU[2][si] = 0.f;
-            return;
-        }
-        if (ox) gx = aux_image(gx, A.nx, A.bc[0], A.bc[1], sgn);
-        if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
-        if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
-    }
-    // brick index and cell in brick -> float offset of field 0 in the state, slot in a one-field array
+    float sgn;
+    // A point outside the grid along ONE axis is the boundary image of a cell along that axis (an arm point
+    // by construction, a tile point when the tile overhangs a ragged grid); outside along two axes it is
+    // never anybody's neighbour.
+    const bool ox = (unsigned)gx >= (unsigned)A.nx, oy = (unsigned)gy >= (unsigned)A.ny, oz = (unsigned)gz >= (unsigned)A.nz;
+    const int nout = (int)ox + (int)oy + (int)oz;
+    const int dout = ox ? 0 : (oy ? 1 : (oz ? 2 : d));
+    if (nout > 1 || (d >= 0 && nout == 1 && dout != d)) { sP[si] = 1.f; return; }
+    if (ox) gx = aux_image(gx, A.nx, A.bc[0], A.bc[1], sgn);
+    if (oy) gy = aux_image(gy, A.ny, A.bc[2], A.bc[3], sgn);
+    if (oz) gz = aux_image(gz, A.nz, A.bc[4], A.bc[5], sgn);
     const int br = ((gz >> 2) * A.nby + (gy >> 2)) * A.nbx + (gx >> 2), cb = (gz & 3) << 4 | (gy & 3) << 2 | (gx & 3);
-    const long long o = (long long)br * PPM_BRICK_FLOATS + cb;
-    // base state: from the per-cell arrays where they exist (RADIAL: spares a table lookup per staged point), else evaluated
-    const float2 b0 = A.P0c ? make_float2(d < 0 ? __ldg(A.R0c + br * 64LL + cb) : 0.f, __ldg(A.P0c + br * 64LL + cb)) : base32(A, gx, gy, gz);
-    sP[si] = b0.y + st[o + 4 * 64];
-    if (d < 0) {
-        rc = b0.x + st[o];
-        const float ux = st[o + 64], uy = st[o + 2 * 64], uz = st[o + 3 * 64];
-        sU[0][si] = ox ? sgn * ux : ux; sU[1][si] = oy ? sgn * uy : uy; sU[2][si] = oz ? sgn * uz : uz;
-    } else {
-        const float u = sgn * st[o + (1 + d) * 64];
-        if (d == 0) sU[0][si] = u; else if (d == 1) sU[1][si] = u; else sU[2][si] = u;
-    }
+    const float p0 = A.P0c ? __ldg(A.P0c + br * 64LL + cb) : base32(A, gx, gy, gz).y;
+    sP[si] = p0 + st[(long long)br * PPM_BRICK_FLOATS + 4 * 64 + cb];
 }
 
-template <bool INSIDE>
-__device__ __forceinline__ void f3_fill(const AuxParams& A, const float* __restrict__ st, float* sP, float (*sU)[F3_N],
-                                        int ox0, int oy0, int oz0, float& rc) {
-    const int tid = threadIdx.x;
-    {   // the tile itself: thread = (brick in tile, cell in brick) -> coalesced brick reads
-        const int b = tid >> 6, c = tid & 63;
-        f3_point<INSIDE>(A, st, sP, sU, ox0, oy0, oz0, (b & 1) * 4 + (c & 3), ((b >> 1) & 1) * 4 + ((c >> 2) & 3), (b >> 2) * 4 + (c >> 4), -1, rc);
-    }
-    // the arms: 6 faces x 2 depths x 64 points = 768 points; a warp works on one (face, depth) slab half, so the
-    // axis and the side are warp-uniform
-    float dummy;
-    for (int r = tid; r < 6 * 2 * 64; r += 512) {
-        const int f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
-        const int d = f >> 1;
-        const int along = (f & 1) ? F3_T + h : -1 - h;
-        const int lx = (d == 0) ? along : (d == 1 ? bb : a);
-        const int ly = (d == 1) ? along : (d == 2 ? bb : a);
-        const int lz = (d == 2) ? along : (d == 0 ? bb : a);
-        f3_point<INSIDE>(A, st, sP, sU, ox0, oy0, oz0, lx, ly, lz, d, dummy);
-    }
+// One slab of the arms of an INTERIOR tile: face (D, SIDE), the 2 x 4 x 4 cells of neighbour brick (ta, tb) that touch the
+// tile — one warp, lane = (depth e, transverse cell a, bq).  Axis and side are compile-time, the brick is warp-uniform: no
+// index decoding per point.
+template <int D, int SIDE>
+__device__ __forceinline__ void f3_arm(const AuxParams& A, const float* __restrict__ st, float* sP, int B0, int ox0, int oy0, int oz0,
+                                       int ta, int tb, int lane) {
+    constexpr int DA = (D == 0) ? 1 : 0, DB = (D == 2) ? 1 : 2;           // the two transverse axes, in increasing order
+    const int e = lane & 1, a = (lane >> 1) & 3, bq = lane >> 3;
+    const int sB[3] = {1, A.nbx, A.nbx * A.nby};
+    const int br = B0 + (SIDE ? 2 : -1) * sB[D] + ta * sB[DA] + tb * sB[DB];
+    const int ca = SIDE ? e : 2 + e;                                      // cell along D inside that brick
+    const int cb = (ca << (2 * D)) | (a << (2 * DA)) | (bq << (2 * DB));
+    int l[3];
+    l[D] = SIDE ? F3_T + e : e - F3_H; l[DA] = 4 * ta + a; l[DB] = 4 * tb + bq;
+    float p0;
+    if (A.P0c) p0 = __ldg(A.P0c + br * 64LL + cb);
+    else p0 = base32(A, ox0 + l[0], oy0 + l[1], oz0 + l[2]).y;
+    sP[f3_idx(l[0], l[1], l[2])] = p0 + st[(long long)br * PPM_BRICK_FLOATS + 4 * 64 + cb];
 }
 
+// CTA = a tile of 2x2x2 bricks, one thread per cell.  Phase 1 stages the full pressure of the tile and of its arms; phase 2
+// evaluates the three 1-D detectors from shared memory.  The velocities and the density enter only where a pressure jump
+// is near (conv, c): those few warps read them from the state directly.
 __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const float* __restrict__ st, float* __restrict__ F3) {
-    __shared__ float sP[F3_N], sU[3][F3_N];
-    const int tid = threadIdx.x;
+    __shared__ float sP[F3_N];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int org[3] = {(int)blockIdx.x * F3_T, (int)blockIdx.y * F3_T, (int)blockIdx.z * F3_T};
     const float gam = A.gamf;
-    float rc = 1.f;
     const bool inside = org[0] >= F3_H && org[1] >= F3_H && org[2] >= F3_H &&
                         org[0] + F3_T + F3_H <= A.nx && org[1] + F3_T + F3_H <= A.ny && org[2] + F3_T + F3_H <= A.nz;
-    if (inside) f3_fill<true>(A, st, sP, sU, org[0], org[1], org[2], rc);
-    else f3_fill<false>(A, st, sP, sU, org[0], org[1], org[2], rc);
-    __syncthreads();
-    const int b = tid >> 6, c = tid & 63;
+    const int b = tid >> 6, c = tid & 63;                                  // thread = (brick in tile, cell in brick)
     const int lx = (b & 1) * 4 + (c & 3), ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3), lz = (b >> 2) * 4 + (c >> 4);
     const int g[3] = {org[0] + lx, org[1] + ly, org[2] + lz};
-    const bool valid = g[0] < A.nx && g[1] < A.ny && g[2] < A.nz;          // (a tile may overhang a ragged grid)
     const int s0 = f3_idx(lx, ly, lz);
+    const int B0 = ((org[2] >> 2) * A.nby + (org[1] >> 2)) * A.nbx + (org[0] >> 2);
+    const int brick = B0 + (b & 1) + ((b >> 1) & 1) * A.nbx + (b >> 2) * A.nbx * A.nby;     // (meaningful where valid)
+    if (inside) {
+        {   // the tile itself: coalesced brick reads
+            const float p0 = A.P0c ? __ldg(A.P0c + brick * 64LL + c) : base32(A, g[0], g[1], g[2]).y;
+            sP[s0] = p0 + st[(long long)brick * PPM_BRICK_FLOATS + 4 * 64 + c];
+        }
+        // the arms: 6 faces x 4 neighbour bricks = 24 slabs of 32 points for 16 warps; face f goes to warps 4 (f & 3) .. + 3
+        const int wq = warp >> 2, ta = warp & 1, tb = (warp >> 1) & 1;
+        if (wq == 0) { f3_arm<0, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); f3_arm<2, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); }
+        else if (wq == 1) { f3_arm<0, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); f3_arm<2, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); }
+        else if (wq == 2) f3_arm<1, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+        else f3_arm<1, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+    } else {
+        f3_point_edge(A, st, sP, org[0], org[1], org[2], lx, ly, lz, -1);
+        // 6 faces x 2 depths x 64 points = 768 arm points; a warp works on one (face, depth) slab half
+        for (int r = tid; r < 6 * 2 * 64; r += 512) {
+            const int f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
+            const int d = f >> 1;
+            const int along = (f & 1) ? F3_T + h : -1 - h;
+            const int ax = (d == 0) ? along : (d == 1 ? bb : a);
+            const int ay = (d == 1) ? along : (d == 2 ? bb : a);
+            const int az = (d == 2) ? along : (d == 0 ? bb : a);
+            f3_point_edge(A, st, sP, org[0], org[1], org[2], ax, ay, az, d);
+        }
+    }
+    __syncthreads();
+    const bool valid = g[0] < A.nx && g[1] < A.ny && g[2] < A.nz;          // (a tile may overhang a ragged grid)
     float F = 0.f;
     const int stride[3] = {1, F3_W, F3_W * F3_W};
+    const int nd[3] = {A.nx, A.ny, A.nz};
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const int sd = stride[d];
@@ -375,18 +380,31 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
         // the jump ramp clamp(3|d1|/min(p) - 1) is zero unless the pressure changes by a third over two cells: when no cell of
         // the warp is that near a shock along d the coefficient is the same zero without the three divisions
         if (__any_sync(0xffffffffu, valid && 3.0f * fabsf(d1) > pmin)) {
-            const float d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
-            const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
-            const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
-            const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), pmin) - 1.0f);
-            const float conv = __saturatef((sU[d][s0 - sd] - sU[d][s0 + sd]) * ics);
-            F = fmaxf(F, steep * jump * conv);
+            if (valid) {
+                // u_d of the two neighbours along d (boundary image: the normal velocity changes sign in a mirror) and the
+                // density of the cell, from the state
+                float um, up;
+#pragma unroll
+                for (int sgi = 0; sgi < 2; ++sgi) {
+                    int q[3] = {g[0], g[1], g[2]};
+                    float sgn = 1.f;
+                    q[d] += sgi ? 1 : -1;
+                    if ((unsigned)q[d] >= (unsigned)nd[d]) q[d] = aux_image(q[d], nd[d], A.bc[2 * d], A.bc[2 * d + 1], sgn);
+                    const float u = sgn * st[cell_offset(A, q[0], q[1], q[2]) + (1 + d) * 64];
+                    if (sgi) up = u; else um = u;
+                }
+                const float r0 = A.P0c ? __ldg(A.R0c + brick * 64LL + c) : base32(A, g[0], g[1], g[2]).x;
+                const float rc = r0 + st[(long long)brick * PPM_BRICK_FLOATS + c];
+                const float d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
+                const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
+                const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
+                const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), pmin) - 1.0f);
+                const float conv = __saturatef((um - up) * ics);
+                F = fmaxf(F, steep * jump * conv);
+            }
         }
     }
-    if (valid) {
-        const long long brick = ((long long)(g[2] >> 2) * A.nby + (g[1] >> 2)) * A.nbx + (g[0] >> 2);
-        F3[brick * 64 + c] = F;
-    }
+    if (valid) F3[brick * 64LL + c] = F;
 }
 
 // rho0, p0 of every storage slot (pad cells included: harmless values), fp32 exactly as base32 gives them
