@@ -327,37 +327,67 @@ __device__ __forceinline__ void f3_arm(const AuxParams& A, const float* __restri
     sP[f3_idx(l[0], l[1], l[2])] = p0 + st[(long long)br * PPM_BRICK_FLOATS + 4 * 64 + cb];
 }
 
-// CTA = a tile of 2x2x2 bricks, one thread per cell.  Phase 1 stages the full pressure of the tile and of its arms; phase 2
-// evaluates the three 1-D detectors from shared memory.  The velocities and the density enter only where a pressure jump
-// is near (conv, c): those few warps read them from the state directly.
-__global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const float* __restrict__ st, float* __restrict__ F3) {
+// CTA = a tile of 2x2x2 bricks, 128 threads, FOUR cells per thread (the same cell of the four bricks of a y-z square: four
+// times the loads in flight per warp, the per-thread set-up paid once; 2 and 8 cells per thread measured slower).  Phase 1
+// stages the full pressure of the tile and of its arms; phase 2 evaluates the three 1-D detectors from shared memory.  The
+// velocities and the density enter only where a pressure jump is near (conv, c): those few warps read them from the state.
+#ifndef PPM_F3_CPT
+#define PPM_F3_CPT 4
+#endif
+#ifndef PPM_F3_MINB
+#define PPM_F3_MINB (4 * PPM_F3_CPT)
+#endif
+constexpr int F3_CPT = PPM_F3_CPT, F3_THREADS = 512 / F3_CPT;      // cells per thread (2: bricks adjacent in z; 4: in y and z; 8: all of the tile's)
+__global__ void __launch_bounds__(F3_THREADS, PPM_F3_MINB) flatten3d_kernel(const AuxParams A, const float* __restrict__ st, float* __restrict__ F3) {
     __shared__ float sP[F3_N];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int org[3] = {(int)blockIdx.x * F3_T, (int)blockIdx.y * F3_T, (int)blockIdx.z * F3_T};
     const float gam = A.gamf;
     const bool inside = org[0] >= F3_H && org[1] >= F3_H && org[2] >= F3_H &&
                         org[0] + F3_T + F3_H <= A.nx && org[1] + F3_T + F3_H <= A.ny && org[2] + F3_T + F3_H <= A.nz;
-    const int b = tid >> 6, c = tid & 63;                                  // thread = (brick in tile, cell in brick)
-    const int lx = (b & 1) * 4 + (c & 3), ly = ((b >> 1) & 1) * 4 + ((c >> 2) & 3), lz = (b >> 2) * 4 + (c >> 4);
-    const int g[3] = {org[0] + lx, org[1] + ly, org[2] + lz};
+    const int b = tid >> 6, c = tid & 63;                                  // thread = (first of its bricks, cell in brick)
+    const int lx = (b & 1) * 4 + (c & 3), ly = (b >> 1) * 4 + ((c >> 2) & 3), lz = c >> 4;       // first cell; cell h: see hy, hz
+    const int gx = org[0] + lx, gy = org[1] + ly;
     const int s0 = f3_idx(lx, ly, lz);
     const int B0 = ((org[2] >> 2) * A.nby + (org[1] >> 2)) * A.nbx + (org[0] >> 2);
-    const int brick = B0 + (b & 1) + ((b >> 1) & 1) * A.nbx + (b >> 2) * A.nbx * A.nby;     // (meaningful where valid)
+    const int bz = A.nbx * A.nby;
+    const int brick0 = B0 + (b & 1) + (b >> 1) * A.nbx;                    // (meaningful where valid)
+    // cell h of a thread: the same cell of the brick shifted by (hx, hy, hz) bricks
+    auto hx = [](int h) { return F3_CPT == 8 ? (h & 1) : 0; };
+    auto hy = [](int h) { return F3_CPT == 8 ? ((h >> 1) & 1) : (F3_CPT == 4 ? (h & 1) : 0); };
+    auto hz = [](int h) { return F3_CPT == 8 ? (h >> 2) : (F3_CPT == 4 ? (h >> 1) : h); };
     if (inside) {
         {   // the tile itself: coalesced brick reads
-            const float p0 = A.P0c ? __ldg(A.P0c + brick * 64LL + c) : base32(A, g[0], g[1], g[2]).y;
-            sP[s0] = p0 + st[(long long)brick * PPM_BRICK_FLOATS + 4 * 64 + c];
+            float p0[F3_CPT], pq[F3_CPT];
+#pragma unroll
+            for (int h = 0; h < F3_CPT; ++h) {
+                const int br = brick0 + hx(h) + hy(h) * A.nbx + hz(h) * bz;
+                p0[h] = A.P0c ? __ldg(A.P0c + br * 64LL + c) : base32(A, gx + 4 * hx(h), gy + 4 * hy(h), org[2] + lz + 4 * hz(h)).y;
+                pq[h] = st[(long long)br * PPM_BRICK_FLOATS + 4 * 64 + c];
+            }
+#pragma unroll
+            for (int h = 0; h < F3_CPT; ++h) sP[s0 + 4 * hx(h) + 4 * hy(h) * F3_W + 4 * hz(h) * F3_W * F3_W] = p0[h] + pq[h];
         }
-        // the arms: 6 faces x 4 neighbour bricks = 24 slabs of 32 points for 16 warps; face f goes to warps 4 (f & 3) .. + 3
-        const int wq = warp >> 2, ta = warp & 1, tb = (warp >> 1) & 1;
-        if (wq == 0) { f3_arm<0, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); f3_arm<2, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); }
-        else if (wq == 1) { f3_arm<0, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); f3_arm<2, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane); }
-        else if (wq == 2) f3_arm<1, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
-        else f3_arm<1, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+        // the arms: 6 faces x 4 neighbour bricks = 24 slabs of 32 points, dealt to the warps by (neighbour brick, side)
+        constexpr int NW = F3_THREADS / 32;
+#pragma unroll
+        for (int i = 0; i < 8 / NW; ++i) {
+            const int k = warp + i * NW, ta = k & 1, tb = (k >> 1) & 1;
+            if ((k >> 2) == 0) {
+                f3_arm<0, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+                f3_arm<1, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+                f3_arm<2, 0>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+            } else {
+                f3_arm<0, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+                f3_arm<1, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+                f3_arm<2, 1>(A, st, sP, B0, org[0], org[1], org[2], ta, tb, lane);
+            }
+        }
     } else {
-        f3_point_edge(A, st, sP, org[0], org[1], org[2], lx, ly, lz, -1);
+#pragma unroll
+        for (int h = 0; h < F3_CPT; ++h) f3_point_edge(A, st, sP, org[0], org[1], org[2], lx + 4 * hx(h), ly + 4 * hy(h), lz + 4 * hz(h), -1);
         // 6 faces x 2 depths x 64 points = 768 arm points; a warp works on one (face, depth) slab half
-        for (int r = tid; r < 6 * 2 * 64; r += 512) {
+        for (int r = tid; r < 6 * 2 * 64; r += F3_THREADS) {
             const int f = r >> 7, w = r & 127, h = w >> 6, a = w & 7, bb = (w >> 3) & 7;
             const int d = f >> 1;
             const int along = (f & 1) ? F3_T + h : -1 - h;
@@ -368,43 +398,49 @@ __global__ void __launch_bounds__(512) flatten3d_kernel(const AuxParams A, const
         }
     }
     __syncthreads();
-    const bool valid = g[0] < A.nx && g[1] < A.ny && g[2] < A.nz;          // (a tile may overhang a ragged grid)
-    float F = 0.f;
     const int stride[3] = {1, F3_W, F3_W * F3_W};
     const int nd[3] = {A.nx, A.ny, A.nz};
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const int sd = stride[d];
-        const float pp = sP[s0 + sd], pm = sP[s0 - sd];
-        const float d1 = pp - pm, pmin = fminf(pp, pm);
-        // the jump ramp clamp(3|d1|/min(p) - 1) is zero unless the pressure changes by a third over two cells: when no cell of
-        // the warp is that near a shock along d the coefficient is the same zero without the three divisions
-        if (__any_sync(0xffffffffu, valid && 3.0f * fabsf(d1) > pmin)) {
-            if (valid) {
-                // u_d of the two neighbours along d (boundary image: the normal velocity changes sign in a mirror) and the
-                // density of the cell, from the state
-                float um, up;
+    for (int h = 0; h < F3_CPT; ++h) {
+        const int g[3] = {gx + 4 * hx(h), gy + 4 * hy(h), org[2] + lz + 4 * hz(h)};
+        const int sc = s0 + 4 * hx(h) + 4 * hy(h) * F3_W + 4 * hz(h) * F3_W * F3_W;
+        const int brick = brick0 + hx(h) + hy(h) * A.nbx + hz(h) * bz;
+        const bool valid = g[0] < A.nx && g[1] < A.ny && g[2] < A.nz;          // (a tile may overhang a ragged grid)
+        float F = 0.f;
 #pragma unroll
-                for (int sgi = 0; sgi < 2; ++sgi) {
-                    int q[3] = {g[0], g[1], g[2]};
-                    float sgn = 1.f;
-                    q[d] += sgi ? 1 : -1;
-                    if ((unsigned)q[d] >= (unsigned)nd[d]) q[d] = aux_image(q[d], nd[d], A.bc[2 * d], A.bc[2 * d + 1], sgn);
-                    const float u = sgn * st[cell_offset(A, q[0], q[1], q[2]) + (1 + d) * 64];
-                    if (sgi) up = u; else um = u;
+        for (int d = 0; d < 3; ++d) {
+            const int sd = stride[d];
+            const float pp = sP[sc + sd], pm = sP[sc - sd];
+            const float d1 = pp - pm, pmin = fminf(pp, pm);
+            // the jump ramp clamp(3|d1|/min(p) - 1) is zero unless the pressure changes by a third over two cells: when no cell of
+            // the warp is that near a shock along d the coefficient is the same zero without the three divisions
+            if (__any_sync(0xffffffffu, valid && 3.0f * fabsf(d1) > pmin)) {
+                if (valid) {
+                    // u_d of the two neighbours along d (boundary image: the normal velocity changes sign in a mirror) and the
+                    // density of the cell, from the state
+                    float um = 0.f, up = 0.f;
+#pragma unroll
+                    for (int sgi = 0; sgi < 2; ++sgi) {
+                        int q[3] = {g[0], g[1], g[2]};
+                        float sgn = 1.f;
+                        q[d] += sgi ? 1 : -1;
+                        if ((unsigned)q[d] >= (unsigned)nd[d]) q[d] = aux_image(q[d], nd[d], A.bc[2 * d], A.bc[2 * d + 1], sgn);
+                        const float u = sgn * st[cell_offset(A, q[0], q[1], q[2]) + (1 + d) * 64];
+                        if (sgi) up = u; else um = u;
+                    }
+                    const float r0 = A.P0c ? __ldg(A.R0c + brick * 64LL + c) : base32(A, g[0], g[1], g[2]).x;
+                    const float rc = r0 + st[(long long)brick * PPM_BRICK_FLOATS + c];
+                    const float d2 = sP[sc + 2 * sd] - sP[sc - 2 * sd];
+                    const float ics = rsqrtf(gam * __fdividef(sP[sc], rc)) * 20.0f;        // 1 / (0.05 c)
+                    const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
+                    const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), pmin) - 1.0f);
+                    const float conv = __saturatef((um - up) * ics);
+                    F = fmaxf(F, steep * jump * conv);
                 }
-                const float r0 = A.P0c ? __ldg(A.R0c + brick * 64LL + c) : base32(A, g[0], g[1], g[2]).x;
-                const float rc = r0 + st[(long long)brick * PPM_BRICK_FLOATS + c];
-                const float d2 = sP[s0 + 2 * sd] - sP[s0 - 2 * sd];
-                const float ics = rsqrtf(gam * __fdividef(sP[s0], rc)) * 20.0f;        // 1 / (0.05 c)
-                const float steep = __saturatef(10.0f * (__fdividef(fabsf(d1), fmaxf(fabsf(d2), PPM_TINY)) - 0.75f));
-                const float jump = __saturatef(__fdividef(3.0f * fabsf(d1), pmin) - 1.0f);
-                const float conv = __saturatef((um - up) * ics);
-                F = fmaxf(F, steep * jump * conv);
             }
         }
+        if (valid) F3[brick * 64LL + c] = F;
     }
-    if (valid) F3[brick * 64LL + c] = F;
 }
 
 // rho0, p0 of every storage slot (pad cells included: harmless values), fp32 exactly as base32 gives them
@@ -529,7 +565,7 @@ cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z
 
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c) {
     const dim3 grid((c->nbx + 1) / 2, (c->nby + 1) / 2, (c->nbz + 1) / 2);
-    flatten3d_kernel<<<grid, 512, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->F3);
+    flatten3d_kernel<<<grid, F3_THREADS, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->F3);
     c->launches += 1;
     return cudaGetLastError();
 }
