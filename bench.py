@@ -34,7 +34,7 @@ from paper_1810_13416_b200 import workloads as W  # noqa: E402
 METRIC = "cell-updates/s per 3-D PPM+PPB step (fp32); achieved HBM GB/s vs peak"
 UNIT = "cell-updates/s"
 BYTES_PER_CELL_SWEEP = 120.0      # 15 fp32 fields read + written by every sweep
-BYTES_PER_CELL_SWEEP_ADVECT = 84.0   # PPB-only sweep: 1 velocity + 10 coefficients read, 10 written (it moves 120: hydro copied through)
+BYTES_PER_CELL_SWEEP_ADVECT = 84.0   # PPB-only sweep: 1 velocity + 10 coefficients read, 10 written (the hydro fields stay in their buffer)
 FLOPS_PER_CELL_SWEEP = 1307.0     # operation count of the oracle's sweep body, FMA = 2
 FP32_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x FMA x max SM clock (B200_PROFILING.md); fallback only
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep launch from the committed `ncu --set full` captures, keyed by
@@ -206,7 +206,8 @@ def _roofline(n, ms_per_step, advect, peak, peak_kind, fp32_peak, fp32_kind):
     tr = NCU_TRAFFIC.get(n) if not advect else None
     return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
             "traffic": tr[0] if tr else None, "traffic_from": tr[1] if tr else None, "peak_kind": "of " + peak_kind,
-            "kernel": ("ppm_advect_bulk_kernel" if advect else "ppm_sweep_bulk_kernel") + " (3 launches per step; every launch moves 120 B/cell)",
+            "kernel": ("ppm_advect_bulk_kernel (3 launches per step; every launch moves 84 B/cell: u_d and the ten PPB coefficients in, the coefficients out)"
+                       if advect else "ppm_sweep_bulk_kernel (3 launches per step; every launch moves 120 B/cell)"),
             "alu": {"achieved": alu, "peak": fp32_peak, "unit": "TFLOP/s", "frac": alu / fp32_peak, "peak_kind": fp32_kind,
                     "flops_per_cell_sweep": flops_cs}}
 
@@ -426,7 +427,7 @@ def run_gpu(args):
                    "flatten": "3-D detector field" if args.flatten3d else "1-D per sweep (baseline scheme)",
                    "eos": "two-fluid: gamma 1.4 (tracked, FV) / 5/3 (ppm_set_two_fluid; reading R25)" if args.two_fluid else "one ideal gas",
                    "geometry": "star inside the confining sphere inscribed in the cube (ppm_set_sphere; PAPER.md L69): cell-updates count ALL cells of the cube, 52 % of which are fluid" if args.sphere else "reflecting cube",
-                   "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic, 120 moved)" if args.advect else "full PPM+PPB (ppm_step, CFL max-reduction fused into the last sweep)",
+                   "step": "PPB-only advection (ppm_advect; 84 B/cell/sweep algorithmic and moved: the hydro fields stay in their buffer)" if args.advect else "full PPM+PPB (ppm_step, CFL max-reduction fused into the last sweep)",
                    "fv_shortcut": "on (library default): the PPB remap is skipped where FV is uniform under a whole warp — same values; 'without_fv_shortcut' is the same run with it off",
                    "timing": "median of %d repetitions of the %d-step region (CUDA events on the library's stream)" % (len(r["ms_reps"]), K)},
         "repetitions_ms_per_step": [x / K for x in r["ms_reps"]],

@@ -108,7 +108,9 @@ int ppm_sweep(ppm_ctx *ctx, double dt, int axis);
  * coefficients) is advected by the stored velocity field with the PPB remap P2-P4 of the full step.  Reading R22
  * (DESIGN.md): the gas is taken as uniform and the velocity at a face is the mean of the two cell values, so the
  * mode is meant for velocity fields whose component along an axis does not vary along that axis (rotation, shear,
- * translation), for which every sweep is volume preserving.  Only enqueues work (3 kernel launches). */
+ * translation), for which every sweep is volume preserving.  Only enqueues work (3 kernel launches).  On a grid whose three
+ * extents are multiples of 4 these sweeps move the PPB part of the records only; the next call of any other kind then first
+ * copies the hydro fields to where the coefficients are (one more launch, after an odd number of PPB-only sweeps). */
 int ppm_advect(ppm_ctx *ctx, double dt, int sweep_order);
 
 /* dt = cfl*dx / max over cells of max_d(|u_d|) + c, c from the full rho, p (the scheme is explicit, PAPER.md L55;

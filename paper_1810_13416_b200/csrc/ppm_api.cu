@@ -89,7 +89,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     c = (ppm_ctx*)mem;
     c->prm = *prm;
     c->prm.grav.g = c->prm.grav.rho0 = c->prm.grav.p0 = nullptr;   // host arrays are not kept
-    c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0;
+    c->buf[0] = dev_buf_a; c->buf[1] = dev_buf_b; c->cur = 0; c->hyd = 0;
     {   // the device that owns the buffers (falls back to the current one for memory the runtime does not know)
         cudaPointerAttributes pa;
         int cur = 0;
@@ -173,6 +173,7 @@ extern "C" int ppm_set_state(ppm_ctx* c, const float* const fields[PPM_NFIELDS],
     DevGuard guard(c);
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_set_state: fields[%d] is NULL", f); return PPM_EINVAL; }
     const long long plane = (long long)c->prm.nx * c->prm.ny;
+    CU(ppm_make_whole(c));                  // (the scratch buffer may hold the hydro fields after PPB-only sweeps)
     float* st = c->buf[c->cur];
     float* scratch = c->buf[c->cur ^ 1];    // free between steps: stages the dense slab
     const long long tot = plane * nzs;
@@ -191,6 +192,7 @@ extern "C" int ppm_get_state(ppm_ctx* c, float* const fields[PPM_NFIELDS], int z
     DevGuard guard(c);
     for (int f = 0; f < PPM_NFIELDS; ++f) if (!fields[f]) { set_err(c, "ppm_get_state: fields[%d] is NULL", f); return PPM_EINVAL; }
     const long long plane = (long long)c->prm.nx * c->prm.ny, tot = plane * nzs;
+    CU(ppm_make_whole(c));
     float* scratch = c->buf[c->cur ^ 1];    // free between steps
     CU(ppm_launch_to_full(c, c->buf[c->cur], scratch, z0, nzs));
     const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;

@@ -563,7 +563,32 @@ cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z
     return cudaGetLastError();
 }
 
+// hydro part (the first 5 of the 15 fields: 320 floats) of every brick record, src -> dst
+__global__ void __launch_bounds__(256) hydro_part_copy_kernel(const float4* __restrict__ src, float4* __restrict__ dst, long long nbricks) {
+    constexpr int H4 = 5 * 64 / 4, R4 = PPM_BRICK_FLOATS / 4;
+    const long long tot = nbricks * H4;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < tot; t += (long long)gridDim.x * blockDim.x) {
+        const long long b = t / H4;
+        const int e = (int)(t - b * H4);
+        dst[b * R4 + e] = src[b * R4 + e];
+    }
+}
+
+// After PPB-only sweeps through the bulk-staged path the PPB coefficients are in buf[cur] and the hydro fields still in
+// buf[hyd]: this brings them together in buf[cur] (one copy of 20 B per cell, only when something other than another
+// PPB-only sweep looks at the state).
+cudaError_t ppm_make_whole(ppm_ctx* c) {
+    if (c->hyd == c->cur) return cudaSuccess;
+    const long long nbricks = (long long)c->nbx * c->nby * c->nbz;
+    hydro_part_copy_kernel<<<grid_for(nbricks * 80, c->sms * 8), 256, 0, c->stream>>>(reinterpret_cast<const float4*>(c->buf[c->hyd]),
+                                                                                  reinterpret_cast<float4*>(c->buf[c->cur]), nbricks);
+    c->hyd = c->cur;
+    c->launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     const dim3 grid((c->nbx + 1) / 2, (c->nby + 1) / 2, (c->nbz + 1) / 2);
     flatten3d_kernel<<<grid, F3_THREADS, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->F3);
     c->launches += 1;
@@ -579,6 +604,7 @@ cudaError_t ppm_launch_base_fill(ppm_ctx* c) {
 }
 
 cudaError_t ppm_launch_cfl(ppm_ctx* c) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     cudaError_t e = cudaMemsetAsync(c->cflmax, 0, sizeof(unsigned int), c->stream);
     if (e != cudaSuccess) return e;
     const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
@@ -588,6 +614,7 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c) {
 }
 
 cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     const long long n = (long long)c->nbx * c->nby * c->nbz * 64;
     const double cx = c->sphere ? c->sph_c[0] : c->prm.grav.center[0], cy = c->sphere ? c->sph_c[1] : c->prm.grav.center[1];
     spin_up_kernel<<<grid_for(n, c->sms * 16), 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], domega, cx, cy);
@@ -596,6 +623,7 @@ cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega) {
 }
 
 cudaError_t ppm_launch_pack_halo(ppm_ctx* c, int axis, int side, float* dst) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     const int nbd = (axis == 0) ? c->nbx : (axis == 1 ? c->nby : c->nbz);
     const int na = (axis == 0) ? c->nby : c->nbx, nb = (axis == 2) ? c->nby : c->nbz;
     const long long tot = (long long)na * nb * (PPM_BRICK_FLOATS / 4);
@@ -630,6 +658,7 @@ cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops) {
 }
 
 cudaError_t ppm_launch_conserved(ppm_ctx* c) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     const int nb = c->nblocks_red;
     conserved_kernel<<<nb, 256, 0, c->stream>>>(make_aux(c), c->buf[c->cur], c->partial);
     cudaError_t e = cudaGetLastError();
@@ -671,6 +700,7 @@ static cudaError_t static_partial_ptr(double** out) {
 // same two kernels, same assignment of cells to threads and the same reduction trees as ppm_launch_conserved: with
 // nb = c->nblocks_red the six sums come out bit for bit the same.  The caller made c's device current.
 cudaError_t ppm_launch_conserved_static(ppm_ctx* c, int nb, double* dev_out) {
+    { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     double* partial = nullptr;
     cudaError_t e = static_partial_ptr(&partial);
     if (e != cudaSuccess) return e;

@@ -60,12 +60,15 @@ struct SweepParams {
     // 3-D flattening mode: F~ of every cell, [brick][4z][4y][4x] (a brick is 64 floats: strides = SB / 15); else NULL
     const float* flat;
     long long FBd, FBa, FBb;
+    // PPB-only sweeps, bulk-staged path: the brick records at in + hdelta hold the hydro fields (the other state buffer, or 0)
+    long long hdelta;
 };
 
 struct ppm_ctx {
     ppm_params prm;
     float* buf[2];
-    int cur;                        // buf[cur] holds the state
+    int cur;                        // buf[cur] holds the state ...
+    int hyd;                        // ... except, after PPB-only sweeps, the hydro part of the records: that is in buf[hyd] (ppm_make_whole)
     cudaStream_t stream;
     int device;                     // the device that owns buf[0], buf[1]; every entry point switches to it
     float4* tab;                    // device gravity table (fp32 nodes)
@@ -105,6 +108,7 @@ bool ppm_axis_is_bulk(const ppm_ctx* c, int axis);
 int ppm_tail_chunk(int ntail, int slots, int n);   // segment length for the pencils of the ragged last wave
 cudaError_t ppm_launch_to_perturbation(ppm_ctx* c, const float* dense_slab, float* state, int z0, int nzs);
 cudaError_t ppm_launch_to_full(ppm_ctx* c, const float* state, float* dst, int z0, int nzs);
+cudaError_t ppm_make_whole(ppm_ctx* c);          // hyd != cur: copies the hydro part of every record into buf[cur]; every reader of the state calls it
 cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_base_fill(ppm_ctx* c);    // fills R0c, P0c

@@ -1175,9 +1175,13 @@ __device__ __forceinline__ void tma_wait_read0_p(bool lead) {
     asm volatile("{\n.reg .pred q;\n.reg .pred e;\nelect.sync _|e, 0xffffffff;\nsetp.ne.b32 q, %0, 0;\nand.pred q, q, e;\n@q cp.async.bulk.wait_group.read 0;\n}\n" ::"r"((int)lead) : "memory");
 }
 
-template <int DIR>
+// ADV: the PPB-only sweeps (NEXT-2) — of a brick's hydro part only the velocity component along the sweep axis is staged (one
+// 256-byte field, from the buffer that holds the hydro fields: P.in + P.hdelta) and only its PPB part goes back to global memory.
+template <int DIR, bool ADV = false>
 struct IoBulk {
     using G = BulkGeom<DIR>;
+    static constexpr int HOFF = ADV ? 64 * Dir<DIR>::U : 0;          // first float of a brick's hydro part that is staged
+    static constexpr int HBYTES = ADV ? 64 * 4 : G::HB * 4;         // bytes of it
     static constexpr int SH = 2 * DIR;   // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
     float* const hyd;            // warp's hydro ring [NH][HSLOT], already offset to the lane's layer-0 element
@@ -1244,9 +1248,10 @@ struct IoBulk {
     }
     // src = the record of the wanted brick in the warp's first column, st2 = stride to its second column
     __device__ __forceinline__ void issue_hydro_at(const float* src, long long st2, int slot) {       // lane 0 only
-        mbar_expect_tx(bar + slot, ncol * G::HB * 4);
-        bulk_g2s(hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
-        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + st2, G::HB * 4, bar + slot);
+        if (ADV) src += P.hdelta + HOFF;
+        mbar_expect_tx(bar + slot, ncol * HBYTES);
+        bulk_g2s(hyd0 + slot * G::HSLOT + HOFF, src, HBYTES, bar + slot);
+        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD + HOFF, src + st2, HBYTES, bar + slot);
     }
     __device__ __forceinline__ void issue_ppb_at(const float* src, long long st2, int slot) {         // lane 0 only
         mbar_expect_tx(bar + G::NH + slot, ncol * G::PB * 4);
@@ -1416,10 +1421,10 @@ struct IoBulk {
                 float* dst = P.out + gcol + (long long)(i >> 2) * P.SBd;
                 const float* sh = hyd0 + hprv;
                 const float* sp = ppr0 + pst;
-                bulk_s2g(dst, sh, G::HB * 4);
+                if (!ADV) bulk_s2g(dst, sh, G::HB * 4);
                 bulk_s2g(dst + G::HB, sp, G::PB * 4);
                 if (ncol > 1) {
-                    bulk_s2g(dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
+                    if (!ADV) bulk_s2g(dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
                     bulk_s2g(dst + P.SBa + G::HB, sp + G::PB + G::PAD, G::PB * 4);
                 }
                 tma_commit();
@@ -1573,8 +1578,10 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS
     }
 }
 
-// PPB-only sweep (NEXT-2), bulk-staged path: same rings; the hydro slots travel through unchanged
-template <int DIR>
+// PPB-only sweep (NEXT-2), bulk-staged path: same rings; the hydro fields stay where they are (the buffer P.in + P.hdelta) and
+// only the PPB part of every brick is written to P.out — the launcher keeps track of which buffer holds which part
+// (SPLIT = false: whole records in, whole records out — grids on which another axis takes the direct path)
+template <int DIR, bool SPLIT>
 __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS) ppm_advect_bulk_kernel(const SweepParams P) {
     using G = BulkGeom<DIR>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -1592,7 +1599,7 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS
     const int ba0 = (tx * G::WARPS + warp) * 2;
     if (ba0 >= nba) return;
     const long long gcol = (long long)ba0 * P.SBa + (long long)bb * P.SBb;
-    IoBulk<DIR> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
+    IoBulk<DIR, SPLIT> io(P, sm + warp * G::WARP_FLOATS, bars + warp * (G::NH + G::NP), 0u, lane, gcol, min(2, nba - ba0), c0, c1);
     march_ppb<DIR>(P, io, c0, c1);
 }
 
@@ -1663,9 +1670,10 @@ cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st
     return launch_bulk_kernel<DIR>(ppm_sweep_bulk_kernel<DIR, GRAV, FLAT, false, false, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
-cudaError_t launch_advect_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    static int occ[MAX_DEV] = {};
-    return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR>, occ, P, sms, user_chunk, st);
+cudaError_t launch_advect_bulk(SweepParams& P, bool split, int sms, int user_chunk, cudaStream_t st) {
+    static int occ[2][MAX_DEV] = {};
+    if (split) return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR, true>, occ[1], P, sms, user_chunk, st);
+    return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
 cudaError_t launch_bulk_dir(SweepParams& P, int grav, int sms, int user_chunk, cudaStream_t st) {
@@ -1720,8 +1728,14 @@ bool ppm_axis_is_bulk(const ppm_ctx* c, int axis) {
 cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool fuse_cfl) {
     const ppm_params& p = c->prm;
     SweepParams P;
+    // A PPB-only sweep through the bulk-staged path writes the PPB part of the records only: the hydro fields stay in the buffer
+    // c->hyd while the PPB coefficients move to the other one.  Every other kind of sweep needs (and leaves) a whole state.
+    // (only on grids where all three axes take that path: a direct-path sweep in between would need the whole state back each time)
+    const bool split = advect && ppm_axis_is_bulk(c, 0) && ppm_axis_is_bulk(c, 1) && ppm_axis_is_bulk(c, 2);
+    if (!split) { cudaError_t ew = ppm_make_whole(c); if (ew != cudaSuccess) return ew; }
     P.in = c->buf[c->cur];
     P.out = c->buf[c->cur ^ 1];
+    P.hdelta = split ? (long long)(c->buf[c->hyd] - c->buf[c->cur]) : 0;
     const int ext[3] = {p.nx, p.ny, p.nz};
     const int ia = (axis == 0) ? 1 : 0;       // first transverse axis
     const int ib = (axis == 2) ? 1 : 2;       // second transverse axis
@@ -1767,9 +1781,9 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
         const int uc = c->chunk > 0 ? chunk : 0;                              // 0: whole pencils, the last wave cut to finish together
 #ifndef PPM_EXP_ONE
         if (advect) {
-            if (axis == 0) e = launch_advect_bulk<0>(P, c->sms, uc, c->stream);
-            else if (axis == 1) e = launch_advect_bulk<1>(P, c->sms, uc, c->stream);
-            else e = launch_advect_bulk<2>(P, c->sms, uc, c->stream);
+            if (axis == 0) e = launch_advect_bulk<0>(P, split, c->sms, uc, c->stream);
+            else if (axis == 1) e = launch_advect_bulk<1>(P, split, c->sms, uc, c->stream);
+            else e = launch_advect_bulk<2>(P, split, c->sms, uc, c->stream);
         } else
 #endif
         if (axis == 0) e = launch_bulk_dir<0>(P, p.grav.kind, c->sms, uc, c->stream);
@@ -1790,6 +1804,6 @@ cudaError_t ppm_launch_sweep(ppm_ctx* c, int axis, double dt, bool advect, bool 
         else if (axis == 1) e = launch_dir<1>(P, p.grav.kind, grid, block, c->stream);
         else e = launch_dir<2>(P, p.grav.kind, grid, block, c->stream);
     }
-    if (e == cudaSuccess) { c->cur ^= 1; c->launches += 1; }
+    if (e == cudaSuccess) { c->cur ^= 1; c->launches += 1; if (!split) c->hyd = c->cur; }
     return e;
 }

@@ -359,6 +359,46 @@ def test_advect_matches_oracle_and_paths_agree():
         assert np.abs(os_[5] - f[5]).max() > 1e-3               # ... and FV really moved
 
 
+def test_advect_split_state_mixes_with_every_other_call():
+    """the bulk-staged PPB-only sweeps write the PPB part of the brick records only, so after an odd number of them the hydro
+    fields and the PPB coefficients sit in different buffers until something else looks at the state (ppm_make_whole):
+    interleaved with full steps, single sweeps, partial loads, reductions and reads, the bulk-staged path must return bit
+    for bit what the direct path (whole records in every sweep) returns"""
+    PPM = _gpu()
+    from paper_1810_13416_b200.binding import OPT_IO_PATH
+    w = W.make(1)
+    f = w.fields().numpy()
+    f[1:4] *= 4.0
+    dt = 0.3 * w.dx / (np.abs(f[1:4]).max() + np.sqrt(1.4 * f[4].max() / f[0].min()))
+    res = []
+    for io in (0, 1):
+        g = PPM.from_workload(w)
+        g.set_option(OPT_IO_PATH, io)
+        g.set_state(f)
+        out = []
+        g.advect(dt, 0)                                   # 3 sweeps: split
+        out.append(g.get_state().cpu().numpy())           # read of a split state
+        assert np.array_equal(out[-1][:5], f[:5])
+        g.advect(dt, 1)
+        g.step(dt, 2)                                     # full step on a split state
+        g.advect(dt, 3)
+        out.append(np.array([g.cfl_dt(0.8)]))             # reduction over a split state
+        g.advect(dt, 4)
+        g.advect(dt, 5)                                   # even number: whole again without a copy
+        g.sweep(dt, 1)
+        g.advect(dt, 0)
+        out.append(g.reduce_conserved())
+        g.advect(dt, 2)
+        g.set_state(np.ascontiguousarray(f[:, 8:16]), z0=8)     # partial load (z-planes 8..15) into a split state
+        g.advect(dt, 1)
+        out.append(g.get_state().cpu().numpy())
+        res.append(out)
+        g.close()
+    for a, b in zip(res[0], res[1]):
+        assert np.array_equal(a, b)
+    assert not np.array_equal(res[0][0][5], f[5])
+
+
 def test_advect_slotted_disc_one_revolution_fig3():
     """PAPER.md Fig. 3 on the paper's grid: 100 x 100 cells (x 1: the 2-D case, six in-plane coefficients), one
     revolution = 1256 PPB-only steps, against the oracle.  The field is a 0/1 indicator, so the bar is the L1 one."""
