@@ -917,8 +917,8 @@ __device__ __forceinline__ void march(const SweepParams& P, IO& io, const int a,
 }
 
 // =====================================================================================================
-// NEXT-2 (Fig. 3): PPB-only sweep.  The hydro state is held fixed (its fields are
-// copied through) and FV is advected by the stored velocity field: uniform gas (rho = 1), face velocity = mean of
+// NEXT-2 (Fig. 3): PPB-only sweep.  The hydro state is held fixed (direct path: its fields are
+// copied through; bulk-staged path: they stay in their buffer, see IoBulk<DIR, ADV>) and FV is advected by the stored velocity field: uniform gas (rho = 1), face velocity = mean of
 // the two cell values, mass through the face = dt * u_f (reading R22); P2-P4 exactly as in march().
 // Same iteration timing as march(), so the IO classes serve both: iteration n takes the velocity of cell n and
 // the coefficients of cell n-3, and finishes cell n-4.
