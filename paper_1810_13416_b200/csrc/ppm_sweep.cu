@@ -1131,17 +1131,19 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 // for 3 bricks of marching (input, output, in flight to global) and a PPB slot for 2: rings of 3 and 2 slots,
 // 17.8 KB per warp, 12 warps per SM.
 // =====================================================================================================
-template <int DIR> struct BulkGeom {
+// ADV: the split PPB-only sweeps stage one hydro field per brick, so the hydro slots shrink and four CTAs fit an SM
+template <int DIR, bool ADV = false> struct BulkGeom {
     static constexpr int AXA = (DIR == 0) ? 1 : 0, AXB = (DIR == 2) ? 1 : 2;
     // the second brick of a slot is shifted so that the two half warps fall on different banks where the
     // direction allows it (z: 16 lanes contiguous; y: 4-float runs 16 apart; x: every 4th bank, 4-way inherent)
     static constexpr int PAD = (DIR == 2) ? 16 : ((DIR == 1) ? 8 : 4);
-    static constexpr int HB = 5 * 64, PB = 10 * 64;             // floats per brick: hydro part, PPB part
-    static constexpr int HSLOT = 2 * HB + PAD, PSLOT = 2 * PB + PAD;
+    static constexpr int HB = 5 * 64, PB = 10 * 64;             // floats per brick record: hydro part, PPB part
+    static constexpr int HBS = ADV ? 64 : HB;                   // floats of a brick's hydro part in shared memory
+    static constexpr int HSLOT = 2 * HBS + PAD, PSLOT = 2 * PB + PAD;
     static constexpr int NH = 3, NP = 2;                        // ring depths
     static constexpr int WARP_FLOATS = NH * HSLOT + NP * PSLOT;
     static constexpr int WARPS = PPM_BULK_WARPS;                // warps per CTA (build knob; 12 warps are resident per SM)
-    static constexpr int CTAS = 12 / PPM_BULK_WARPS;            // resident CTAs per SM the launch bounds ask for
+    static constexpr int CTAS = (ADV ? 16 : 12) / PPM_BULK_WARPS;   // resident CTAs per SM the launch bounds ask for
     static constexpr size_t SMEM = (size_t)WARPS * WARP_FLOATS * 4 + WARPS * (NH + NP) * sizeof(uint64_t);
 };
 
@@ -1179,9 +1181,10 @@ __device__ __forceinline__ void tma_wait_read0_p(bool lead) {
 // 256-byte field, from the buffer that holds the hydro fields: P.in + P.hdelta) and only its PPB part goes back to global memory.
 template <int DIR, bool ADV = false>
 struct IoBulk {
-    using G = BulkGeom<DIR>;
-    static constexpr int HOFF = ADV ? 64 * Dir<DIR>::U : 0;          // first float of a brick's hydro part that is staged
-    static constexpr int HBYTES = ADV ? 64 * 4 : G::HB * 4;         // bytes of it
+    using G = BulkGeom<DIR, ADV>;
+    static constexpr int HOFF = ADV ? 64 * Dir<DIR>::U : 0;          // first float of a record's hydro part that is staged
+    static constexpr int HBYTES = G::HBS * 4;                       // bytes of it
+    static constexpr int FU = ADV ? 0 : 64 * Dir<DIR>::U;            // where the normal velocity sits in a staged hydro part
     static constexpr int SH = 2 * DIR;   // in-brick stride along the sweep axis = 1 << SH floats
     const SweepParams& P;
     float* const hyd;            // warp's hydro ring [NH][HSLOT], already offset to the lane's layer-0 element
@@ -1205,7 +1208,7 @@ struct IoBulk {
     __device__ __forceinline__ IoBulk(const SweepParams& P_, float* wsm, uint64_t* wbar, unsigned ph_, int lane_, long long gcol_, int ncol_, int c0, int c1,
                                       long long hcol_ = 0)
         : P(P_),
-          hyd(wsm + (lane_ >> 4) * (G::HB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
+          hyd(wsm + (lane_ >> 4) * (G::HBS + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
           ppr(wsm + G::NH * G::HSLOT + (lane_ >> 4) * (G::PB + G::PAD) + ((lane_ & 3) << (2 * G::AXA)) + (((lane_ >> 2) & 3) << (2 * G::AXB))),
           hyd0(wsm), ppr0(wsm + G::NH * G::HSLOT), bar(wbar), lane(lane_), gcol(gcol_), hcol(hcol_), ncol(ncol_), k0(c0 / 4 - 1), kend(c1 / 4),
           ph(ph_), hs(0), ps(0), hcur(0), hprv(0), pcur(0), pst(0), hrev(0), prev(0), jb(0) {
@@ -1239,7 +1242,7 @@ struct IoBulk {
     __device__ __forceinline__ void issue_hydro_w(bool lead, const float* src, long long st2, int slot) {
         mbar_expect_tx_p(lead, bar + slot, ncol * G::HB * 4);
         bulk_g2s_p(lead, hyd0 + slot * G::HSLOT, src, G::HB * 4, bar + slot);
-        bulk_g2s_p(lead && ncol > 1, hyd0 + slot * G::HSLOT + G::HB + G::PAD, src + st2, G::HB * 4, bar + slot);
+        bulk_g2s_p(lead && ncol > 1, hyd0 + slot * G::HSLOT + G::HBS + G::PAD, src + st2, G::HB * 4, bar + slot);
     }
     __device__ __forceinline__ void issue_ppb_w(bool lead, const float* src, long long st2, int slot) {
         mbar_expect_tx_p(lead, bar + G::NH + slot, ncol * G::PB * 4);
@@ -1250,8 +1253,8 @@ struct IoBulk {
     __device__ __forceinline__ void issue_hydro_at(const float* src, long long st2, int slot) {       // lane 0 only
         if (ADV) src += P.hdelta + HOFF;
         mbar_expect_tx(bar + slot, ncol * HBYTES);
-        bulk_g2s(hyd0 + slot * G::HSLOT + HOFF, src, HBYTES, bar + slot);
-        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HB + G::PAD + HOFF, src + st2, HBYTES, bar + slot);
+        bulk_g2s(hyd0 + slot * G::HSLOT, src, HBYTES, bar + slot);
+        if (ncol > 1) bulk_g2s(hyd0 + slot * G::HSLOT + G::HBS + G::PAD, src + st2, HBYTES, bar + slot);
     }
     __device__ __forceinline__ void issue_ppb_at(const float* src, long long st2, int slot) {         // lane 0 only
         mbar_expect_tx(bar + G::NH + slot, ncol * G::PB * 4);
@@ -1346,7 +1349,7 @@ struct IoBulk {
             j = n;
             const float* src = hyd + hcur + (((S < 4) ? S : (n & 3)) << SH);
             v[0] = src[0];
-            v[1] = src[64 * Dir<DIR>::U];
+            v[1] = src[FU];
             v[2] = src[64 * Dir<DIR>::V];
             v[3] = src[64 * Dir<DIR>::W];
             v[4] = src[64 * 4];
@@ -1356,9 +1359,10 @@ struct IoBulk {
         sgn = hrev ? -1.0f : 1.0f;
         j = jb + s;
         const float* src = hyd + hcur + (s << SH);
-        v[0] = src[0];
-        const float un = src[64 * Dir<DIR>::U];
+        const float un = src[FU];
         v[1] = hrev ? -un : un;                                // normal velocity: odd under the mirror
+        if (ADV) { v[0] = v[2] = v[3] = v[4] = 0.f; return; }   // (the PPB-only sweeps stage nothing else)
+        v[0] = src[0];
         v[2] = src[64 * Dir<DIR>::V];
         v[3] = src[64 * Dir<DIR>::W];
         v[4] = src[64 * 4];
@@ -1414,7 +1418,7 @@ struct IoBulk {
                 const float* sp = ppr0 + pst;
                 bulk_s2g_p(lead, dst, sh, G::HB * 4);
                 bulk_s2g_p(lead, dst + G::HB, sp, G::PB * 4);
-                bulk_s2g_p(lead && ncol > 1, dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
+                bulk_s2g_p(lead && ncol > 1, dst + P.SBa, sh + G::HBS + G::PAD, G::HB * 4);
                 bulk_s2g_p(lead && ncol > 1, dst + P.SBa + G::HB, sp + G::PB + G::PAD, G::PB * 4);
                 tma_commit_p(lead);
             } else if (lane == 0) {
@@ -1424,7 +1428,7 @@ struct IoBulk {
                 if (!ADV) bulk_s2g(dst, sh, G::HB * 4);
                 bulk_s2g(dst + G::HB, sp, G::PB * 4);
                 if (ncol > 1) {
-                    if (!ADV) bulk_s2g(dst + P.SBa, sh + G::HB + G::PAD, G::HB * 4);
+                    if (!ADV) bulk_s2g(dst + P.SBa, sh + G::HBS + G::PAD, G::HB * 4);
                     bulk_s2g(dst + P.SBa + G::HB, sp + G::PB + G::PAD, G::PB * 4);
                 }
                 tma_commit();
@@ -1582,8 +1586,8 @@ __global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS
 // only the PPB part of every brick is written to P.out — the launcher keeps track of which buffer holds which part
 // (SPLIT = false: whole records in, whole records out — grids on which another axis takes the direct path)
 template <int DIR, bool SPLIT>
-__global__ void __launch_bounds__(BulkGeom<DIR>::WARPS * 32, BulkGeom<DIR>::CTAS) ppm_advect_bulk_kernel(const SweepParams P) {
-    using G = BulkGeom<DIR>;
+__global__ void __launch_bounds__(BulkGeom<DIR, SPLIT>::WARPS * 32, BulkGeom<DIR, SPLIT>::CTAS) ppm_advect_bulk_kernel(const SweepParams P) {
+    using G = BulkGeom<DIR, SPLIT>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* sm = reinterpret_cast<float*>(smem_raw);
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)G::WARPS * G::WARP_FLOATS * 4);
@@ -1622,9 +1626,9 @@ int ppm_tail_chunk_impl(int ntail, int slots, int n) {
 // segment plan + launch of one bulk-path kernel; occs caches the kernel's resident CTAs per SM, per device (the
 // shared-memory opt-in is a per-device function attribute)
 constexpr int MAX_DEV = 64;
-template <int DIR>
+template <int DIR, bool ADV = false>
 cudaError_t launch_bulk_kernel(void (*kern)(const SweepParams), int (&occs)[MAX_DEV], SweepParams& P, int sms, int user_chunk, cudaStream_t st) {
-    using G = BulkGeom<DIR>;
+    using G = BulkGeom<DIR, ADV>;
     int dev = 0;
     cudaGetDevice(&dev);
     int& occ = occs[dev & (MAX_DEV - 1)];
@@ -1672,7 +1676,7 @@ cudaError_t launch_bulk(SweepParams& P, int sms, int user_chunk, cudaStream_t st
 template <int DIR>
 cudaError_t launch_advect_bulk(SweepParams& P, bool split, int sms, int user_chunk, cudaStream_t st) {
     static int occ[2][MAX_DEV] = {};
-    if (split) return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR, true>, occ[1], P, sms, user_chunk, st);
+    if (split) return launch_bulk_kernel<DIR, true>(ppm_advect_bulk_kernel<DIR, true>, occ[1], P, sms, user_chunk, st);
     return launch_bulk_kernel<DIR>(ppm_advect_bulk_kernel<DIR, false>, occ[0], P, sms, user_chunk, st);
 }
 template <int DIR>
