@@ -134,8 +134,8 @@ int ppm_reduce_conserved(ppm_ctx *ctx, double out[6]);
  * The array (6 * PPM_STATIC_RED_BLOCKS doubles = 48 KB) is held by every GPU that loads the library until the process
  * exits and is SHARED by every call on that GPU, whatever the context: calls that may overlap on the GPU (different
  * streams) race on it — order them.  It keeps the last call's contents; nothing in it has to start at zero (every slot
- * that is read was written by the same call).  The first call on a device looks the array's address up
- * (cudaGetSymbolAddress; no allocation by this library). */
+ * that is read was written by the same call).  ppm_create looks the array's address up for its device (cudaGetSymbolAddress; no
+ * allocation by this library), so the call itself only launches. */
 #define PPM_STATIC_RED_BLOCKS 1024
 int ppm_reduce_conserved_static(ppm_ctx *ctx, int nblocks, double *dev_out);
 

@@ -114,6 +114,7 @@ extern "C" int ppm_create(ppm_ctx** out, const ppm_params* prm, float* dev_buf_a
     CUC(cudaMalloc(&c->cflmax, sizeof(unsigned int)));
     CUC(cudaMalloc(&c->partial, sizeof(double) * 6 * c->nblocks_red));
     CUC(cudaMalloc(&c->result, sizeof(double) * 6));
+    ppm_static_scratch_prepare();     // set-up, this device current: the address of the static scratch array of ppm_reduce_conserved_static
     if (g.kind != PPM_GRAV_NONE) {
         std::vector<float4> t32(g.n);
         std::vector<double> t64(3 * (size_t)g.n);

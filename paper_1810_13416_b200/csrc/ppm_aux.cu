@@ -697,6 +697,13 @@ static cudaError_t static_partial_ptr(double** out) {
     return cudaSuccess;
 }
 
+// called by ppm_create with the context's device current: the look-up happens at set-up, outside any capture; should it fail
+// there, ppm_reduce_conserved_static tries again and reports the error
+void ppm_static_scratch_prepare() {
+    double* p = nullptr;
+    if (static_partial_ptr(&p) != cudaSuccess) cudaGetLastError();
+}
+
 // same two kernels, same assignment of cells to threads and the same reduction trees as ppm_launch_conserved: with
 // nb = c->nblocks_red the six sums come out bit for bit the same.  The caller made c's device current.
 cudaError_t ppm_launch_conserved_static(ppm_ctx* c, int nb, double* dev_out) {

@@ -113,6 +113,7 @@ cudaError_t ppm_launch_cfl(ppm_ctx* c);
 cudaError_t ppm_launch_flatten3d(ppm_ctx* c);
 cudaError_t ppm_launch_base_fill(ppm_ctx* c);    // fills R0c, P0c
 cudaError_t ppm_launch_conserved(ppm_ctx* c);
+void ppm_static_scratch_prepare();                 // looks the array's address up for the current device (never fails the caller)
 cudaError_t ppm_launch_conserved_static(ppm_ctx* c, int nblocks, double* dev_out);   // partial sums in a file-scope device array
 cudaError_t ppm_run_fma_peak(ppm_ctx* c, double* tflops);
 cudaError_t ppm_launch_spin_up(ppm_ctx* c, double domega);
