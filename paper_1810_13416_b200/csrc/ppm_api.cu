@@ -261,6 +261,7 @@ extern "C" int ppm_advect(ppm_ctx* c, double dt, int sweep_order) {
     if (!(dt > 0.0) || !isfinite(dt) || sweep_order < 0 || sweep_order > 5) { set_err(c, "ppm_advect: need finite dt > 0 and sweep_order in 0..5"); return PPM_EINVAL; }
     if (c->sphere) { set_err(c, "ppm_advect: the PPB-only mode has no confining sphere"); return PPM_EINVAL; }
     if (has_halo(c)) { set_err(c, "ppm_advect: not on a grid with PPM_BC_HALO faces"); return PPM_EINVAL; }
+    if (c->twof) c->cfl_valid = 0;      // two-fluid EOS: the sound speed depends on FV, which these sweeps move
     for (int s = 0; s < 3; ++s) CU(ppm_launch_sweep(c, ORDERS[sweep_order][s], dt, true));
     return PPM_OK;
 }

@@ -887,6 +887,34 @@ def test_two_fluid_ragged_grid_mixed_boundaries():
     g.close()
 
 
+def test_two_fluid_cfl_dt_sees_fv_moved_by_ppb_only_sweeps():
+    """with two gases the sound speed depends on FV: after PPB-only sweeps ppm_cfl_dt must not return the maximum cached
+    by the last full step (a one-cell spike of the stiffer gas spreads out, so the fastest signal slows down)"""
+    PPM = _gpu()
+    n = 16
+    f = np.zeros((15, n, n, n), dtype=np.float32)
+    f[0], f[4] = 1.0, 1.0
+    f[1] = 0.3                                            # uniform translation along x
+    f[5, 8, 8, 8] = 1.0
+    g = PPM(n, n, n, 1.0 / n, 1.2, (0,) * 6)
+    g.set_two_fluid(3.0, 1.2)
+    g.set_state(f)
+    dt = 0.2 * g.cfl_dt(0.8)
+    g.step(dt, 0)                                         # leaves the maximum of its final state on the device
+    dt_a = g.cfl_dt(0.8)
+    for k in range(6):
+        g.advect(dt, k % 6)
+    dt_b = g.cfl_dt(0.8)
+    st = g.get_state()
+    h = PPM(n, n, n, 1.0 / n, 1.2, (0,) * 6)
+    h.set_two_fluid(3.0, 1.2)
+    h.set_state(st)
+    assert dt_b == h.cfl_dt(0.8)
+    assert dt_b > dt_a * 1.0001
+    g.close()
+    h.close()
+
+
 def test_two_fluid_argument_checks():
     PPM = _gpu()
     from paper_1810_13416_b200.binding import OPT_FLATTEN3D
