@@ -31,6 +31,13 @@ def test_library_exports_every_declared_symbol(lib):
     assert declared == set(lib.EXPORTS)
 
 
+def test_binding_constants_match_header(lib):
+    hdr = open(os.path.join(ROOT, "include", "ppm.h")).read()
+    assert int(re.search(r"#define\s+PPM_STATIC_RED_BLOCKS\s+(\d+)", hdr).group(1)) == lib.STATIC_RED_BLOCKS
+    assert int(re.search(r"#define\s+PPM_NFIELDS\s+(\d+)", hdr).group(1)) == lib.NF
+    assert int(re.search(r"PPM_BC_HALO\s*=\s*(\d+)", hdr).group(1)) == lib.BC_HALO
+
+
 def test_struct_layout_matches_header(lib):
     # the ctypes mirror must agree with the C struct (struct_size is checked by ppm_create)
     assert C.sizeof(lib.ppm_gravity) == 72
@@ -103,6 +110,7 @@ def test_null_context_calls_return_einval(lib):
     assert L.ppm_cfl_dt(None, 0.8, C.byref(v)) == lib.PPM_EINVAL
     assert L.ppm_reduce_conserved(None, None) == lib.PPM_EINVAL
     assert L.ppm_sync(None) == lib.PPM_EINVAL
+    assert L.ppm_reduce_conserved_static(None, 0, None) == lib.PPM_EINVAL
     assert L.ppm_set_chunk(None, 4) == lib.PPM_EINVAL
     assert L.ppm_launch_count(None) == 0
     L.ppm_destroy(None)
